@@ -1,0 +1,185 @@
+/*
+ * nb.h — C ABI of libnb.so: the data-parallel hot path of the direct-summation Hermite-6
+ * block-time-step N-body method of arXiv:1411.5234 (Spera 2014, "HiGPUs" as template),
+ * implemented as hand-written CUDA for NVIDIA B200 (sm_100a).  One GPU per context.
+ *
+ * The method (citations are PAPER.md lines):
+ *   eq. (1)  r''_i = -G sum_{j != i} m_j r_ij / r_ij^3
+ *   eq. (2)  softened pair force  F = -G m_i m_j r_ij / (r_ij^2 + eps^2)^(3/2)
+ *   Hermite 6th-order integrator: Taylor-series predictor for all N, one pairwise evaluation
+ *   per step, corrector for the active particles
+ *   Block time steps: power-of-two steps, m <= N active particles per step,
+ *   cost O(mN) per step
+ * G = 1.  Everything the paper names without printing is fixed in DESIGN.md ("Readings").
+ *
+ * Conventions common to all calls
+ *   - fp64 throughout; indices are int32; sizes are int64.
+ *   - Vector arguments x, v, a, jerk, snap are row-major [n][3]; m, pot, t, dt are [n].
+ *   - Every pointer argument marked "(h/d)" is a HOST pointer if cfg->ptrs_on_device == 0 and a
+ *     DEVICE pointer (on cfg->device) if cfg->ptrs_on_device == 1.  The caller owns every buffer it
+ *     passes; the library neither frees nor retains them after the call returns, EXCEPT the
+ *     workspace, which the context uses until nb_free.
+ *   - All device memory lives in the caller-provided workspace (PyTorch is the allocator).
+ *   - Work is enqueued on cfg->stream.  With host pointers a call returns after its outputs have
+ *     arrived (it synchronises the stream); with device pointers calls are asynchronous.
+ *   - Return value: NB_OK (0) or a negative nb_status.  No exceptions, no exit(), nothing is
+ *     printed.  A context is not thread-safe.
+ */
+#ifndef NB_H
+#define NB_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nb_ctx nb_ctx; /* opaque: one particle system on one GPU */
+
+typedef enum {
+    NB_OK = 0,
+    NB_EINVAL = -1, /* bad argument: N < 1, eps < 0, NULL where not allowed, n_act out of range, bad level range */
+    NB_ENOMEM = -2, /* workspace missing, misaligned (< 256 B) or smaller than nb_workspace_bytes(N) */
+    NB_ESTATE = -3, /* call order: nb_force without nb_predict since the last state change, nb_corrector without nb_force */
+    NB_ECUDA = -4   /* a CUDA runtime call or kernel failed; nb_last_error(ctx) holds the CUDA message */
+} nb_status;
+
+typedef struct {
+    int device;             /* CUDA device ordinal */
+    void* stream;           /* cudaStream_t to enqueue on; NULL = the legacy default stream */
+    void* workspace;        /* DEVICE memory, 256-B aligned, >= nb_workspace_bytes(N) bytes, owned by the caller */
+    size_t workspace_bytes;
+    int ptrs_on_device;     /* 0: (h/d) pointers are host pointers; 1: device pointers */
+    double eta;             /* accuracy parameter of the time-step criterion (reading R11); 0 -> 0.45 */
+    double eta_s;           /* same, for the startup step dt = eta_s |a|/|jerk|;             0 -> 0.01 */
+    int k_min, k_max;       /* allowed levels: dt = 2^k, k_min <= k <= k_max; both 0 -> -20, -3 */
+} nb_config;
+
+/* Selectors of nb_get_state / nb_set_state.  Width = doubles per particle. */
+typedef enum {
+    NB_M = 0,   /* mass, 1 */
+    NB_X = 1,   /* position at t_i, 3 */
+    NB_V = 2,   /* velocity at t_i, 3 */
+    NB_A = 3,   /* acceleration at t_i, 3 */
+    NB_J = 4,   /* jerk  (da/dt), 3 */
+    NB_S = 5,   /* snap  (d2a/dt2), 3 */
+    NB_C = 6,   /* crackle (d3a/dt3, from the corrector's interpolant; 0 before the first step), 3 */
+    NB_T = 7,   /* particle time t_i, 1 */
+    NB_DT = 8,  /* particle step dt_i (a power of two), 1 */
+    NB_XP = 9,  /* predicted position at the time of the last nb_predict, 3 (get only) */
+    NB_VP = 10, /* predicted velocity, 3 (get only) */
+    NB_AP = 11  /* predicted acceleration, 3 (get only) */
+} nb_field;
+
+/* How nb_force maps an evaluation onto the GPU (reading R15; "Bfactor"). */
+typedef struct {
+    int kernel;       /* 0 = lanes-over-i (each thread owns I active particles, j-tiles broadcast from shared memory)
+                         1 = lanes-over-j (each warp owns I active particles, its lanes take different j) */
+    int n_units;      /* i-tiles (kernel 0) or i-groups per warp (kernel 1) */
+    int n_split;      /* S: number of j-slices each unit is split into ("Bfactor") */
+    int slice_tiles;  /* j-tiles per slice (the last slice may hold fewer) */
+    int grid;         /* CTAs launched */
+    double waves;     /* work items / resident CTAs (or warps) on the device */
+} nb_plan;
+
+/* Bytes of device workspace a context for N particles needs.  Pure; 0 if N < 1. */
+size_t nb_workspace_bytes(int64_t N);
+
+/* Pure host logic: the launch plan nb_force would use for n_act active particles out of N on a device
+ * with n_sm multiprocessors.  NB_EINVAL on bad sizes. */
+int nb_plan_force(int64_t N, int64_t n_act, int n_sm, nb_plan* plan);
+
+/*
+ * nb_init — create a system from the initial conditions of eq. (1): masses m[N],
+ * positions x[N][3], velocities v[N][3] (h/d), softening eps >= 0 of eq. (2).
+ * Copies the inputs, sets t_i = 0 and performs the startup (reading R8): one evaluation with a_j = 0
+ * to get a and jerk, a second with those a to get snap; crackle = 0; dt_i = eta_s |a|/|jerk| floored
+ * to a power of two in [2^k_min, 2^k_max].  eps = 0 is legal (eq. 1): coincident particles then give
+ * inf/NaN.  On success *ctx is a new context (host bookkeeping only); release with nb_free.
+ */
+int nb_init(nb_ctx** ctx, int64_t N, const double* m, const double* x, const double* v, double eps,
+            const nb_config* cfg);
+
+/*
+ * nb_predict — Taylor-extrapolate ALL N particles from their own t_i to time t (PAPER.md:58:
+ * "the kinematic state will be estimated using Taylor expansions"; orders per reading R6):
+ * x_p to 5th order, v_p to 4th, a_p to 3rd.  Fills the internal predicted j-records that
+ * nb_force streams.  t may be any time (also < t_i).
+ */
+int nb_predict(nb_ctx* ctx, double t);
+
+/*
+ * nb_force — the O(N n_act) pairwise evaluation (eq. 1-2 and their first two time
+ * derivatives, reading R3): for each active particle i = active_idx[k], over all j != i of the
+ * predicted records,
+ *   a = sum m_j dx / s^(3/2), jerk = da/dt, snap = d2a/dt2, pot = -sum m_j / s^(1/2),
+ *   s = |x_j - x_i|^2 + eps^2.
+ * active_idx (h/d): n_act unique int32 in [0, N), any order; NULL = all N in index order (then
+ * n_act must equal N).  Outputs (h/d), row k <-> active_idx[k]: a, jerk, snap [n_act][3], pot
+ * [n_act]; any may be NULL.  The results are also kept inside the context for nb_corrector.
+ * Small active sets are split over j-slices so that the whole GPU is used, and the
+ * partial sums are added in a fixed order: results are bitwise reproducible run to run.
+ * n_act == 0 is a no-op.  NB_ESTATE if no nb_predict since the last change of state.
+ */
+int nb_force(nb_ctx* ctx, const int32_t* active_idx, int64_t n_act,
+             double* a, double* jerk, double* snap, double* pot);
+
+/*
+ * nb_corrector — finish the Hermite-6 step (formulas: reading R10) for the active
+ * particles of the preceding nb_force (same active_idx, same n_act): corrects x and v with the
+ * two-point quintic Hermite quadrature, stores the new a, jerk, snap and the interpolant's crackle,
+ * sets t_i to the time of the last nb_predict.
+ *   dt > 0 : shared time step — every active particle steps h = dt; dt_i := dt.
+ *   dt <= 0: block time steps — h = dt_i; then the new power-of-two dt_i from the
+ *            6th-order Aarseth criterion (reading R11) under the block rule (reading R12).
+ * Invalidates the predicted records.
+ */
+int nb_corrector(nb_ctx* ctx, const int32_t* active_idx, int64_t n_act, double dt);
+
+/*
+ * nb_next_block — block scheduler: t_next = min_i (t_i + dt_i) and the active list
+ * { i : t_i + dt_i == t_next } in increasing index order.  t_next, n_act: HOST pointers always.
+ * active_idx (h/d): capacity N int32; may be NULL (then the list stays inside the context and
+ * nb_force / nb_corrector accept NB_ACTIVE_INTERNAL in its place).
+ */
+int nb_next_block(nb_ctx* ctx, double* t_next, int32_t* active_idx, int64_t* n_act);
+
+/* Pass as active_idx to use the list the last nb_next_block left inside the context. */
+#define NB_ACTIVE_INTERNAL ((const int32_t*)(uintptr_t)1)
+
+/* Read / write one field for the particles idx[0..n) (h/d; NULL = the first n in index order). */
+int nb_get_state(nb_ctx* ctx, int field, const int32_t* idx, int64_t n, double* out);
+int nb_set_state(nb_ctx* ctx, int field, const int32_t* idx, int64_t n, const double* in);
+
+/*
+ * nb_energy — kinetic and potential energy of the STORED state (x, v at t_i; meaningful when all
+ * t_i are equal): K = 1/2 sum m |v|^2, W = 1/2 sum m_i pot_i with pot from a full evaluation.
+ * kinetic, potential: HOST pointers always.  Invalidates the predicted records.
+ */
+int nb_energy(nb_ctx* ctx, double* kinetic, double* potential);
+
+/*
+ * nb_probe_fp64_peak — measurement aid: runs a register-resident chain of independent FP64 FMAs on
+ * every SM for about `seconds` and returns the sustained rate in TFLOP/s (FMA = 2 flop).  This is the
+ * measured denominator of the "fraction of FP64 peak" that bench.py reports.  workspace: >= 64 KiB
+ * of device memory.
+ */
+int nb_probe_fp64_peak(int device, void* stream, void* workspace, size_t workspace_bytes,
+                       double seconds, double* tflops, int* n_sm);
+
+/* Kernel launches issued by this context so far (what bench.py reports as gpu_launches). */
+int64_t nb_launch_count(const nb_ctx* ctx);
+
+/* Device time in ms of the force kernel(s) of the last nb_force (CUDA events on cfg->stream,
+ * excludes index upload and output copies); synchronises the stream.  < 0 on error. */
+double nb_last_force_ms(nb_ctx* ctx);
+
+const char* nb_strerror(int status);
+const char* nb_last_error(const nb_ctx* ctx); /* detail of the last NB_ECUDA of this context, "" if none */
+void nb_free(nb_ctx* ctx);                    /* host bookkeeping only; NULL is allowed */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NB_H */

@@ -1,0 +1,435 @@
+// nb_api.cu — the C ABI of include/nb.h: context, workspace carving, launch planning, call-order
+// checks.  No arithmetic of the method lives here; every step runs in the kernels of nb_force.cu
+// and nb_step.cu.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "nb_internal.h"
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t x, size_t a = ALIGN) { return (x + a - 1) / a * a; }
+inline int64_t pad_n(int64_t N) { return (N + NB_PAD - 1) / NB_PAD * NB_PAD; }
+inline int64_t partial_rows(int64_t Npad) { return 4 * Npad + (int64_t(1) << 19); }
+inline size_t scratch_bytes(int64_t Npad) { return 65536 + (size_t)Npad / 8; }
+
+struct Carve {
+    size_t off = 0;
+    char* base;
+    explicit Carve(void* b) : base((char*)b) {}
+    template <class T> T* take(size_t count) { T* p = (T*)(base + off); off = align_up(off + count * sizeof(T)); return p; }
+};
+
+// one place that defines the workspace layout, used for sizing (base = nullptr) and for carving
+struct Layout {
+    StateArrays s;
+    double *fa, *fj, *fs, *fp;          // force results, row k <-> active_idx[k]
+    double* partial;
+    int32_t *idx_user, *idx_sched, *idx_tmp;
+    double* stage;                      // staging for host <-> device transfers, 10 doubles per particle
+    char* scratch;
+    size_t bytes;
+    Layout(void* base, int64_t Npad)
+    {
+        Carve c(base);
+        s.st0 = c.take<double4>(Npad); s.st1 = c.take<double4>(Npad); s.st2 = c.take<double4>(Npad);
+        s.st3 = c.take<double4>(Npad); s.st4 = c.take<double4>(Npad); s.dt = c.take<double>(Npad);
+        s.pj0 = c.take<double4>(Npad); s.pj1 = c.take<double4>(Npad); s.pj2 = c.take<double2>(Npad);
+        fa = c.take<double>(3 * Npad); fj = c.take<double>(3 * Npad); fs = c.take<double>(3 * Npad); fp = c.take<double>(Npad);
+        partial = c.take<double>(10 * partial_rows(Npad));
+        idx_user = c.take<int32_t>(Npad); idx_sched = c.take<int32_t>(Npad); idx_tmp = c.take<int32_t>(Npad);
+        stage = c.take<double>(10 * Npad);
+        scratch = c.take<char>(scratch_bytes(Npad));
+        bytes = c.off;
+    }
+};
+
+}  // namespace
+
+struct nb_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    bool on_device = false;
+    int64_t N = 0, Npad = 0;
+    double eps = 0, eta = 0.45, eta_s = 0.01;
+    int k_min = -20, k_max = -3;
+    int n_sm = 148;
+    Layout L{nullptr, 0};
+    double t_pred = 0;
+    bool predicted = false;        // predicted records are valid
+    int64_t forced_n = -1;         // n_act of the last nb_force since the last predict (-1: none)
+    int64_t sched_n = -1;          // length of the internal active list (-1: none)
+    int64_t launches = 0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    bool ev_valid = false;
+    char err[256] = {0};
+};
+
+namespace {
+
+int fail_cuda(nb_ctx* c, cudaError_t e, const char* where)
+{
+    snprintf(c->err, sizeof c->err, "%s: %s", where, cudaGetErrorString(e));
+    return NB_ECUDA;
+}
+#define CU(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail_cuda(ctx, e_, where); } while (0)
+
+// device pointer to n_act indices: uploads a host list into `buf`, or passes a device list through
+int resolve_idx(nb_ctx* ctx, const int32_t* idx, int64_t n, int32_t* buf, const int32_t** out)
+{
+    if (idx == nullptr) { *out = nullptr; return NB_OK; }
+    if (idx == NB_ACTIVE_INTERNAL) {
+        if (ctx->sched_n < 0 || n != ctx->sched_n) return NB_ESTATE;
+        *out = ctx->L.idx_sched;
+        return NB_OK;
+    }
+    if (ctx->on_device) { *out = idx; return NB_OK; }
+    CU(cudaMemcpyAsync(buf, idx, n * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream), "upload active_idx");
+    *out = buf;
+    return NB_OK;
+}
+
+int copy_out(nb_ctx* ctx, double* dst, const double* src, size_t count)
+{
+    if (!dst) return NB_OK;
+    CU(cudaMemcpyAsync(dst, src, count * sizeof(double), ctx->on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
+                       ctx->stream), "copy result");
+    return NB_OK;
+}
+
+// Smallest-cost split: cost(S) = ceil(units*S / resident) * (slice_tiles + fixed), in j-tiles.
+void choose_split(int64_t n_units, int64_t n_tiles, int64_t resident, int64_t s_max, int fixed, nb_plan* p)
+{
+    int64_t best_S = 1, best_tiles = n_tiles;
+    double best_cost = 1e300;
+    s_max = std::max<int64_t>(1, std::min(s_max, n_tiles));
+    for (int64_t S = 1; S <= s_max; ++S) {
+        const int64_t st = (n_tiles + S - 1) / S;
+        const int64_t S_eff = (n_tiles + st - 1) / st;           // slices that are not empty
+        if (S_eff != S) continue;
+        const int64_t rounds = (n_units * S + resident - 1) / resident;
+        const double cost = (double)rounds * (double)(st + fixed);
+        if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best_S = S; best_tiles = st; }
+    }
+    p->n_split = (int)best_S;
+    p->slice_tiles = (int)best_tiles;
+    p->waves = (double)(n_units * best_S) / (double)resident;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t nb_workspace_bytes(int64_t N)
+{
+    if (N < 1) return 0;
+    return Layout(nullptr, pad_n(N)).bytes;
+}
+
+int nb_plan_force(int64_t N, int64_t n_act, int n_sm, nb_plan* plan)
+{
+    if (!plan || N < 1 || n_act < 1 || n_act > N || n_sm < 1 || N > (int64_t(1) << 30)) return NB_EINVAL;
+    const int64_t Npad = pad_n(N);
+    const int64_t rows = partial_rows(Npad);
+    nb_plan p{};
+    if (n_act <= LJ_MAX_ACT) {
+        // lanes-over-j: a work item is (warp i-group, j-slice); resident = warps on the device
+        p.kernel = 1;
+        p.n_units = (int)((n_act + LJ_I - 1) / LJ_I);
+        const int64_t n_tiles = Npad / LJ_TJ;
+        const int64_t resident = (int64_t)n_sm * LJ_CTAS_PER_SM * LJ_WARPS;
+        const int64_t s_cap = rows / ((int64_t)p.n_units * LJ_I);
+        choose_split(p.n_units, n_tiles, resident, std::min<int64_t>(s_cap, n_tiles / 4), 6, &p);
+        const int64_t items = (int64_t)p.n_units * p.n_split;
+        p.grid = (int)std::min<int64_t>((items + LJ_WARPS - 1) / LJ_WARPS, (int64_t)n_sm * LJ_CTAS_PER_SM);
+    } else {
+        // lanes-over-i: a work item is (i-tile of LI_UNIT particles, j-slice); resident = CTAs on the device
+        p.kernel = 0;
+        p.n_units = (int)((n_act + LI_UNIT - 1) / LI_UNIT);
+        const int64_t n_tiles = Npad / LI_TJ;
+        const int64_t resident = (int64_t)n_sm * LI_CTAS_PER_SM;
+        const int64_t s_cap = rows / ((int64_t)p.n_units * LI_UNIT);
+        choose_split(p.n_units, n_tiles, resident, std::min<int64_t>(s_cap, n_tiles / 2), 1, &p);
+        const int64_t items = (int64_t)p.n_units * p.n_split;
+        p.grid = (int)std::min<int64_t>(items, resident);
+    }
+    *plan = p;
+    return NB_OK;
+}
+
+int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const double* v, double eps, const nb_config* cfg)
+{
+    if (!out || !cfg || !m || !x || !v || N < 1 || N > (int64_t(1) << 30) || !(eps >= 0.0)) return NB_EINVAL;
+    const int k_min = (cfg->k_min == 0 && cfg->k_max == 0) ? -20 : cfg->k_min;
+    const int k_max = (cfg->k_min == 0 && cfg->k_max == 0) ? -3 : cfg->k_max;
+    if (k_min > k_max || k_min < -1000 || k_max > 1000 || cfg->eta < 0 || cfg->eta_s < 0) return NB_EINVAL;
+    const int64_t Npad = pad_n(N);
+    if (!cfg->workspace || ((uintptr_t)cfg->workspace % ALIGN) != 0 || cfg->workspace_bytes < Layout(nullptr, Npad).bytes)
+        return NB_ENOMEM;
+
+    nb_ctx* ctx = new (std::nothrow) nb_ctx();
+    if (!ctx) return NB_ENOMEM;
+    *out = ctx;                       // returned even on NB_ECUDA so that nb_last_error can be read; free with nb_free
+    ctx->device = cfg->device;
+    ctx->stream = (cudaStream_t)cfg->stream;
+    ctx->on_device = cfg->ptrs_on_device != 0;
+    ctx->N = N; ctx->Npad = Npad; ctx->eps = eps;
+    ctx->eta = cfg->eta > 0 ? cfg->eta : 0.45;
+    ctx->eta_s = cfg->eta_s > 0 ? cfg->eta_s : 0.01;
+    ctx->k_min = k_min; ctx->k_max = k_max;
+    ctx->L = Layout(cfg->workspace, Npad);
+
+    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    CU(cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, ctx->device), "device attribute");
+    CU(cudaEventCreate(&ctx->ev0), "event");
+    CU(cudaEventCreate(&ctx->ev1), "event");
+    CU(cudaMemsetAsync(ctx->L.scratch, 0, scratch_bytes(Npad), ctx->stream), "memset scratch");
+
+    const double *dm = m, *dx = x, *dv = v;
+    if (!ctx->on_device) {
+        double* st = ctx->L.stage;
+        CU(cudaMemcpyAsync(st, m, N * sizeof(double), cudaMemcpyHostToDevice, ctx->stream), "upload m");
+        CU(cudaMemcpyAsync(st + Npad, x, 3 * N * sizeof(double), cudaMemcpyHostToDevice, ctx->stream), "upload x");
+        CU(cudaMemcpyAsync(st + 4 * Npad, v, 3 * N * sizeof(double), cudaMemcpyHostToDevice, ctx->stream), "upload v");
+        dm = st; dx = st + Npad; dv = st + 4 * Npad;
+    }
+    CU(nb_launch_init_state(ctx->L.s, N, Npad, dm, dx, dv, ctx->stream), "init_state");
+    ctx->launches += 1;
+
+    // startup (reading R8): two all-active evaluations at t = 0
+    for (int pass = 1; pass <= 2; ++pass) {
+        CU(nb_launch_predict(ctx->L.s, N, 0.0, true, ctx->stream), "predict");
+        ctx->launches += 1;
+        ctx->predicted = true; ctx->t_pred = 0.0;
+        const int rc = nb_force(ctx, nullptr, N, nullptr, nullptr, nullptr, nullptr);
+        if (rc != NB_OK) return rc;
+        CU(nb_launch_startup(ctx->L.s, N, ctx->L.fa, ctx->L.fj, ctx->L.fs, pass, ctx->eta_s, k_min, k_max, ctx->stream), "startup");
+        ctx->launches += 1;
+    }
+    ctx->predicted = false; ctx->forced_n = -1;
+    if (!ctx->on_device) CU(cudaStreamSynchronize(ctx->stream), "nb_init");
+    return NB_OK;
+}
+
+int nb_predict(nb_ctx* ctx, double t)
+{
+    if (!ctx || !std::isfinite(t)) return NB_EINVAL;
+    CU(nb_launch_predict(ctx->L.s, ctx->N, t, false, ctx->stream), "predict");
+    ctx->launches += 1;
+    ctx->t_pred = t; ctx->predicted = true; ctx->forced_n = -1;
+    return NB_OK;
+}
+
+int nb_force(nb_ctx* ctx, const int32_t* active_idx, int64_t n_act, double* a, double* jerk, double* snap, double* pot)
+{
+    if (!ctx || n_act < 0 || n_act > ctx->N) return NB_EINVAL;
+    if (active_idx == nullptr && n_act != 0 && n_act != ctx->N) return NB_EINVAL;
+    if (!ctx->predicted) return NB_ESTATE;
+    if (n_act == 0) { ctx->forced_n = 0; return NB_OK; }
+
+    const int32_t* didx = nullptr;
+    int rc = resolve_idx(ctx, active_idx, n_act, ctx->L.idx_user, &didx);
+    if (rc != NB_OK) return rc;
+
+    nb_plan plan;
+    rc = nb_plan_force(ctx->N, n_act, ctx->n_sm, &plan);
+    if (rc != NB_OK) return rc;
+
+    ForceArgs A{};
+    A.pj0 = ctx->L.s.pj0; A.pj1 = ctx->L.s.pj1; A.pj2 = ctx->L.s.pj2;
+    A.idx = didx;
+    A.n_act = (int)n_act;
+    A.n_units = plan.n_units; A.n_split = plan.n_split; A.slice_tiles = plan.slice_tiles;
+    A.n_tiles = (int)(ctx->Npad / (plan.kernel == 0 ? LI_TJ : LJ_TJ));
+    A.n_items = plan.n_units * plan.n_split;
+    A.ld = plan.n_units * (plan.kernel == 0 ? LI_UNIT : LJ_I);
+    A.eps2 = ctx->eps * ctx->eps;
+    A.partial = ctx->L.partial;
+    A.out_a = ctx->L.fa; A.out_j = ctx->L.fj; A.out_s = ctx->L.fs; A.out_p = ctx->L.fp;
+
+    int launches = 0;
+    CU(cudaEventRecord(ctx->ev0, ctx->stream), "event record");
+    CU(nb_launch_force(plan, A, ctx->eps == 0.0, ctx->stream, &launches), "force kernel");
+    CU(cudaEventRecord(ctx->ev1, ctx->stream), "event record");
+    ctx->ev_valid = true;
+    ctx->launches += launches;
+    ctx->forced_n = n_act;
+
+    if ((rc = copy_out(ctx, a, ctx->L.fa, 3 * n_act)) != NB_OK) return rc;
+    if ((rc = copy_out(ctx, jerk, ctx->L.fj, 3 * n_act)) != NB_OK) return rc;
+    if ((rc = copy_out(ctx, snap, ctx->L.fs, 3 * n_act)) != NB_OK) return rc;
+    if ((rc = copy_out(ctx, pot, ctx->L.fp, n_act)) != NB_OK) return rc;
+    if (!ctx->on_device) CU(cudaStreamSynchronize(ctx->stream), "nb_force");
+    return NB_OK;
+}
+
+int nb_corrector(nb_ctx* ctx, const int32_t* active_idx, int64_t n_act, double dt)
+{
+    if (!ctx || n_act < 0 || n_act > ctx->N || !(dt == dt)) return NB_EINVAL;
+    if (active_idx == nullptr && n_act != 0 && n_act != ctx->N) return NB_EINVAL;
+    if (ctx->forced_n < 0 || ctx->forced_n != n_act) return NB_ESTATE;
+    if (n_act > 0) {
+        const int32_t* didx = nullptr;
+        const int rc = resolve_idx(ctx, active_idx, n_act, ctx->L.idx_user, &didx);
+        if (rc != NB_OK) return rc;
+        CU(nb_launch_corrector(ctx->L.s, didx, n_act, dt, ctx->t_pred, ctx->L.fa, ctx->L.fj, ctx->L.fs, ctx->eta, ctx->k_min,
+                               ctx->k_max, ctx->stream), "corrector");
+        ctx->launches += 1;
+    }
+    ctx->predicted = false; ctx->forced_n = -1; ctx->sched_n = -1;
+    if (!ctx->on_device) CU(cudaStreamSynchronize(ctx->stream), "nb_corrector");
+    return NB_OK;
+}
+
+int nb_next_block(nb_ctx* ctx, double* t_next, int32_t* active_idx, int64_t* n_act)
+{
+    if (!ctx || !t_next || !n_act) return NB_EINVAL;
+    int launches = 0;
+    CU(nb_launch_next_block(ctx->L.s, ctx->N, ctx->L.idx_sched, ctx->L.scratch, ctx->stream, &launches), "scheduler");
+    ctx->launches += launches;
+    struct { double t; long long n; } res;
+    CU(cudaMemcpyAsync(&res, ctx->L.scratch, sizeof res, cudaMemcpyDeviceToHost, ctx->stream), "scheduler result");
+    CU(cudaStreamSynchronize(ctx->stream), "nb_next_block");
+    *t_next = res.t; *n_act = res.n; ctx->sched_n = res.n;
+    if (active_idx && res.n > 0) {
+        CU(cudaMemcpyAsync(active_idx, ctx->L.idx_sched, res.n * sizeof(int32_t),
+                           ctx->on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream), "active list");
+        if (!ctx->on_device) CU(cudaStreamSynchronize(ctx->stream), "nb_next_block");
+    }
+    return NB_OK;
+}
+
+static int field_width_host(int f) { return (f == NB_M || f == NB_T || f == NB_DT) ? 1 : 3; }
+
+int nb_get_state(nb_ctx* ctx, int field, const int32_t* idx, int64_t n, double* out)
+{
+    if (!ctx || !out || n < 0 || n > ctx->N || field < NB_M || field > NB_AP) return NB_EINVAL;
+    if (n == 0) return NB_OK;
+    const int32_t* didx = nullptr;
+    const int rc = resolve_idx(ctx, idx, n, ctx->L.idx_tmp, &didx);
+    if (rc != NB_OK) return rc;
+    const size_t count = (size_t)n * field_width_host(field);
+    double* dst = ctx->on_device ? out : ctx->L.stage;
+    CU(nb_launch_get(ctx->L.s, field, didx, n, dst, ctx->stream), "get_state");
+    ctx->launches += 1;
+    if (!ctx->on_device) {
+        CU(cudaMemcpyAsync(out, dst, count * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream), "get_state copy");
+        CU(cudaStreamSynchronize(ctx->stream), "nb_get_state");
+    }
+    return NB_OK;
+}
+
+int nb_set_state(nb_ctx* ctx, int field, const int32_t* idx, int64_t n, const double* in)
+{
+    if (!ctx || !in || n < 0 || n > ctx->N || field < NB_M || field > NB_DT) return NB_EINVAL;
+    if (n == 0) return NB_OK;
+    const int32_t* didx = nullptr;
+    const int rc = resolve_idx(ctx, idx, n, ctx->L.idx_tmp, &didx);
+    if (rc != NB_OK) return rc;
+    const size_t count = (size_t)n * field_width_host(field);
+    const double* src = in;
+    if (!ctx->on_device) {
+        CU(cudaMemcpyAsync(ctx->L.stage, in, count * sizeof(double), cudaMemcpyHostToDevice, ctx->stream), "set_state copy");
+        src = ctx->L.stage;
+    }
+    CU(nb_launch_set(ctx->L.s, field, didx, n, src, ctx->stream), "set_state");
+    ctx->launches += 1;
+    ctx->predicted = false; ctx->forced_n = -1; ctx->sched_n = -1;
+    if (!ctx->on_device) CU(cudaStreamSynchronize(ctx->stream), "nb_set_state");
+    return NB_OK;
+}
+
+int nb_energy(nb_ctx* ctx, double* kinetic, double* potential)
+{
+    if (!ctx || !kinetic || !potential) return NB_EINVAL;
+    CU(nb_launch_predict(ctx->L.s, ctx->N, 0.0, true, ctx->stream), "predict");
+    ctx->launches += 1;
+    ctx->predicted = true;
+    const bool od = ctx->on_device;
+    ctx->on_device = true;                                  // no copies, no sync inside nb_force
+    const int rc = nb_force(ctx, nullptr, ctx->N, nullptr, nullptr, nullptr, nullptr);
+    ctx->on_device = od;
+    if (rc != NB_OK) return rc;
+    int launches = 0;
+    CU(nb_launch_energy(ctx->L.s, ctx->N, ctx->L.fp, (double*)ctx->L.scratch + 16, ctx->stream, &launches), "energy");
+    ctx->launches += launches;
+    double res[2];
+    CU(cudaMemcpyAsync(res, (double*)ctx->L.scratch + 16, sizeof res, cudaMemcpyDeviceToHost, ctx->stream), "energy result");
+    CU(cudaStreamSynchronize(ctx->stream), "nb_energy");
+    *kinetic = res[0]; *potential = res[1];
+    ctx->predicted = false; ctx->forced_n = -1;
+    return NB_OK;
+}
+
+int nb_probe_fp64_peak(int device, void* stream, void* workspace, size_t workspace_bytes, double seconds, double* tflops, int* n_sm_out)
+{
+    if (!workspace || workspace_bytes < 65536 || !tflops || !(seconds > 0)) return NB_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    int n_sm = 0;
+    if (cudaSetDevice(device) != cudaSuccess) return NB_ECUDA;
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return NB_ECUDA;
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return NB_ECUDA;
+    const double flop_per_iter = (double)n_sm * 4 * 256 * 16 * 8 * 2;
+    int iters = 20000;
+    float ms = 0;
+    double best = 0;
+    int rc = NB_OK;
+    // calibrate, then run back-to-back launches of ~0.25 s until `seconds` have elapsed
+    for (int round = 0; round < 2 && rc == NB_OK; ++round) {
+        double elapsed = 0;
+        do {
+            cudaEventRecord(e0, st);
+            if (nb_launch_fp64_probe((double*)workspace, n_sm, iters, st) != cudaSuccess) { rc = NB_ECUDA; break; }
+            cudaEventRecord(e1, st);
+            if (cudaEventSynchronize(e1) != cudaSuccess || cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) { rc = NB_ECUDA; break; }
+            elapsed += ms * 1e-3;
+            if (round == 1) best = flop_per_iter * iters / (ms * 1e-3) * 1e-12;   // the LAST launch: sustained, not burst
+        } while (round == 1 && elapsed < seconds);
+        if (round == 0 && ms > 0) iters = std::max(1000, (int)(iters * 250.0 / ms));
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    if (rc != NB_OK) return rc;
+    *tflops = best;
+    if (n_sm_out) *n_sm_out = n_sm;
+    return NB_OK;
+}
+
+int64_t nb_launch_count(const nb_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+double nb_last_force_ms(nb_ctx* ctx)
+{
+    if (!ctx || !ctx->ev_valid) return -1.0;
+    float ms = 0;
+    if (cudaEventSynchronize(ctx->ev1) != cudaSuccess) return -1.0;
+    if (cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1) != cudaSuccess) return -1.0;
+    return (double)ms;
+}
+
+const char* nb_strerror(int status)
+{
+    switch (status) {
+        case NB_OK: return "ok";
+        case NB_EINVAL: return "invalid argument";
+        case NB_ENOMEM: return "workspace missing, misaligned or too small";
+        case NB_ESTATE: return "call order: nb_predict -> nb_force -> nb_corrector";
+        case NB_ECUDA: return "CUDA error (see nb_last_error)";
+        default: return "unknown status";
+    }
+}
+
+const char* nb_last_error(const nb_ctx* ctx) { return ctx ? ctx->err : ""; }
+
+void nb_free(nb_ctx* ctx)
+{
+    if (!ctx) return;
+    if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+    if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    delete ctx;
+}
+
+}  // extern "C"

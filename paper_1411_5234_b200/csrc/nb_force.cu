@@ -1,0 +1,296 @@
+// nb_force.cu — the pairwise evaluation: acceleration, jerk, snap and
+// potential of eq. (1)-(2) and their time derivatives (R3), for
+// the active particles against all N predicted j-records.  fp64 on the FP64 ALU pipe; tensor cores
+// are not used (no dense contraction).  Two kernel shapes, both writing per-slice partial sums
+// that a third kernel adds in slice order (the "Bfactor" j-split of PAPER.md:59-65, made
+// deterministic):
+//   force_li_kernel  lanes-over-i: a thread owns LI_I active particles in registers; the CTA
+//                    streams j-tiles into shared memory with 1-D TMA bulk copies (UBLKCP) signalled
+//                    on mbarriers, double-buffered; every lane reads the same j-record (broadcast LDS).
+//   force_lj_kernel  lanes-over-j: a warp owns LJ_I active particles (same in every lane); its 32
+//                    lanes read 32 different j-records straight from global memory (coalesced) and
+//                    the ten sums per particle are combined with a warp-shuffle butterfly.
+#include "nb_internal.h"
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------
+// One pair.  54 FP64-pipe instructions (32 DFMA + 11 DMUL + 11 DADD) + 1 MUFU.RSQ64H.
+// ---------------------------------------------------------------------------------------------
+struct Sums { double ax, ay, az, jx, jy, jz, sx, sy, sz, p; };
+
+struct IPart { double x, y, z, vx, vy, vz, ax, ay, az; };
+
+// fp64 reciprocal-square-root seed: MUFU.RSQ64H works on the high word only (about 20 good bits).
+__device__ __forceinline__ double rsqrt_seed(double s)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(s));
+    return y;
+}
+
+template <bool EPS0>
+__device__ __forceinline__ void pair(const IPart& pi, const double4 p0, const double4 p1, const double2 p2,
+                                     const double eps2, const bool self, Sums& S)
+{
+    const double dx = p0.x - pi.x, dy = p0.y - pi.y, dz = p0.z - pi.z;
+    const double dvx = p1.x - pi.vx, dvy = p1.y - pi.vy, dvz = p1.z - pi.vz;
+    const double dax = p1.w - pi.ax, day = p2.x - pi.ay, daz = p2.y - pi.az;
+    double s = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+    if (EPS0) s = self ? 1.0 : s;                        // eps = 0: keep the masked self pair finite
+    // y = s^(-1/2): seed e0 ~ 2^-20, one cubic (Halley) step leaves 5/16 e0^3 < 2^-60
+    const double y0 = rsqrt_seed(s);
+    const double e = fma(-s, y0 * y0, 1.0);
+    const double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);
+    const double rv = fma(dx, dvx, fma(dy, dvy, dz * dvz));                           // dx.dv
+    const double B = fma(dx, dax, fma(dy, day, fma(dz, daz, fma(dvx, dvx, fma(dvy, dvy, dvz * dvz)))));  // dv.dv + dx.da
+    const double yy = y * y;                             // 1/s
+    const double z = -3.0 * yy;
+    const double mr = p0.w * y;                          // m_j / sqrt(s)
+    const double q = mr * yy;                            // m_j s^(-3/2)
+    const double alpha = rv * yy;
+    const double c1 = rv * z;                            // -3 alpha
+    const double c3 = fma(c1, alpha, B * z);             // -3 beta = -3 (B/s + alpha^2)
+    const double c2 = c1 + c1;                           // -6 alpha
+    const double ux = fma(c1, dx, dvx), uy = fma(c1, dy, dvy), uz = fma(c1, dz, dvz);      // dv - 3 alpha dx
+    const double wx = fma(c3, dx, fma(c2, ux, dax));     // da - 6 alpha u - 3 beta dx
+    const double wy = fma(c3, dy, fma(c2, uy, day));
+    const double wz = fma(c3, dz, fma(c2, uz, daz));
+    S.ax = fma(q, dx, S.ax); S.ay = fma(q, dy, S.ay); S.az = fma(q, dz, S.az);
+    S.jx = fma(q, ux, S.jx); S.jy = fma(q, uy, S.jy); S.jz = fma(q, uz, S.jz);
+    S.sx = fma(q, wx, S.sx); S.sy = fma(q, wy, S.sy); S.sz = fma(q, wz, S.sz);
+    S.p += self ? 0.0 : mr;                              // j != i (eq. 1); a, jerk, snap get exactly 0 from the self pair
+}
+
+__device__ __forceinline__ IPart load_ipart(const ForceArgs& A, int i)
+{
+    const double4 a = A.pj0[i], b = A.pj1[i];
+    const double2 c = A.pj2[i];
+    return IPart{a.x, a.y, a.z, b.x, b.y, b.z, b.w, c.x, c.y};
+}
+
+__device__ __forceinline__ void store_sums(const ForceArgs& A, int slice, int k, bool valid, const Sums& S)
+{
+    if (A.n_split > 1) {
+        double* P = A.partial + (size_t)slice * 10 * A.ld + k;      // plane (slice, c) is contiguous in k
+        const size_t ld = A.ld;
+        P[0] = S.ax; P[ld] = S.ay; P[2 * ld] = S.az;
+        P[3 * ld] = S.jx; P[4 * ld] = S.jy; P[5 * ld] = S.jz;
+        P[6 * ld] = S.sx; P[7 * ld] = S.sy; P[8 * ld] = S.sz; P[9 * ld] = S.p;
+    } else if (valid) {
+        A.out_a[3 * k] = S.ax; A.out_a[3 * k + 1] = S.ay; A.out_a[3 * k + 2] = S.az;
+        A.out_j[3 * k] = S.jx; A.out_j[3 * k + 1] = S.jy; A.out_j[3 * k + 2] = S.jz;
+        A.out_s[3 * k] = S.sx; A.out_s[3 * k + 1] = S.sy; A.out_s[3 * k + 2] = S.sz;
+        A.out_p[k] = -S.p;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// mbarrier / TMA bulk-copy helpers (PTX; SASS: SYNCS.*, UBLKCP)
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\t"
+                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                     "selp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    } while (!done);
+}
+
+// ---------------------------------------------------------------------------------------------
+// lanes-over-i
+// ---------------------------------------------------------------------------------------------
+static_assert((LI_STAGES & (LI_STAGES - 1)) == 0, "LI_STAGES must be a power of two");
+
+template <bool EPS0>
+__global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(const ForceArgs A)
+{
+    __shared__ alignas(128) double4 s0[LI_STAGES][LI_TJ];
+    __shared__ alignas(128) double4 s1[LI_STAGES][LI_TJ];
+    __shared__ alignas(128) double2 s2[LI_STAGES][LI_TJ];
+    __shared__ alignas(8) unsigned long long full[LI_STAGES];
+
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        for (int s = 0; s < LI_STAGES; ++s) mbar_init(smem_u32(&full[s]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // one elected thread stages j-tile `tile` into stage `st`: three bulk copies, one barrier
+    auto stage_tile = [&](int tile, int st) {
+        const uint32_t bar = smem_u32(&full[st]);
+        const size_t j0 = (size_t)tile * LI_TJ;
+        mbar_expect_tx(bar, LI_TJ * 80);
+        bulk_g2s(smem_u32(&s0[st][0]), A.pj0 + j0, LI_TJ * 32, bar);
+        bulk_g2s(smem_u32(&s1[st][0]), A.pj1 + j0, LI_TJ * 32, bar);
+        bulk_g2s(smem_u32(&s2[st][0]), A.pj2 + j0, LI_TJ * 16, bar);
+    };
+
+    uint32_t uses = 0;   // j-tiles this CTA has consumed so far: stage = uses % STAGES, parity = (uses / STAGES) & 1
+    for (int item = blockIdx.x; item < A.n_items; item += gridDim.x) {
+        const int unit = item % A.n_units, slice = item / A.n_units;
+        const int t0 = slice * A.slice_tiles;
+        const int nt = min(A.slice_tiles, A.n_tiles - t0);
+
+        if (tid == 0)
+            for (int f = 0; f < LI_STAGES && f < nt; ++f) stage_tile(t0 + f, (uses + f) & (LI_STAGES - 1));
+
+        int ii[LI_I];
+        bool valid[LI_I];
+        IPart pi[LI_I];
+        Sums acc[LI_I];
+#pragma unroll
+        for (int q = 0; q < LI_I; ++q) {
+            const int k = unit * LI_UNIT + q * LI_THREADS + tid;
+            valid[q] = k < A.n_act;
+            const int kk = valid[q] ? k : 0;
+            ii[q] = A.idx ? A.idx[kk] : kk;
+            pi[q] = load_ipart(A, ii[q]);
+            acc[q] = Sums{0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+        }
+
+        for (int t = 0; t < nt; ++t) {
+            const uint32_t u = uses + t;
+            const int st = u & (LI_STAGES - 1);
+            mbar_wait(smem_u32(&full[st]), (u / LI_STAGES) & 1);
+            const int jbase = (t0 + t) * LI_TJ;
+#pragma unroll 2
+            for (int jj = 0; jj < LI_TJ; ++jj) {
+                const double4 p0 = s0[st][jj], p1 = s1[st][jj];
+                const double2 p2 = s2[st][jj];
+#pragma unroll
+                for (int q = 0; q < LI_I; ++q) pair<EPS0>(pi[q], p0, p1, p2, A.eps2, jbase + jj == ii[q], acc[q]);
+            }
+            __syncthreads();                                   // every warp is done with stage st
+            if (tid == 0 && t + LI_STAGES < nt) stage_tile(t0 + t + LI_STAGES, st);
+        }
+        uses += nt;
+
+#pragma unroll
+        for (int q = 0; q < LI_I; ++q) store_sums(A, slice, unit * LI_UNIT + q * LI_THREADS + tid, valid[q], acc[q]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// lanes-over-j
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+template <bool EPS0>
+__global__ void __launch_bounds__(LJ_THREADS, LJ_CTAS_PER_SM) force_lj_kernel(const ForceArgs A)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int wi = blockIdx.x * LJ_WARPS + warp; wi < A.n_items; wi += gridDim.x * LJ_WARPS) {
+        const int unit = wi % A.n_units, slice = wi / A.n_units;
+        const int t0 = slice * A.slice_tiles;
+        const int nt = min(A.slice_tiles, A.n_tiles - t0);
+
+        int ii[LJ_I];
+        bool valid[LJ_I];
+        IPart pi[LJ_I];
+        Sums acc[LJ_I];
+#pragma unroll
+        for (int q = 0; q < LJ_I; ++q) {
+            const int k = unit * LJ_I + q;
+            valid[q] = k < A.n_act;
+            const int kk = valid[q] ? k : 0;
+            ii[q] = A.idx ? A.idx[kk] : kk;
+            pi[q] = load_ipart(A, ii[q]);
+            acc[q] = Sums{0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+        }
+
+        int j = t0 * LJ_TJ + lane;
+        double4 n0 = A.pj0[j], n1 = A.pj1[j];
+        double2 n2 = A.pj2[j];
+        for (int t = 0; t < nt; ++t) {
+            const double4 p0 = n0, p1 = n1;
+            const double2 p2 = n2;
+            if (t + 1 < nt) { n0 = A.pj0[j + LJ_TJ]; n1 = A.pj1[j + LJ_TJ]; n2 = A.pj2[j + LJ_TJ]; }   // prefetch
+#pragma unroll
+            for (int q = 0; q < LJ_I; ++q) pair<EPS0>(pi[q], p0, p1, p2, A.eps2, j == ii[q], acc[q]);
+            j += LJ_TJ;
+        }
+
+#pragma unroll
+        for (int q = 0; q < LJ_I; ++q) {
+            Sums& S = acc[q];
+            S.ax = warp_sum(S.ax); S.ay = warp_sum(S.ay); S.az = warp_sum(S.az);
+            S.jx = warp_sum(S.jx); S.jy = warp_sum(S.jy); S.jz = warp_sum(S.jz);
+            S.sx = warp_sum(S.sx); S.sy = warp_sum(S.sy); S.sz = warp_sum(S.sz);
+            S.p = warp_sum(S.p);
+            if (lane == 0) store_sums(A, slice, unit * LJ_I + q, valid[q], S);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// partial-sum reduction: one thread per active particle, slices added in increasing order
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) reduce_partials_kernel(const ForceArgs A)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= A.n_act) return;
+    double r[10];
+#pragma unroll
+    for (int c = 0; c < 10; ++c) r[c] = 0.0;
+    const double* P = A.partial + k;
+    for (int s = 0; s < A.n_split; ++s, P += (size_t)10 * A.ld) {
+#pragma unroll
+        for (int c = 0; c < 10; ++c) r[c] += P[(size_t)c * A.ld];
+    }
+    A.out_a[3 * k] = r[0]; A.out_a[3 * k + 1] = r[1]; A.out_a[3 * k + 2] = r[2];
+    A.out_j[3 * k] = r[3]; A.out_j[3 * k + 1] = r[4]; A.out_j[3 * k + 2] = r[5];
+    A.out_s[3 * k] = r[6]; A.out_s[3 * k + 1] = r[7]; A.out_s[3 * k + 2] = r[8];
+    A.out_p[k] = -r[9];
+}
+
+}  // namespace
+
+cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps_is_zero, cudaStream_t st, int* launches)
+{
+    if (plan.kernel == 0) {
+        if (eps_is_zero) force_li_kernel<true><<<plan.grid, LI_THREADS, 0, st>>>(args);
+        else             force_li_kernel<false><<<plan.grid, LI_THREADS, 0, st>>>(args);
+    } else {
+        if (eps_is_zero) force_lj_kernel<true><<<plan.grid, LJ_THREADS, 0, st>>>(args);
+        else             force_lj_kernel<false><<<plan.grid, LJ_THREADS, 0, st>>>(args);
+    }
+    ++*launches;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if (plan.n_split > 1) {
+        reduce_partials_kernel<<<(args.n_act + 127) / 128, 128, 0, st>>>(args);
+        ++*launches;
+        e = cudaGetLastError();
+    }
+    return e;
+}
+
+void nb_force_occupancy(int* li, int* lj)
+{
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(li, force_li_kernel<false>, LI_THREADS, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(lj, force_lj_kernel<false>, LJ_THREADS, 0);
+}

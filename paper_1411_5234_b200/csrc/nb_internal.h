@@ -1,0 +1,65 @@
+// nb_internal.h — declarations shared by the translation units of libnb.so (CUDA path only).
+// Data layout in HBM:
+//   state, 5 arrays of double4 (one 32-B sector each per particle, so gathers by active index use
+//   whole sectors and the predictor reads exactly the 160 B it needs):
+//     st0 = (x, y, z, m)   st1 = (vx, vy, vz, t)   st2 = (ax, ay, az, jx)
+//     st3 = (jy, jz, sx, sy)   st4 = (sz, cx, cy, cz)           + dt[N]
+//   predicted j-records, 80 B per particle, three contiguous arrays so a j-tile is three bulk copies:
+//     pj0 = (xp, yp, zp, m)   pj1 = (vxp, vyp, vzp, axp)   pj2 = (ayp, azp)
+//   padded to a multiple of NB_PAD particles with massless records far away (contribute exactly 0).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "nb.h"
+
+constexpr int NB_PAD = 256;          // particle arrays are padded to a multiple of this
+
+// lanes-over-i kernel: each thread owns LI_I active particles, a CTA streams j-tiles through smem
+constexpr int LI_THREADS = 128;
+constexpr int LI_I = 2;
+constexpr int LI_UNIT = LI_THREADS * LI_I;   // active particles per i-tile
+constexpr int LI_TJ = 128;                   // j-records per smem stage (10 KB)
+constexpr int LI_STAGES = 2;
+constexpr int LI_CTAS_PER_SM = 3;
+// lanes-over-j kernel: each warp owns LJ_I active particles, lanes take different j
+constexpr int LJ_THREADS = 128;
+constexpr int LJ_WARPS = LJ_THREADS / 32;
+constexpr int LJ_I = 2;
+constexpr int LJ_TJ = 32;                    // j-records per warp iteration
+constexpr int LJ_CTAS_PER_SM = 3;
+constexpr int64_t LJ_MAX_ACT = 1024;         // n_act <= this -> lanes-over-j
+
+struct ForceArgs {
+    const double4* pj0; const double4* pj1; const double2* pj2;   // predicted records (padded)
+    const int32_t* idx;      // active indices or nullptr (i = k)
+    int n_act;
+    int n_units;             // i-tiles (LI) or warp i-groups (LJ)
+    int n_split;             // S
+    int slice_tiles;         // j-tiles per slice
+    int n_tiles;             // total j-tiles (Npad / TJ)
+    int n_items;             // n_units * n_split
+    int ld;                  // rows of the partial buffer per (slice, component) plane
+    double eps2;
+    double* partial;         // [S][10][ld] when S > 1
+    double* out_a; double* out_j; double* out_s; double* out_p;   // [n_act][3] x3, [n_act]
+};
+
+// nb_force.cu
+cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps_is_zero, cudaStream_t st, int* launches);
+void nb_force_occupancy(int* li_ctas_per_sm, int* lj_ctas_per_sm);
+
+// nb_step.cu
+struct StateArrays { double4 *st0, *st1, *st2, *st3, *st4; double* dt; double4 *pj0, *pj1; double2* pj2; };
+cudaError_t nb_launch_init_state(const StateArrays& s, int64_t N, int64_t Npad, const double* m, const double* x, const double* v, cudaStream_t st);
+cudaError_t nb_launch_predict(const StateArrays& s, int64_t N, double t, bool own_time, cudaStream_t st);
+cudaError_t nb_launch_startup(const StateArrays& s, int64_t N, const double* fa, const double* fj, const double* fs, int pass,
+                              double eta_s, int k_min, int k_max, cudaStream_t st);
+cudaError_t nb_launch_corrector(const StateArrays& s, const int32_t* idx, int64_t n_act, double dt_shared, double t_new,
+                                const double* fa, const double* fj, const double* fs,
+                                double eta, int k_min, int k_max, cudaStream_t st);
+cudaError_t nb_launch_get(const StateArrays& s, int field, const int32_t* idx, int64_t n, double* out, cudaStream_t st);
+cudaError_t nb_launch_set(const StateArrays& s, int field, const int32_t* idx, int64_t n, const double* in, cudaStream_t st);
+// scheduler: scratch = >= 64 KiB; result: scratch_out[0] = t_next (double), ((int64*)scratch_out)[1] = n_act
+cudaError_t nb_launch_next_block(const StateArrays& s, int64_t N, int32_t* active, void* scratch, cudaStream_t st, int* launches);
+cudaError_t nb_launch_energy(const StateArrays& s, int64_t N, const double* pot, double* scratch, cudaStream_t st, int* launches);
+cudaError_t nb_launch_fp64_probe(double* out, int n_sm, int iters, cudaStream_t st);

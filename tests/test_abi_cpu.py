@@ -1,0 +1,113 @@
+"""CPU-only checks of the boundary: libnb.so builds for sm_100a, loads, exports every symbol that
+include/nb.h declares, and its pure host logic (workspace sizing, launch planning, argument
+validation) behaves.  No kernel is launched here."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1411_5234_b200 import build, binding
+    build.build()
+    binding.lib()
+    return binding
+
+
+def test_library_exports_every_declared_symbol(B):
+    hdr = open(os.path.join(ROOT, "include", "nb.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = sorted(set(re.findall(r"\b(nb_[a-z0-9_]+)\s*\(", hdr)))
+    assert declared == sorted(B.EXPORTS)
+    L = B.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_struct_layouts_match_header(B):
+    # nb_config: int, void*, void*, size_t, int, double, double, int, int  (natural alignment)
+    assert C.sizeof(B.nb_config) == 64
+    assert B.nb_config.workspace.offset == 16 and B.nb_config.eta.offset == 40 and B.nb_config.k_max.offset == 60
+    assert C.sizeof(B.nb_plan) == 32
+
+
+def test_workspace_bytes(B):
+    assert B.nb_workspace_bytes(0) == 0 and B.nb_workspace_bytes(-5) == 0
+    b1, b2 = B.nb_workspace_bytes(1), B.nb_workspace_bytes(256)
+    assert b1 == b2 and b1 % 256 == 0                        # padded to 256 particles
+    assert B.nb_workspace_bytes(257) > b2
+    big = B.nb_workspace_bytes(1 << 20)
+    assert 600e6 < big < 1.2e9                               # ~0.8 GB for 2^20 particles: fits 180 GB many times over
+
+
+@pytest.mark.parametrize("N", [1, 2, 255, 1024, 5000, 65536, 262144, 1 << 20])
+def test_plan_invariants(B, N):
+    for n_act in sorted({1, 2, 7, 64, 512, 1024, 1025, 4096, 32768, N // 3 + 1, N} & set(range(1, N + 1)) | {N}):
+        for n_sm in (148, 132, 8):
+            p = B.nb_plan_force(N, n_act, n_sm)
+            Npad = (N + 255) // 256 * 256
+            if n_act <= 1024:
+                assert p.kernel == 1 and p.n_units == (n_act + 1) // 2
+                n_tiles, unit = Npad // 32, 2
+                assert p.grid <= n_sm * 3
+            else:
+                assert p.kernel == 0 and p.n_units == (n_act + 255) // 256
+                n_tiles, unit = Npad // 128, 256
+                assert p.grid <= n_sm * 3
+            S, st = p.n_split, p.slice_tiles
+            assert S >= 1 and st >= 1 and p.grid >= 1
+            assert S * st >= n_tiles and (S - 1) * st < n_tiles            # slices cover all j-tiles, none empty
+            assert S * p.n_units * unit <= 4 * Npad + (1 << 19)            # partial-sum buffer capacity
+            # small active sets are split so that the device is filled
+            resident = n_sm * 3 * (4 if p.kernel == 1 else 1)
+            if p.n_units < resident and n_tiles >= 16 * resident:
+                assert p.n_units * S >= 0.5 * resident
+
+
+def test_plan_rejects_bad_sizes(B):
+    p = B.nb_plan()
+    L = B.lib()
+    assert L.nb_plan_force(0, 1, 148, C.byref(p)) == B.NB_EINVAL
+    assert L.nb_plan_force(10, 11, 148, C.byref(p)) == B.NB_EINVAL
+    assert L.nb_plan_force(10, 0, 148, C.byref(p)) == B.NB_EINVAL
+    assert L.nb_plan_force(10, 5, 0, C.byref(p)) == B.NB_EINVAL
+    assert L.nb_plan_force(10, 5, 148, None) == B.NB_EINVAL
+
+
+def test_argument_validation_without_gpu(B):
+    L = B.lib()
+    ctx = C.c_void_p()
+    m = np.ones(4); x = np.zeros((4, 3)); v = np.zeros((4, 3))
+    cfg = B.nb_config(0, None, None, 0, 0, 0, 0, 0, 0)
+    pm, px, pv = B._ptr(m), B._ptr(x), B._ptr(v)
+    assert L.nb_init(C.byref(ctx), 4, pm, px, pv, 1e-3, C.byref(cfg)) == B.NB_ENOMEM       # no workspace
+    assert L.nb_init(C.byref(ctx), 0, pm, px, pv, 1e-3, C.byref(cfg)) == B.NB_EINVAL
+    assert L.nb_init(C.byref(ctx), 4, None, px, pv, 1e-3, C.byref(cfg)) == B.NB_EINVAL
+    assert L.nb_init(C.byref(ctx), 4, pm, px, pv, float("nan"), C.byref(cfg)) == B.NB_EINVAL
+    bad = B.nb_config(0, None, None, 0, 0, 0, 0, -3, -20)                                   # k_min > k_max
+    assert L.nb_init(C.byref(ctx), 4, pm, px, pv, 1e-3, C.byref(bad)) == B.NB_EINVAL
+    assert L.nb_predict(None, 0.0) == B.NB_EINVAL
+    assert L.nb_force(None, None, 0, None, None, None, None) == B.NB_EINVAL
+    assert L.nb_launch_count(None) == 0
+    assert L.nb_strerror(B.NB_ESTATE).decode().startswith("call order")
+    assert L.nb_strerror(12345).decode() == "unknown status"
+    L.nb_free(None)
+
+
+def test_product_path_has_no_oracle_or_cpu_fallback():
+    """The package never imports oracle/, and System refuses to run without CUDA."""
+    pkg = os.path.join(ROOT, "paper_1411_5234_b200")
+    for fn in os.listdir(pkg):
+        if fn.endswith(".py"):
+            src = open(os.path.join(pkg, fn)).read()
+            assert not re.search(r"^\s*(from|import)\s+oracle\b", src, flags=re.M), fn
+    import torch
+    if not torch.cuda.is_available():
+        from paper_1411_5234_b200 import binding
+        with pytest.raises(RuntimeError):
+            binding.System(np.ones(2), np.zeros((2, 3)), np.zeros((2, 3)), 1e-3)

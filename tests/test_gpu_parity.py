@@ -1,0 +1,332 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle,
+element by element on the same seeded inputs.  Tolerances (BASELINE.json north_star):
+  a, jerk, snap per particle: || gpu - oracle ||_2 / || oracle ||_2 <= 1e-11;  pot: relative 1e-11
+  total energy after 8 steps: relative 1e-10
+  indices, times, step levels: bit-exact.
+"""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+from paper_1411_5234_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1411_5234_b200 import binding
+    binding.lib()
+    return binding
+
+
+def relvec(g, o):
+    return np.linalg.norm(g - o, axis=-1) / np.linalg.norm(o, axis=-1)
+
+
+def assert_force_parity(g, o, tol=TOL):
+    ga, gj, gs, gp = g
+    oa, oj, os_, op = o
+    assert relvec(ga, oa).max() <= tol, ("acc", relvec(ga, oa).max())
+    assert relvec(gj, oj).max() <= tol, ("jerk", relvec(gj, oj).max())
+    assert relvec(gs, os_).max() <= tol, ("snap", relvec(gs, os_).max())
+    assert np.abs(gp / op - 1).max() <= tol, ("pot", np.abs(gp / op - 1).max())
+
+
+def oracle_on_gpu_records(oracle, sysg, eps, idx):
+    """O1 on the predicted records the GPU kernel read (nb_force is a pure function of them)."""
+    m = sysg.nb_get_state("M")
+    xp, vp, ap = sysg.nb_get_state("XP"), sysg.nb_get_state("VP"), sysg.nb_get_state("AP")
+    return oracle.hermite6.force(m, xp, vp, ap, eps, idx)
+
+
+# ------------------------------------------------------------------ config 1, end to end
+def test_config1_force_and_8_steps(B, oracle):
+    c, m, x, v = W.config_inputs(1)
+    g = B.System(m, x, v, c.eps)
+    o = oracle.OracleSystem(m, x, v, c.eps)
+    # startup (two-pass) state
+    for f, ref in (("A", o.a), ("J", o.j), ("S", o.s)):
+        assert relvec(g.nb_get_state(f), ref).max() <= TOL
+    assert np.array_equal(g.nb_get_state("DT"), o.dt)
+    # one predict + force
+    g.nb_predict(0.0); o.predict(0.0)
+    assert_force_parity(g.nb_force(), o.force())
+    Kg0, Wg0 = g.nb_energy()
+    Ko0, Wo0 = o.energy()
+    assert abs((Kg0 + Wg0) / (Ko0 + Wo0) - 1) <= 1e-12
+    # 8 shared steps
+    t = 0.0
+    for _ in range(c.n_steps):
+        t += c.dt
+        g.nb_predict(t); g.nb_force(outputs=False); g.nb_corrector(None, c.dt)
+        o.shared_step(c.dt)
+    assert np.all(g.nb_get_state("T") == t)
+    for f, ref, tol in (("X", o.x, 1e-13), ("V", o.v, 1e-12), ("A", o.a, TOL), ("J", o.j, TOL), ("S", o.s, TOL)):
+        assert relvec(g.nb_get_state(f), ref).max() <= tol, f
+    cr = relvec(g.nb_get_state("C"), o.c)
+    assert np.median(cr) < 1e-9 and cr.max() < 1e-5          # crackle is a 5th difference: ill-conditioned by construction
+    Kg, Wg = g.nb_energy()
+    Ko, Wo = o.energy()
+    assert abs((Kg + Wg) - (Ko + Wo)) / abs(Ko + Wo) <= 1e-10
+    g.nb_free()
+
+
+# ------------------------------------------------------------------ force kernel shapes, ragged sizes, edge cases
+@pytest.mark.parametrize("N,eps,masses", [(1000, 1e-3, "equal"), (4099, 1e-4, "kroupa"), (2, 0.0, "equal"), (257, 0.0, "kroupa")])
+def test_force_parity_active_sets(B, oracle, N, eps, masses):
+    m, x, v = W.plummer(N, 1000 + N, masses)
+    g = B.System(m, x, v, eps)
+    # advance once so that a, jerk, snap, crackle are all non-zero and D != 0 in the predictor
+    g.nb_predict(2.0 ** -9); g.nb_force(outputs=False); g.nb_corrector(None, 2.0 ** -9)
+    g.nb_predict(2.0 ** -9 + 2.0 ** -11)
+    rng = np.random.default_rng(N)
+    sizes = sorted({1, 2, 3, 31, 33, 64, 255, 1023, 1024, 1025, 2049, N} & set(range(1, N + 1)) | {N})
+    for n_act in sizes:
+        idx = None if n_act == N else rng.choice(N, n_act, replace=False).astype(np.int32)
+        got = g.nb_force(idx)
+        ref = oracle_on_gpu_records(oracle, g, eps, idx)
+        assert_force_parity(got, ref)
+        plan = B.nb_plan_force(N, n_act, 148)
+        assert plan.kernel == (1 if n_act <= 1024 else 0)
+    # permuted full list: row k <-> idx[k]
+    perm = rng.permutation(N).astype(np.int32)
+    got = g.nb_force(perm)
+    ref = oracle_on_gpu_records(oracle, g, eps, perm)
+    assert_force_parity(got, ref)
+    g.nb_free()
+
+
+def test_predictor_and_corrector_parity_block_steps(B, oracle):
+    """Same block-step sequence on both sides, N = 384 Kroupa masses: scheduler output bit-exact,
+    predictor/corrector/time-step levels compared after every block step."""
+    N, eps = 384, 1e-3
+    m, x, v = W.plummer(N, 77, "kroupa")
+    g = B.System(m, x, v, eps)
+    o = oracle.OracleSystem(m, x, v, eps)
+    assert np.array_equal(g.nb_get_state("DT"), o.dt)
+    n_steps = 0
+    while True:
+        tg, ng, actg = g.nb_next_block()
+        to, acto = o.next_block()
+        assert tg == to and ng == acto.size and np.array_equal(actg, acto)      # bit-exact
+        if to > 2.0 ** -5:
+            break
+        g.nb_predict(tg); o.predict(to)
+        for f, ref in (("XP", o.xp), ("VP", o.vp), ("AP", o.ap)):
+            assert relvec(g.nb_get_state(f), ref).max() <= 1e-12, f
+        assert_force_parity(g.nb_force(actg), o.force(acto), 1e-10)     # states differ at round-off by now
+        g.nb_corrector(actg, 0.0); o.corrector(acto, 0.0)
+        assert np.array_equal(g.nb_get_state("T"), o.t)
+        assert np.array_equal(g.nb_get_state("DT"), o.dt)               # same level decisions
+        n_steps += 1
+    assert n_steps > 20
+    for f, ref, tol in (("X", o.x, 1e-12), ("V", o.v, 1e-11)):
+        assert relvec(g.nb_get_state(f), ref).max() <= tol
+    g.nb_free()
+
+
+def test_internal_active_list_and_device_pointers(B, oracle):
+    import torch
+    N, eps = 3000, 1e-3
+    m, x, v = W.plummer(N, 5, "kroupa")
+    gh = B.System(m, x, v, eps, host=True)
+    dev = "cuda:0"
+    gd = B.System(torch.tensor(m, device=dev), torch.tensor(x, device=dev), torch.tensor(v, device=dev), eps, host=False)
+    for _ in range(5):
+        th, nh, acth = gh.nb_next_block()
+        td, nd, _ = gd.nb_next_block(want_list=False)
+        assert th == td and nh == nd
+        gh.nb_predict(th); gd.nb_predict(td)
+        fh = gh.nb_force(acth)
+        fd = gd.nb_force(B.ACTIVE_INTERNAL, n_act=nd)
+        torch.cuda.synchronize()
+        for a, b in zip(fh, fd):
+            assert np.array_equal(a, b.cpu().numpy())                   # same kernels, same plan: bitwise equal
+        gh.nb_corrector(acth, 0.0); gd.nb_corrector(B.ACTIVE_INTERNAL, 0.0, n_act=nd)
+    torch.cuda.synchronize()
+    assert np.array_equal(gh.nb_get_state("X"), gd.nb_get_state("X").cpu().numpy())
+    gh.nb_free(); gd.nb_free()
+
+
+def test_run_to_run_determinism(B):
+    N = 20000
+    m, x, v = W.plummer(N, 8)
+    res = []
+    for _ in range(2):
+        g = B.System(m, x, v, 1e-4)
+        g.nb_predict(2.0 ** -10)
+        idx = W.active_set(N, 3000, 4)
+        res.append((g.nb_force(idx), g.nb_force(None), g.nb_force(idx[:50].copy())))
+        g.nb_free()
+    for r0, r1 in zip(*res):
+        for a, b in zip(r0, r1):
+            assert np.array_equal(a, b)
+
+
+def test_scheduler_bit_exact_on_crafted_times(B, oracle):
+    N = 5000
+    m, x, v = W.plummer(N, 9)
+    g = B.System(m, x, v, 1e-3)
+    rng = np.random.default_rng(3)
+    lev = rng.integers(-12, -3, N)
+    dt = 2.0 ** lev
+    t = dt * rng.integers(0, 5, N)
+    g.nb_set_state("T", t); g.nb_set_state("DT", dt)
+    assert np.array_equal(g.nb_get_state("T"), t) and np.array_equal(g.nb_get_state("DT"), dt)
+    tn, n, act = g.nb_next_block()
+    act_o = np.zeros(N, dtype=np.int32)
+    tn_o = C.c_double()
+    n_o = oracle.lib("ld").oracle_next_block(N, oracle.hermite6._p(t), oracle.hermite6._p(dt), C.byref(tn_o),
+                                             oracle.hermite6._pi(act_o))
+    assert tn == tn_o.value and n == n_o and np.array_equal(act, act_o[:n_o])
+    # everyone active
+    g.nb_set_state("T", np.zeros(N)); g.nb_set_state("DT", np.full(N, 0.125))
+    tn, n, act = g.nb_next_block()
+    assert tn == 0.125 and n == N and np.array_equal(act, np.arange(N, dtype=np.int32))
+    g.nb_free()
+
+
+def test_state_io_and_errors(B):
+    N = 700
+    m, x, v = W.plummer(N, 10)
+    g = B.System(m, x, v, 1e-3)
+    assert np.array_equal(g.nb_get_state("M"), m) and np.array_equal(g.nb_get_state("X"), x)
+    assert np.array_equal(g.nb_get_state("V"), v)
+    idx = np.array([5, 699, 0, 17], dtype=np.int32)
+    assert np.array_equal(g.nb_get_state("X", idx), x[idx])
+    rng = np.random.default_rng(0)
+    for f in ("X", "V", "A", "J", "S", "C"):
+        val = rng.normal(size=(4, 3))
+        g.nb_set_state(f, val, idx)
+        assert np.array_equal(g.nb_get_state(f, idx), val)
+        full = g.nb_get_state(f)
+        assert np.array_equal(full[idx], val)
+    # neighbours untouched by the packed-field writes
+    assert np.array_equal(g.nb_get_state("M"), m)
+    # call-order and argument errors
+    with pytest.raises(B.NBError) as e:
+        g.nb_force()
+    assert e.value.status == B.NB_ESTATE
+    g.nb_predict(0.0)
+    with pytest.raises(B.NBError) as e:
+        g.nb_corrector(None, 0.1)
+    assert e.value.status == B.NB_ESTATE
+    assert g.L.nb_force(g.ctx, None, N + 1, None, None, None, None) == B.NB_EINVAL
+    assert g.L.nb_force(g.ctx, None, 5, None, None, None, None) == B.NB_EINVAL       # NULL list needs n_act == N
+    assert g.L.nb_force(g.ctx, None, 0, None, None, None, None) == B.NB_OK           # empty active set: no-op
+    g.nb_free()
+    # workspace too small / bad arguments
+    import torch
+    ws = torch.empty(4096, dtype=torch.uint8, device="cuda:0")
+    cfg = B.nb_config(0, None, C.c_void_p(ws.data_ptr()), 4096, 0, 0, 0, 0, 0)
+    ctx = C.c_void_p()
+    mm = np.ascontiguousarray(m)
+    args = (B._ptr(mm), B._ptr(np.ascontiguousarray(x)), B._ptr(np.ascontiguousarray(v)))
+    assert B.lib().nb_init(C.byref(ctx), N, *args, 1e-3, C.byref(cfg)) == B.NB_ENOMEM
+    assert B.lib().nb_init(C.byref(ctx), 0, *args, 1e-3, C.byref(cfg)) == B.NB_EINVAL
+    assert B.lib().nb_init(C.byref(ctx), N, *args, -1.0, C.byref(cfg)) == B.NB_EINVAL
+
+
+def test_newton_third_law_and_energy_on_gpu(B):
+    """Properties that hold at any size: sum m a = sum m jerk = sum m snap = 0; 6th-order energy behaviour."""
+    N = 30000
+    m, x, v = W.plummer(N, 12, "kroupa")
+    g = B.System(m, x, v, 1e-3)
+    for f in ("A", "J", "S"):
+        arr = g.nb_get_state(f)
+        assert np.abs((m[:, None] * arr).sum(0)).max() <= 1e-13 * (m[:, None] * np.abs(arr)).sum()
+    g.nb_free()
+
+
+# ------------------------------------------------------------------ full sizes, sampled (configs 2, 4, 5)
+@pytest.fixture(scope="module")
+def big(B):
+    c, m, x, v = W.config_inputs(4)
+    g = B.System(m, x, v, c.eps)
+    yield c, m, x, v, g
+    g.nb_free()
+
+
+def test_config4_full_size_sampled(big, B, oracle):
+    c, m, x, v, g = big
+    N = c.N
+    g.nb_predict(0.0)
+    ga, gj, gs, gp = g.nb_force()                    # the bench configuration: all N active
+    ms = g.nb_last_force_ms()
+    assert ms > 0
+    sample = W.active_set(N, 96, 999)
+    a_state = g.nb_get_state("A")
+    ref = oracle.hermite6.force(m, x, v, a_state, c.eps, sample)
+    assert_force_parity((ga[sample], gj[sample], gs[sample], gp[sample]), ref)
+    # properties over all N: Newton's third law, potential energy consistent with Henon units
+    for arr in (ga, gj, gs):
+        assert np.abs((m[:, None] * arr).sum(0)).max() <= 1e-12 * (m[:, None] * np.abs(arr)).sum()
+    Wpot = 0.5 * (m * gp).sum()
+    assert abs(Wpot + 0.5) < 0.01
+
+
+@pytest.mark.parametrize("n_act", [1, 8, 64, 512, 4096, 32768])
+def test_config5_small_active_sets_full_size(big, B, oracle, n_act):
+    c, m, x, v, g = big
+    idx = W.config5_active(n_act)
+    g.nb_predict(0.0)
+    got = g.nb_force(idx)
+    rows = np.arange(n_act) if n_act <= 64 else np.random.default_rng(n_act).choice(n_act, 64, replace=False)
+    a_state = g.nb_get_state("A")
+    ref = oracle.hermite6.force(m, x, v, a_state, c.eps, idx[rows])
+    assert_force_parity(tuple(a[rows] for a in got), ref)
+
+
+def test_config2_sampled_and_steps(B, oracle):
+    c, m, x, v = W.config_inputs(2)
+    g = B.System(m, x, v, c.eps)
+    K0, W0 = g.nb_energy()
+    t = 0.0
+    for _ in range(c.n_steps):
+        t += c.dt
+        g.nb_predict(t); g.nb_force(outputs=False); g.nb_corrector(None, c.dt)
+    g.nb_predict(t)
+    got = g.nb_force()
+    sample = W.active_set(c.N, 128, 123)
+    ref = oracle_on_gpu_records(oracle, g, c.eps, sample)
+    assert_force_parity(tuple(a[sample] for a in got), ref)
+    K1, W1 = g.nb_energy()
+    assert abs((K1 + W1) / (K0 + W0) - 1) < 1e-7        # energy drift of the method at dt = 2^-12 (reported by bench/DESIGN)
+    g.nb_free()
+
+
+def test_config3_reduced_twin_block_steps(B, oracle):
+    """Config 3's recipe at N = 2048 run end to end to t = 1/8 on both sides."""
+    _, m, x, v = W.config_inputs(3, N=2048)
+    eps = W.CONFIGS[3].eps
+    g = B.System(m, x, v, eps)
+    o = oracle.OracleSystem(m, x, v, eps)
+    Kg0, Wg0 = g.nb_energy()
+    mism = 0
+    n_blocks = 0
+    while True:
+        tg, ng, actg = g.nb_next_block()
+        if tg > 0.125:
+            break
+        to, acto = o.next_block()
+        if not (tg == to and np.array_equal(actg, acto)):
+            mism += 1
+            break
+        g.nb_predict(tg); g.nb_force(actg, outputs=False); g.nb_corrector(actg, 0.0)
+        o.predict(to); o.force(acto); o.corrector(acto, 0.0)
+        n_blocks += 1
+    assert mism == 0, f"schedules diverged after {n_blocks} block steps"
+    assert np.all(g.nb_get_state("T") == 0.125)
+    assert relvec(g.nb_get_state("X"), o.x).max() < 1e-9
+    Kg, Wg = g.nb_energy()
+    Ko, Wo = o.energy()
+    assert abs((Kg + Wg) - (Ko + Wo)) / abs(Ko + Wo) < 1e-10
+    assert abs((Kg + Wg) / (Kg0 + Wg0) - 1) < 1e-5
+    g.nb_free()
