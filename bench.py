@@ -41,6 +41,28 @@ def n_cores() -> int:
     return len(os.sched_getaffinity(0))
 
 
+# ------------------------------------------------------------------------------------------ multi-rank plumbing
+def replica_seed(base_seed: int, rank: int, world: int) -> int:
+    """Replicas only: rank r of an N > 1 run steps its own realisation of the workload."""
+    return base_seed if world == 1 else base_seed + 1000 * rank
+
+
+def max_over_ranks(x: float, world: int, device="cpu") -> float:
+    """The job's time is the slowest rank's (all-reduce MAX; works on nccl with a cuda device and on gloo with cpu)."""
+    if world == 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, steps: int, units_per_step_per_rank: float, ms: float) -> float:
+    """Units all ranks processed / the max-over-ranks time (weak scaling: per-rank work is fixed)."""
+    return world * steps * units_per_step_per_rank / (ms * 1e-3)
+
+
 # ------------------------------------------------------------------------------------------ clocks
 class ClockSampler:
     """nvidia-smi clocks/throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
@@ -154,7 +176,7 @@ def run_ours(args, cfg_dict):
 
     c, m, x, v = W.config_inputs(4, N=args.N)
     if world > 1:                                       # replicas: every rank its own realisation
-        m, x, v = W.plummer(m.shape[0], c.seed + 1000 * rank, c.masses)
+        m, x, v = W.plummer(m.shape[0], replica_seed(c.seed, rank, world), c.masses)
     N = m.shape[0]
     inter_per_step = N * (N - 1)
 
@@ -189,11 +211,8 @@ def run_ours(args, cfg_dict):
     ms = ev0.elapsed_time(ev1)
     launches = g.nb_launch_count() - launches0
     clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        tms = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-        ms = float(tms.item())
-    value = world * args.steps * inter_per_step / (ms * 1e-3)
+    ms = max_over_ranks(ms, world, dev)
+    value = whole_job_value(world, args.steps, inter_per_step, ms)
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D of x, v and D2H of a, jerk, snap, pot every step
     gh = B.System(m, x, v, c.eps, host=True, device=local)
@@ -219,11 +238,8 @@ def run_ours(args, cfg_dict):
         res = step_host()
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        tt = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_s = float(tt.item())
-    e2e_value = world * e2e_steps * inter_per_step / e2e_s
+    e2e_s = max_over_ranks(e2e_s, world, dev)
+    e2e_value = whole_job_value(world, e2e_steps, inter_per_step, e2e_s * 1e3)
     assert np.isfinite(res[0]).all()
 
     if rank != 0:
