@@ -14,7 +14,7 @@ namespace {
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t x, size_t a = ALIGN) { return (x + a - 1) / a * a; }
 inline int64_t pad_n(int64_t N) { return (N + NB_PAD - 1) / NB_PAD * NB_PAD; }
-inline int64_t partial_rows(int64_t Npad) { return 4 * Npad + (int64_t(1) << 19); }
+inline int64_t partial_rows(int64_t Npad) { return 8 * Npad + (int64_t(1) << 19); }
 inline size_t scratch_bytes(int64_t Npad) { return 65536 + (size_t)Npad / 8; }
 
 struct Carve {
@@ -32,6 +32,7 @@ struct Layout {
     int32_t *idx_user, *idx_sched, *idx_tmp;
     double* stage;                      // staging for host <-> device transfers, 10 doubles per particle
     char* scratch;
+    int* queue;                         // work queue of the force kernels (2 counters)
     size_t bytes;
     Layout(void* base, int64_t Npad)
     {
@@ -44,6 +45,7 @@ struct Layout {
         idx_user = c.take<int32_t>(Npad); idx_sched = c.take<int32_t>(Npad); idx_tmp = c.take<int32_t>(Npad);
         stage = c.take<double>(10 * Npad);
         scratch = c.take<char>(scratch_bytes(Npad));
+        queue = c.take<int>(64);
         bytes = c.off;
     }
 };
@@ -101,7 +103,10 @@ int copy_out(nb_ctx* ctx, double* dst, const double* src, size_t count)
     return NB_OK;
 }
 
-// Smallest-cost split: cost(S) = ceil(units*S / resident) * (slice_tiles + fixed), in j-tiles.
+// Split chosen by a cost model (reading R15), in units of one j-tile of work on one work slot.  Work items
+// (unit, slice) are pulled from a queue by `resident` workers (CTAs or warps); an item costs
+// slice_tiles + fixed.  Up to a few rounds the last round is counted whole; beyond that the queue balances
+// the workers up to a tail of about one item.
 void choose_split(int64_t n_units, int64_t n_tiles, int64_t resident, int64_t s_max, int fixed, nb_plan* p)
 {
     int64_t best_S = 1, best_tiles = n_tiles;
@@ -111,8 +116,10 @@ void choose_split(int64_t n_units, int64_t n_tiles, int64_t resident, int64_t s_
         const int64_t st = (n_tiles + S - 1) / S;
         const int64_t S_eff = (n_tiles + st - 1) / st;           // slices that are not empty
         if (S_eff != S) continue;
-        const int64_t rounds = (n_units * S + resident - 1) / resident;
-        const double cost = (double)rounds * (double)(st + fixed);
+        const int64_t items = n_units * S;
+        const double rounds = items <= 4 * resident ? (double)((items + resident - 1) / resident)
+                                                    : (double)items / (double)resident + 0.7;
+        const double cost = rounds * (double)(st + fixed);
         if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best_S = S; best_tiles = st; }
     }
     p->n_split = (int)best_S;
@@ -153,7 +160,7 @@ int nb_plan_force(int64_t N, int64_t n_act, int n_sm, nb_plan* plan)
         const int64_t n_tiles = Npad / LI_TJ;
         const int64_t resident = (int64_t)n_sm * LI_CTAS_PER_SM;
         const int64_t s_cap = rows / ((int64_t)p.n_units * LI_UNIT);
-        choose_split(p.n_units, n_tiles, resident, std::min<int64_t>(s_cap, n_tiles / 2), 1, &p);
+        choose_split(p.n_units, n_tiles, resident, std::min<int64_t>(std::min<int64_t>(s_cap, 256), n_tiles / 2), 2, &p);
         const int64_t items = (int64_t)p.n_units * p.n_split;
         p.grid = (int)std::min<int64_t>(items, resident);
     }
@@ -188,6 +195,7 @@ int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const dou
     CU(cudaEventCreate(&ctx->ev0), "event");
     CU(cudaEventCreate(&ctx->ev1), "event");
     CU(cudaMemsetAsync(ctx->L.scratch, 0, scratch_bytes(Npad), ctx->stream), "memset scratch");
+    CU(cudaMemsetAsync(ctx->L.queue, 0, 64 * sizeof(int), ctx->stream), "memset queue");
 
     const double *dm = m, *dx = x, *dv = v;
     if (!ctx->on_device) {
@@ -249,6 +257,7 @@ int nb_force(nb_ctx* ctx, const int32_t* active_idx, int64_t n_act, double* a, d
     A.ld = plan.n_units * (plan.kernel == 0 ? LI_UNIT : LJ_I);
     A.eps2 = ctx->eps * ctx->eps;
     A.partial = ctx->L.partial;
+    A.queue = ctx->L.queue;                                 // zeroed by nb_init, left at 0 by every launch
     A.out_a = ctx->L.fa; A.out_j = ctx->L.fj; A.out_s = ctx->L.fs; A.out_p = ctx->L.fp;
 
     int launches = 0;

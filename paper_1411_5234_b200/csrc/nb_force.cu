@@ -10,6 +10,11 @@
 //   force_lj_kernel  lanes-over-j: a warp owns LJ_I active particles (same in every lane); its 32
 //                    lanes read 32 different j-records straight from global memory (coalesced) and
 //                    the ten sums per particle are combined with a warp-shuffle butterfly.
+// Work items (i-unit, j-slice) are handed out by an atomic queue, not by a static stride: warps of
+// co-resident CTAs do NOT get equal shares of the FP64 pipe (measured: of three CTAs with equal work on
+// one SM the first finished after 40 % of the time the last one needed), so a static partition ends in a
+// long tail of under-occupied SMs.  Where an item's sums are stored depends only on the item, so the
+// results stay bitwise reproducible.
 #include "nb_internal.h"
 
 namespace {
@@ -114,6 +119,13 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
     } while (!done);
 }
 
+// The CTA (or warp) that finds the queue empty last puts both counters back to 0 for the next launch.
+__device__ __forceinline__ void queue_retire(int* queue, int n_workers)
+{
+    __threadfence();
+    if (atomicAdd(queue + 1, 1) == n_workers - 1) { queue[0] = 0; queue[1] = 0; }
+}
+
 // ---------------------------------------------------------------------------------------------
 // lanes-over-i
 // ---------------------------------------------------------------------------------------------
@@ -126,6 +138,7 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
     __shared__ alignas(128) double4 s1[LI_STAGES][LI_TJ];
     __shared__ alignas(128) double2 s2[LI_STAGES][LI_TJ];
     __shared__ alignas(8) unsigned long long full[LI_STAGES];
+    __shared__ int next_item;
 
     const int tid = threadIdx.x;
     if (tid == 0) {
@@ -145,7 +158,12 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
     };
 
     uint32_t uses = 0;   // j-tiles this CTA has consumed so far: stage = uses % STAGES, parity = (uses / STAGES) & 1
-    for (int item = blockIdx.x; item < A.n_items; item += gridDim.x) {
+    for (;;) {
+        if (tid == 0) next_item = atomicAdd(A.queue, 1);
+        __syncthreads();
+        const int item = next_item;
+        __syncthreads();                                   // everyone has read next_item before it is overwritten
+        if (item >= A.n_items) break;
         const int unit = item % A.n_units, slice = item / A.n_units;
         const int t0 = slice * A.slice_tiles;
         const int nt = min(A.slice_tiles, A.n_tiles - t0);
@@ -187,6 +205,7 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
 #pragma unroll
         for (int q = 0; q < LI_I; ++q) store_sums(A, slice, unit * LI_UNIT + q * LI_THREADS + tid, valid[q], acc[q]);
     }
+    if (tid == 0) queue_retire(A.queue, gridDim.x);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -202,8 +221,12 @@ __device__ __forceinline__ double warp_sum(double v)
 template <bool EPS0>
 __global__ void __launch_bounds__(LJ_THREADS, LJ_CTAS_PER_SM) force_lj_kernel(const ForceArgs A)
 {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int wi = blockIdx.x * LJ_WARPS + warp; wi < A.n_items; wi += gridDim.x * LJ_WARPS) {
+    const int lane = threadIdx.x & 31;
+    for (;;) {
+        int wi = 0;
+        if (lane == 0) wi = atomicAdd(A.queue, 1);
+        wi = __shfl_sync(0xffffffffu, wi, 0);
+        if (wi >= A.n_items) break;
         const int unit = wi % A.n_units, slice = wi / A.n_units;
         const int t0 = slice * A.slice_tiles;
         const int nt = min(A.slice_tiles, A.n_tiles - t0);
@@ -244,6 +267,7 @@ __global__ void __launch_bounds__(LJ_THREADS, LJ_CTAS_PER_SM) force_lj_kernel(co
             if (lane == 0) store_sums(A, slice, unit * LJ_I + q, valid[q], S);
         }
     }
+    if (lane == 0) queue_retire(A.queue, gridDim.x * LJ_WARPS);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -14,17 +14,20 @@
 
 constexpr int NB_PAD = 256;          // particle arrays are padded to a multiple of this
 
+// Both force kernels keep ONE active particle per thread (lanes-over-i) or per warp (lanes-over-j) in
+// 80 registers so that 24 warps (6 per scheduler) are resident per SM: the FP64 pipe is fed by warp-level
+// parallelism, which measured faster than two particles per thread at 3 warps per scheduler.
 // lanes-over-i kernel: each thread owns LI_I active particles, a CTA streams j-tiles through smem
-constexpr int LI_THREADS = 128;
-constexpr int LI_I = 2;
+constexpr int LI_THREADS = 256;
+constexpr int LI_I = 1;
 constexpr int LI_UNIT = LI_THREADS * LI_I;   // active particles per i-tile
 constexpr int LI_TJ = 128;                   // j-records per smem stage (10 KB)
 constexpr int LI_STAGES = 2;
 constexpr int LI_CTAS_PER_SM = 3;
 // lanes-over-j kernel: each warp owns LJ_I active particles, lanes take different j
-constexpr int LJ_THREADS = 128;
+constexpr int LJ_THREADS = 256;
 constexpr int LJ_WARPS = LJ_THREADS / 32;
-constexpr int LJ_I = 2;
+constexpr int LJ_I = 1;
 constexpr int LJ_TJ = 32;                    // j-records per warp iteration
 constexpr int LJ_CTAS_PER_SM = 3;
 constexpr int64_t LJ_MAX_ACT = 1024;         // n_act <= this -> lanes-over-j
@@ -41,6 +44,7 @@ struct ForceArgs {
     int ld;                  // rows of the partial buffer per (slice, component) plane
     double eps2;
     double* partial;         // [S][10][ld] when S > 1
+    int* queue;              // work queue: [0] next item, [1] finished CTAs (both 0 between launches)
     double* out_a; double* out_j; double* out_s; double* out_p;   // [n_act][3] x3, [n_act]
 };
 
