@@ -190,7 +190,7 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
             const int st = u & (LI_STAGES - 1);
             mbar_wait(smem_u32(&full[st]), (u / LI_STAGES) & 1);
             const int jbase = (t0 + t) * LI_TJ;
-#pragma unroll 2
+#pragma unroll LI_UNROLL
             for (int jj = 0; jj < LI_TJ; ++jj) {
                 const double4 p0 = s0[st][jj], p1 = s1[st][jj];
                 const double2 p2 = s2[st][jj];

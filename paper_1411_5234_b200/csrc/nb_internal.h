@@ -17,13 +17,33 @@ constexpr int NB_PAD = 256;          // particle arrays are padded to a multiple
 // Both force kernels keep ONE active particle per thread (lanes-over-i) or per warp (lanes-over-j) in
 // 80 registers so that 24 warps (6 per scheduler) are resident per SM: the FP64 pipe is fed by warp-level
 // parallelism, which measured faster than two particles per thread at 3 warps per scheduler.
+// The NB_* macros are build-time tunables (defaults = the measured best); -DNB_...=v overrides one for experiments.
+#ifndef NB_LI_THREADS
+#define NB_LI_THREADS 256
+#endif
+#ifndef NB_LI_I
+#define NB_LI_I 1
+#endif
+#ifndef NB_LI_TJ
+#define NB_LI_TJ 128
+#endif
+#ifndef NB_LI_STAGES
+#define NB_LI_STAGES 2
+#endif
+#ifndef NB_LI_CTAS_PER_SM
+#define NB_LI_CTAS_PER_SM 3
+#endif
+#ifndef NB_LI_UNROLL
+#define NB_LI_UNROLL 2
+#endif
 // lanes-over-i kernel: each thread owns LI_I active particles, a CTA streams j-tiles through smem
-constexpr int LI_THREADS = 256;
-constexpr int LI_I = 1;
+constexpr int LI_THREADS = NB_LI_THREADS;
+constexpr int LI_I = NB_LI_I;
 constexpr int LI_UNIT = LI_THREADS * LI_I;   // active particles per i-tile
-constexpr int LI_TJ = 128;                   // j-records per smem stage (10 KB)
-constexpr int LI_STAGES = 2;
-constexpr int LI_CTAS_PER_SM = 3;
+constexpr int LI_TJ = NB_LI_TJ;              // j-records per smem stage (80 B each)
+constexpr int LI_STAGES = NB_LI_STAGES;
+constexpr int LI_CTAS_PER_SM = NB_LI_CTAS_PER_SM;
+constexpr int LI_UNROLL = NB_LI_UNROLL;       // j-loop unroll factor
 // lanes-over-j kernel: each warp owns LJ_I active particles, lanes take different j
 constexpr int LJ_THREADS = 256;
 constexpr int LJ_WARPS = LJ_THREADS / 32;
