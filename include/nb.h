@@ -80,6 +80,9 @@ typedef struct {
     int n_split;      /* S: number of j-slices each unit is split into ("Bfactor") */
     int slice_tiles;  /* j-tiles per slice (the last slice may hold fewer) */
     int grid;         /* CTAs launched */
+    int unit;         /* active particles per unit (kernel 0: threads per CTA x I; kernel 1: I) */
+    int tile;         /* j-records per j-tile (kernel 0: one shared-memory stage; kernel 1: one warp iteration) */
+    int ctas_per_sm;  /* resident CTAs per multiprocessor the plan assumes */
     double waves;     /* work items / resident CTAs (or warps) on the device */
 } nb_plan;
 

@@ -145,7 +145,7 @@ int nb_plan_force(int64_t N, int64_t n_act, int n_sm, nb_plan* plan)
     nb_plan p{};
     if (n_act <= LJ_MAX_ACT) {
         // lanes-over-j: a work item is (warp i-group, j-slice); resident = warps on the device
-        p.kernel = 1;
+        p.kernel = 1; p.unit = LJ_I; p.tile = LJ_TJ; p.ctas_per_sm = LJ_CTAS_PER_SM;
         p.n_units = (int)((n_act + LJ_I - 1) / LJ_I);
         const int64_t n_tiles = Npad / LJ_TJ;
         const int64_t resident = (int64_t)n_sm * LJ_CTAS_PER_SM * LJ_WARPS;
@@ -155,7 +155,7 @@ int nb_plan_force(int64_t N, int64_t n_act, int n_sm, nb_plan* plan)
         p.grid = (int)std::min<int64_t>((items + LJ_WARPS - 1) / LJ_WARPS, (int64_t)n_sm * LJ_CTAS_PER_SM);
     } else {
         // lanes-over-i: a work item is (i-tile of LI_UNIT particles, j-slice); resident = CTAs on the device
-        p.kernel = 0;
+        p.kernel = 0; p.unit = LI_UNIT; p.tile = LI_TJ; p.ctas_per_sm = LI_CTAS_PER_SM;
         p.n_units = (int)((n_act + LI_UNIT - 1) / LI_UNIT);
         const int64_t n_tiles = Npad / LI_TJ;
         const int64_t resident = (int64_t)n_sm * LI_CTAS_PER_SM;

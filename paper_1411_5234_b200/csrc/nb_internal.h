@@ -19,7 +19,7 @@ constexpr int NB_PAD = 256;          // particle arrays are padded to a multiple
 // parallelism, which measured faster than two particles per thread at 3 warps per scheduler.
 // The NB_* macros are build-time tunables (defaults = the measured best); -DNB_...=v overrides one for experiments.
 #ifndef NB_LI_THREADS
-#define NB_LI_THREADS 256
+#define NB_LI_THREADS 384
 #endif
 #ifndef NB_LI_I
 #define NB_LI_I 1
@@ -31,7 +31,7 @@ constexpr int NB_PAD = 256;          // particle arrays are padded to a multiple
 #define NB_LI_STAGES 2
 #endif
 #ifndef NB_LI_CTAS_PER_SM
-#define NB_LI_CTAS_PER_SM 3
+#define NB_LI_CTAS_PER_SM 2
 #endif
 #ifndef NB_LI_UNROLL
 #define NB_LI_UNROLL 2
