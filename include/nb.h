@@ -75,7 +75,8 @@ typedef enum {
 /* How nb_force maps an evaluation onto the GPU (reading R15; "Bfactor"). */
 typedef struct {
     int kernel;       /* 0 = lanes-over-i (each thread owns I active particles, j-tiles broadcast from shared memory)
-                         1 = lanes-over-j (each warp owns I active particles, its lanes take different j) */
+                         1 = lanes-over-j (each warp owns I active particles, its lanes take different j)
+                         2 = lanes-over-i with 32-particle units: the CTA's warps share the particles and split each j-tile */
     int n_units;      /* i-tiles (kernel 0) or i-groups per warp (kernel 1) */
     int n_split;      /* S: number of j-slices each unit is split into ("Bfactor") */
     int slice_tiles;  /* j-tiles per slice (the last slice may hold fewer) */
@@ -83,6 +84,8 @@ typedef struct {
     int unit;         /* active particles per unit (kernel 0: threads per CTA x I; kernel 1: I) */
     int tile;         /* j-records per j-tile (kernel 0: one shared-memory stage; kernel 1: one warp iteration) */
     int ctas_per_sm;  /* resident CTAs per multiprocessor the plan assumes */
+    int sub;          /* parts each j-tile is split into inside a CTA (kernel 2: warps per CTA; else 1); a unit
+                         writes n_split * sub partial sums */
     double waves;     /* work items / resident CTAs (or warps) on the device */
 } nb_plan;
 

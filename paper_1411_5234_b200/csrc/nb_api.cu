@@ -145,7 +145,7 @@ int nb_plan_force(int64_t N, int64_t n_act, int n_sm, nb_plan* plan)
     nb_plan p{};
     if (n_act <= LJ_MAX_ACT) {
         // lanes-over-j: a work item is (warp i-group, j-slice); resident = warps on the device
-        p.kernel = 1; p.unit = LJ_I; p.tile = LJ_TJ; p.ctas_per_sm = LJ_CTAS_PER_SM;
+        p.kernel = 1; p.unit = LJ_I; p.tile = LJ_TJ; p.ctas_per_sm = LJ_CTAS_PER_SM; p.sub = 1;
         p.n_units = (int)((n_act + LJ_I - 1) / LJ_I);
         const int64_t n_tiles = Npad / LJ_TJ;
         const int64_t resident = (int64_t)n_sm * LJ_CTAS_PER_SM * LJ_WARPS;
@@ -154,12 +154,15 @@ int nb_plan_force(int64_t N, int64_t n_act, int n_sm, nb_plan* plan)
         const int64_t items = (int64_t)p.n_units * p.n_split;
         p.grid = (int)std::min<int64_t>((items + LJ_WARPS - 1) / LJ_WARPS, (int64_t)n_sm * LJ_CTAS_PER_SM);
     } else {
-        // lanes-over-i: a work item is (i-tile of LI_UNIT particles, j-slice); resident = CTAs on the device
-        p.kernel = 0; p.unit = LI_UNIT; p.tile = LI_TJ; p.ctas_per_sm = LI_CTAS_PER_SM;
-        p.n_units = (int)((n_act + LI_UNIT - 1) / LI_UNIT);
+        // lanes-over-i: a work item is (i-tile, j-slice); resident = CTAs on the device.  Up to LIW_MAX_ACT active
+        // particles the i-tile is 32 particles and the CTA's warps each take a part of every j-tile (sub > 1).
+        const bool small = n_act <= LIW_MAX_ACT;
+        p.kernel = small ? 2 : 0; p.sub = small ? LI_W : 1;
+        p.unit = LI_UNIT / p.sub; p.tile = LI_TJ; p.ctas_per_sm = LI_CTAS_PER_SM;
+        p.n_units = (int)((n_act + p.unit - 1) / p.unit);
         const int64_t n_tiles = Npad / LI_TJ;
         const int64_t resident = (int64_t)n_sm * LI_CTAS_PER_SM;
-        const int64_t s_cap = rows / ((int64_t)p.n_units * LI_UNIT);
+        const int64_t s_cap = rows / ((int64_t)p.n_units * p.unit * p.sub);
         choose_split(p.n_units, n_tiles, resident, std::min<int64_t>(std::min<int64_t>(s_cap, 256), n_tiles / 2), 2, &p);
         const int64_t items = (int64_t)p.n_units * p.n_split;
         p.grid = (int)std::min<int64_t>(items, resident);
@@ -252,9 +255,10 @@ int nb_force(nb_ctx* ctx, const int32_t* active_idx, int64_t n_act, double* a, d
     A.idx = didx;
     A.n_act = (int)n_act;
     A.n_units = plan.n_units; A.n_split = plan.n_split; A.slice_tiles = plan.slice_tiles;
-    A.n_tiles = (int)(ctx->Npad / (plan.kernel == 0 ? LI_TJ : LJ_TJ));
+    A.n_tiles = (int)(ctx->Npad / plan.tile);
     A.n_items = plan.n_units * plan.n_split;
-    A.ld = plan.n_units * (plan.kernel == 0 ? LI_UNIT : LJ_I);
+    A.n_planes = plan.n_split * plan.sub;
+    A.ld = plan.n_units * plan.unit;
     A.eps2 = ctx->eps * ctx->eps;
     A.partial = ctx->L.partial;
     A.queue = ctx->L.queue;                                 // zeroed by nb_init, left at 0 by every launch

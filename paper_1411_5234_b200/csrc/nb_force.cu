@@ -57,7 +57,8 @@ __device__ __forceinline__ double twice(double c)
     return __hiloint2double(__double2hiint(c) + 0x00100000, __double2loint(c));
 }
 
-template <bool EPS0>
+// MASK = false: the caller knows that no lane meets its own record here (self is ignored).
+template <bool EPS0, bool MASK = true>
 __device__ __forceinline__ void pair(const IPart& pi, const double4 p0, const double4 p1, const double2 p2,
                                      const double eps2, const bool self, Sums& S)
 {
@@ -65,7 +66,7 @@ __device__ __forceinline__ void pair(const IPart& pi, const double4 p0, const do
     const double dvx = p1.x - pi.vx, dvy = p1.y - pi.vy, dvz = p1.z - pi.vz;
     const double dax = p1.w - pi.ax, day = p2.x - pi.ay, daz = p2.y - pi.az;
     double s = F(dx, dx, F(dy, dy, F(dz, dz, eps2)));
-    if (EPS0) s = self ? 1.0 : s;                        // eps = 0: keep the masked self pair finite
+    if (EPS0 && MASK) s = self ? 1.0 : s;                // eps = 0: keep the masked self pair finite
     // y = s^(-1/2): seed e0 ~ 2^-20, one cubic (Halley) step leaves 5/16 e0^3 < 2^-60
     const double y0 = rsqrt_seed(s);
     const double e = F(-s, M(y0, y0), 1.0);
@@ -94,7 +95,146 @@ __device__ __forceinline__ void pair(const IPart& pi, const double4 p0, const do
     S.ax = F(q, dx, S.ax); S.ay = F(q, dy, S.ay); S.az = F(q, dz, S.az);
     S.jx = F(q, ux, S.jx); S.jy = F(q, uy, S.jy); S.jz = F(q, uz, S.jz);
     S.sx = F(q, wx, S.sx); S.sy = F(q, wy, S.sy); S.sz = F(q, wz, S.sz);
-    S.p += self ? 0.0 : mr;                              // j != i (eq. 1); a, jerk, snap get exactly 0 from the self pair
+    S.p += (MASK && self) ? 0.0 : mr;                    // j != i (eq. 1); a, jerk, snap get exactly 0 from the self pair
+}
+
+// ---------------------------------------------------------------------------------------------
+// Two pairs (one i against records J[0], J[1]) with the ORDER of the FP64 instructions fixed by `asm volatile`.
+// Why: on sm_100a a DFMA that reads three different register pairs holds the FP64 pipe for 3 cycles, not 2.
+// It takes 2 only if one source is a duplicate, an immediate or uniform register, or comes from the
+// operand-reuse cache, i.e. the instruction issued just before it BY THE SAME WARP read that register in the
+// same operand slot (measured with DFMA chains).  Left to itself ptxas interleaves the pairs and
+// loses most of these reuses (28 of 64 DFMAs took 3 cycles).  Here every three-source DFMA sits in a run whose
+// neighbours share a source in the same slot, dependent instructions inside a run are >= 5 issue slots apart
+// (DFMA latency is 8 cycles = 4 slots), and what reads at most two registers (DADD, DMUL, the rsqrt refinement)
+// alternates between the two pairs; a stall there costs nothing while another warp has work.
+// 53 FP64 instructions per pair (32 DFMA + 11 DMUL + 10 DADD) + 1 MUFU.RSQ64H, as in pair().
+// ---------------------------------------------------------------------------------------------
+#define VSUB(d, a, b) asm volatile("sub.rn.f64 %0, %1, %2;" : "=d"(d) : "d"(a), "d"(b))
+#define VADD(d, a, b) asm volatile("add.rn.f64 %0, %1, %2;" : "=d"(d) : "d"(a), "d"(b))
+#define VMUL(d, a, b) asm volatile("mul.rn.f64 %0, %1, %2;" : "=d"(d) : "d"(a), "d"(b))
+#define VFMA(d, a, b, c) asm volatile("fma.rn.f64 %0, %1, %2, %3;" : "=d"(d) : "d"(a), "d"(b), "d"(c))
+#define VFNMA(d, a, b, c) /* d = c - a b */ \
+    asm volatile("{\n\t.reg .f64 n;\n\tneg.f64 n, %1;\n\tfma.rn.f64 %0, n, %2, %3;\n\t}" : "=d"(d) : "d"(a), "d"(b), "d"(c))
+#define VRSQ(d, a) asm volatile("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(d) : "d"(a))
+#define BOTH for (int k = 0; k < 2; ++k)
+
+struct JRec { double4 p0, p1; double2 p2; };
+
+template <bool EPS0, bool MASK>
+__device__ __forceinline__ void pair2(const IPart& pi, const JRec (&J)[2], const double eps2, const bool (&self)[2], Sums& S)
+{
+    // PIN(v): a branch that is never taken (v > 0) but that ptxas cannot see through.  The sums are live on its
+    // taken side, so the run of DFMAs that updates them cannot be moved across it: each pair's run stays in one piece.
+#ifndef NB_NO_PIN
+#define PIN(v) if (__double2hiint(v) < 0) return;
+#else
+#define PIN(v)
+#endif
+    double dx[2], dy[2], dz[2], dvx[2], dvy[2], dvz[2], dax[2], day[2], daz[2];
+    double s[2], rv[2], rv2[2], B[2], y0[2], t[2], e[2], h[2], y[2], yy[2], mr[2], z[2], q[2], c1[2], c2[2], c3[2];
+    // differences, with B = dv.dv (operands are duplicates: two-cycle DFMAs) threaded through them
+#pragma unroll
+    BOTH VSUB(dvz[k], J[k].p1.z, pi.vz);
+#pragma unroll
+    BOTH VSUB(dvy[k], J[k].p1.y, pi.vy);
+#pragma unroll
+    BOTH VSUB(dvx[k], J[k].p1.x, pi.vx);
+#pragma unroll
+    BOTH VMUL(B[k], dvz[k], dvz[k]);
+#pragma unroll
+    BOTH VSUB(dz[k], J[k].p0.z, pi.z);
+#pragma unroll
+    BOTH VSUB(daz[k], J[k].p2.y, pi.az);
+#pragma unroll
+    BOTH VFMA(B[k], dvy[k], dvy[k], B[k]);
+#pragma unroll
+    BOTH VSUB(dy[k], J[k].p0.y, pi.y);
+#pragma unroll
+    BOTH VSUB(day[k], J[k].p2.x, pi.ay);
+#pragma unroll
+    BOTH VFMA(B[k], dvx[k], dvx[k], B[k]);
+#pragma unroll
+    BOTH VSUB(dx[k], J[k].p0.x, pi.x);
+#pragma unroll
+    BOTH VSUB(dax[k], J[k].p1.w, pi.ax);
+    // s = dx.dx + eps2, rv = dx.dv, B += dx.da: runs of three that share d_c in slot A
+#pragma unroll
+    BOTH { VFMA(s[k], dz[k], dz[k], eps2); VMUL(rv[k], dz[k], dvz[k]); VFMA(B[k], dz[k], daz[k], B[k]); }
+#pragma unroll
+    BOTH { VFMA(s[k], dy[k], dy[k], s[k]); VFMA(rv[k], dy[k], dvy[k], rv[k]); VFMA(B[k], dy[k], day[k], B[k]); }
+#pragma unroll
+    BOTH { VFMA(s[k], dx[k], dx[k], s[k]); VFMA(rv[k], dx[k], dvx[k], rv[k]); VFMA(B[k], dx[k], dax[k], B[k]); }
+    if (EPS0 && MASK) {                                   // eps = 0: keep the masked self pair finite
+#pragma unroll
+        BOTH s[k] = self[k] ? 1.0 : s[k];
+    }
+    // y = s^(-1/2): MUFU.RSQ64H seed (e ~ 2^-20), then one cubic step y = y0 + y0 e (1/2 + 3/8 e), e = 1 - s y0^2,
+    // which leaves 5/16 e^3 < 2^-60
+#pragma unroll
+    BOTH VRSQ(y0[k], s[k]);
+#pragma unroll
+    BOTH VMUL(rv2[k], rv[k], rv[k]);
+#pragma unroll
+    BOTH VMUL(t[k], y0[k], y0[k]);
+#pragma unroll
+    BOTH VFNMA(e[k], s[k], t[k], 1.0);
+#pragma unroll
+    BOTH VFMA(h[k], e[k], 0.375, 0.5);
+#pragma unroll
+    BOTH VMUL(t[k], e[k], h[k]);
+#pragma unroll
+    BOTH VFMA(y[k], y0[k], t[k], y0[k]);
+    // scalars: yy = 1/s, mr = m_j/sqrt(s), q = m_j s^(-3/2), c1 = -3 alpha, c2 = -6 alpha, c3 = -3 beta
+    //          with alpha = rv/s, beta = B/s + alpha^2 = (B + rv^2/s)/s
+#pragma unroll
+    BOTH VMUL(yy[k], y[k], y[k]);
+#pragma unroll
+    BOTH VMUL(mr[k], y[k], J[k].p0.w);
+#pragma unroll
+    BOTH VMUL(z[k], yy[k], -3.0);
+#pragma unroll
+    BOTH { VMUL(q[k], mr[k], yy[k]); VFMA(B[k], rv2[k], yy[k], B[k]); }     // yy stays in slot B
+#pragma unroll
+    BOTH VMUL(c1[k], z[k], rv[k]);
+#pragma unroll
+    BOTH VMUL(c3[k], z[k], B[k]);
+#pragma unroll
+    BOTH c2[k] = twice(c1[k]);
+    PIN(s[0])
+    {
+        const double m0 = (MASK && self[0]) ? 0.0 : mr[0];   // j != i (eq. 1); a, jerk, snap get exactly 0 from the self pair
+        VADD(S.p, S.p, m0);
+    }
+    // u = dv + c1 dx, w = da + c3 dx + c2 u, sums += q (dx, u, w): 18 three-source DFMAs per pair in one run;
+    // each shares a source with its predecessor in the same slot (A: c1, c3, q, c2; B: d_c, u_c)
+#pragma unroll
+    BOTH {
+        double ux, uy, uz, wx, wy, wz;
+        VFMA(ux, c1[k], dx[k], dvx[k]);
+        VFMA(uy, c1[k], dy[k], dvy[k]);
+        VFMA(uz, c1[k], dz[k], dvz[k]);
+        VFMA(wz, c3[k], dz[k], daz[k]);
+        VFMA(wy, c3[k], dy[k], day[k]);
+        VFMA(wx, c3[k], dx[k], dax[k]);
+        VFMA(S.ax, q[k], dx[k], S.ax);
+        VFMA(S.ay, q[k], dy[k], S.ay);
+        VFMA(S.az, q[k], dz[k], S.az);
+        VFMA(S.jx, q[k], ux, S.jx);
+        VFMA(wx, c2[k], ux, wx);
+        VFMA(wy, c2[k], uy, wy);
+        VFMA(wz, c2[k], uz, wz);
+        VFMA(S.jz, q[k], uz, S.jz);
+        VFMA(S.jy, q[k], uy, S.jy);
+        VFMA(S.sx, q[k], wx, S.sx);
+        VFMA(S.sy, q[k], wy, S.sy);
+        VFMA(S.sz, q[k], wz, S.sz);
+        PIN(yy[k])
+        if (k == 0) {
+            const double m1 = (MASK && self[1]) ? 0.0 : mr[1];
+            VADD(S.p, S.p, m1);
+        }
+    }
 }
 
 __device__ __forceinline__ IPart load_ipart(const ForceArgs& A, int i)
@@ -106,7 +246,7 @@ __device__ __forceinline__ IPart load_ipart(const ForceArgs& A, int i)
 
 __device__ __forceinline__ void store_sums(const ForceArgs& A, int slice, int k, bool valid, const Sums& S)
 {
-    if (A.n_split > 1) {
+    if (A.n_planes > 1) {
         double* P = A.partial + (size_t)slice * 10 * A.ld + k;      // plane (slice, c) is contiguous in k
         const size_t ld = A.ld;
         P[0] = S.ax; P[ld] = S.ay; P[2 * ld] = S.az;
@@ -160,10 +300,17 @@ __device__ __forceinline__ void queue_retire(int* queue, int n_workers)
 // lanes-over-i
 // ---------------------------------------------------------------------------------------------
 static_assert((LI_STAGES & (LI_STAGES - 1)) == 0, "LI_STAGES must be a power of two");
+static_assert(LI_TJ % 2 == 0, "pair2 takes two j-records at a time");
 
-template <bool EPS0>
+// W = 1: a work item is (i-tile of LI_THREADS particles, j-slice).  W = 4 (17..96 active particles): the CTA's four
+// warps hold the SAME 32 particles and each takes its own quarter of every j-tile, so an item is (32 particles,
+// j-slice) and writes four partial planes (slice * 4 + warp) that the reduction adds like any other slices.
+template <bool EPS0, int W>
 __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(const ForceArgs A)
 {
+    constexpr int UNIT = LI_UNIT / W;                      // active particles per work item
+    constexpr int TJW = LI_TJ / W;                         // records of each j-tile one warp group takes
+    static_assert(W == 1 || (LI_I == 1 && UNIT == 32 && TJW % 2 == 0), "W > 1: one warp per group");
     __shared__ alignas(128) double4 s0[LI_STAGES][LI_TJ];
     __shared__ alignas(128) double4 s1[LI_STAGES][LI_TJ];
     __shared__ alignas(128) double2 s2[LI_STAGES][LI_TJ];
@@ -171,6 +318,8 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
     __shared__ int next_item;
 
     const int tid = threadIdx.x;
+    const int wg = W == 1 ? 0 : tid / UNIT;                // warp group: which part of each j-tile
+    const int til = W == 1 ? tid : tid % UNIT;             // lane within the i-tile
     if (tid == 0) {
         for (int s = 0; s < LI_STAGES; ++s) mbar_init(smem_u32(&full[s]), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -207,7 +356,7 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
         Sums acc[LI_I];
 #pragma unroll
         for (int q = 0; q < LI_I; ++q) {
-            const int k = unit * LI_UNIT + q * LI_THREADS + tid;
+            const int k = unit * UNIT + q * LI_THREADS + til;
             valid[q] = k < A.n_act;
             const int kk = valid[q] ? k : 0;
             ii[q] = A.idx ? A.idx[kk] : kk;
@@ -219,13 +368,32 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
             const uint32_t u = uses + t;
             const int st = u & (LI_STAGES - 1);
             mbar_wait(smem_u32(&full[st]), (u / LI_STAGES) & 1);
-            const int jbase = (t0 + t) * LI_TJ;
-#pragma unroll LI_UNROLL
-            for (int jj = 0; jj < LI_TJ; ++jj) {
-                const double4 p0 = s0[st][jj], p1 = s1[st][jj];
-                const double2 p2 = s2[st][jj];
+            const int jbase = (t0 + t) * LI_TJ + wg * TJW;
+            // the self pair (reading R4) lies in one j-tile per particle: only a warp that has one of its own
+            // particles in this tile runs the loop that masks by index
+            bool own = false;
 #pragma unroll
-                for (int q = 0; q < LI_I; ++q) pair<EPS0>(pi[q], p0, p1, p2, A.eps2, jbase + jj == ii[q], acc[q]);
+            for (int q = 0; q < LI_I; ++q) own |= (unsigned)(ii[q] - jbase) < (unsigned)TJW;
+            const double4 *t0p = &s0[st][wg * TJW], *t1p = &s1[st][wg * TJW];
+            const double2* t2p = &s2[st][wg * TJW];
+            if (__any_sync(0xffffffffu, own)) {
+#pragma unroll 1
+                for (int jj = 0; jj < TJW; jj += 2) {
+                    const JRec J[2] = {{t0p[jj], t1p[jj], t2p[jj]}, {t0p[jj + 1], t1p[jj + 1], t2p[jj + 1]}};
+#pragma unroll
+                    for (int q = 0; q < LI_I; ++q) {
+                        const bool self[2] = {jbase + jj == ii[q], jbase + jj + 1 == ii[q]};
+                        pair2<EPS0, true>(pi[q], J, A.eps2, self, acc[q]);
+                    }
+                }
+            } else {
+#pragma unroll 1
+                for (int jj = 0; jj < TJW; jj += 2) {
+                    const JRec J[2] = {{t0p[jj], t1p[jj], t2p[jj]}, {t0p[jj + 1], t1p[jj + 1], t2p[jj + 1]}};
+                    const bool self[2] = {false, false};
+#pragma unroll
+                    for (int q = 0; q < LI_I; ++q) pair2<EPS0, false>(pi[q], J, A.eps2, self, acc[q]);
+                }
             }
             __syncthreads();                                   // every warp is done with stage st
             if (tid == 0 && t + LI_STAGES < nt) stage_tile(t0 + t + LI_STAGES, st);
@@ -233,7 +401,7 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
         uses += nt;
 
 #pragma unroll
-        for (int q = 0; q < LI_I; ++q) store_sums(A, slice, unit * LI_UNIT + q * LI_THREADS + tid, valid[q], acc[q]);
+        for (int q = 0; q < LI_I; ++q) store_sums(A, slice * W + wg, unit * UNIT + q * LI_THREADS + til, valid[q], acc[q]);
     }
     if (tid == 0) queue_retire(A.queue, gridDim.x);
 }
@@ -301,20 +469,43 @@ __global__ void __launch_bounds__(LJ_THREADS, LJ_CTAS_PER_SM) force_lj_kernel(co
 }
 
 // ---------------------------------------------------------------------------------------------
-// partial-sum reduction: one thread per active particle, slices added in increasing order
+// partial-sum reduction (row a3).  T threads per active particle (T a power of two chosen from S on the host):
+// thread `lane` adds slices lane, lane + T, ... in increasing order, then the T lane sums are combined by a binary
+// tree in shared memory.  The order depends only on (S, T): bitwise reproducible.  T = 1 is the plain loop over
+// slices (large active sets, few slices: the loads of neighbouring threads coalesce over k).
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) reduce_partials_kernel(const ForceArgs A)
+constexpr int RED_THREADS = 256;
+
+__global__ void __launch_bounds__(RED_THREADS) reduce_partials_kernel(const ForceArgs A, const int T)
 {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= A.n_act) return;
+    __shared__ double sm[10][RED_THREADS];
+    const int R = RED_THREADS / T;                         // active particles per block
+    const int kl = threadIdx.x % R, lane = threadIdx.x / R;
+    const int k = blockIdx.x * R + kl;
     double r[10];
 #pragma unroll
     for (int c = 0; c < 10; ++c) r[c] = 0.0;
-    const double* P = A.partial + k;
-    for (int s = 0; s < A.n_split; ++s, P += (size_t)10 * A.ld) {
+    if (k < A.n_act) {
+        const size_t plane = (size_t)10 * A.ld;
+        const double* P = A.partial + (size_t)lane * plane + k;
+        for (int s = lane; s < A.n_planes; s += T, P += (size_t)T * plane) {
 #pragma unroll
-        for (int c = 0; c < 10; ++c) r[c] += P[(size_t)c * A.ld];
+            for (int c = 0; c < 10; ++c) r[c] += P[(size_t)c * A.ld];
+        }
     }
+    for (int off = T >> 1; off > 0; off >>= 1) {           // uniform over the block
+        if (lane >= off && lane < 2 * off) {
+#pragma unroll
+            for (int c = 0; c < 10; ++c) sm[c][threadIdx.x] = r[c];
+        }
+        __syncthreads();
+        if (lane < off) {
+#pragma unroll
+            for (int c = 0; c < 10; ++c) r[c] += sm[c][threadIdx.x + off * R];
+        }
+        __syncthreads();
+    }
+    if (lane != 0 || k >= A.n_act) return;
     A.out_a[3 * k] = r[0]; A.out_a[3 * k + 1] = r[1]; A.out_a[3 * k + 2] = r[2];
     A.out_j[3 * k] = r[3]; A.out_j[3 * k + 1] = r[4]; A.out_j[3 * k + 2] = r[5];
     A.out_s[3 * k] = r[6]; A.out_s[3 * k + 1] = r[7]; A.out_s[3 * k + 2] = r[8];
@@ -326,8 +517,11 @@ __global__ void __launch_bounds__(128) reduce_partials_kernel(const ForceArgs A)
 cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps_is_zero, cudaStream_t st, int* launches)
 {
     if (plan.kernel == 0) {
-        if (eps_is_zero) force_li_kernel<true><<<plan.grid, LI_THREADS, 0, st>>>(args);
-        else             force_li_kernel<false><<<plan.grid, LI_THREADS, 0, st>>>(args);
+        if (eps_is_zero) force_li_kernel<true, 1><<<plan.grid, LI_THREADS, 0, st>>>(args);
+        else             force_li_kernel<false, 1><<<plan.grid, LI_THREADS, 0, st>>>(args);
+    } else if (plan.kernel == 2) {
+        if (eps_is_zero) force_li_kernel<true, LI_W><<<plan.grid, LI_THREADS, 0, st>>>(args);
+        else             force_li_kernel<false, LI_W><<<plan.grid, LI_THREADS, 0, st>>>(args);
     } else {
         if (eps_is_zero) force_lj_kernel<true><<<plan.grid, LJ_THREADS, 0, st>>>(args);
         else             force_lj_kernel<false><<<plan.grid, LJ_THREADS, 0, st>>>(args);
@@ -335,8 +529,12 @@ cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps
     ++*launches;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    if (plan.n_split > 1) {
-        reduce_partials_kernel<<<(args.n_act + 127) / 128, 128, 0, st>>>(args);
+    if (args.n_planes > 1) {
+        // threads per particle: enough to spread S slices, few enough that large active sets keep coalesced rows
+        int T = 1;
+        while (T < RED_THREADS && T * 4 <= args.n_planes && (int64_t)args.n_act * T < (int64_t)1 << 18) T <<= 1;
+        const int R = RED_THREADS / T;
+        reduce_partials_kernel<<<(args.n_act + R - 1) / R, RED_THREADS, 0, st>>>(args, T);
         ++*launches;
         e = cudaGetLastError();
     }
@@ -345,6 +543,6 @@ cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps
 
 void nb_force_occupancy(int* li, int* lj)
 {
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(li, force_li_kernel<false>, LI_THREADS, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(li, force_li_kernel<false, 1>, LI_THREADS, 0);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(lj, force_lj_kernel<false>, LJ_THREADS, 0);
 }

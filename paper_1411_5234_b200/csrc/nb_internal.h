@@ -14,12 +14,13 @@
 
 constexpr int NB_PAD = 256;          // particle arrays are padded to a multiple of this
 
-// Both force kernels keep ONE active particle per thread (lanes-over-i) or per warp (lanes-over-j) in
-// 80 registers so that 24 warps (6 per scheduler) are resident per SM: the FP64 pipe is fed by warp-level
-// parallelism, which measured faster than two particles per thread at 3 warps per scheduler.
+// Both force kernels keep ONE active particle per thread (lanes-over-i) or per warp (lanes-over-j).  The
+// lanes-over-i kernel evaluates two j-records at a time with a fixed instruction order (pair2, nb_force.cu): 112
+// registers, 16 warps (4 per scheduler) per SM as 4 CTAs of 128 threads; CTA shapes that leave the four
+// schedulers with unequal warp counts (5 x 96, 3 x 160) measured 15-27 % slower.
 // The NB_* macros are build-time tunables (defaults = the measured best); -DNB_...=v overrides one for experiments.
 #ifndef NB_LI_THREADS
-#define NB_LI_THREADS 384
+#define NB_LI_THREADS 128
 #endif
 #ifndef NB_LI_I
 #define NB_LI_I 1
@@ -31,33 +32,32 @@ constexpr int NB_PAD = 256;          // particle arrays are padded to a multiple
 #define NB_LI_STAGES 2
 #endif
 #ifndef NB_LI_CTAS_PER_SM
-#define NB_LI_CTAS_PER_SM 2
-#endif
-#ifndef NB_LI_UNROLL
-#define NB_LI_UNROLL 2
+#define NB_LI_CTAS_PER_SM 4
 #endif
 // lanes-over-i kernel: each thread owns LI_I active particles, a CTA streams j-tiles through smem
 constexpr int LI_THREADS = NB_LI_THREADS;
 constexpr int LI_I = NB_LI_I;
 constexpr int LI_UNIT = LI_THREADS * LI_I;   // active particles per i-tile
-constexpr int LI_TJ = NB_LI_TJ;              // j-records per smem stage (80 B each)
+constexpr int LI_TJ = NB_LI_TJ;              // j-records per smem stage (80 B each), even
 constexpr int LI_STAGES = NB_LI_STAGES;
 constexpr int LI_CTAS_PER_SM = NB_LI_CTAS_PER_SM;
-constexpr int LI_UNROLL = NB_LI_UNROLL;       // j-loop unroll factor
+constexpr int LI_W = LI_THREADS / 32;        // small active sets: the CTA's warps share 32 particles and split each j-tile
 // lanes-over-j kernel: each warp owns LJ_I active particles, lanes take different j
 constexpr int LJ_THREADS = 256;
 constexpr int LJ_WARPS = LJ_THREADS / 32;
 constexpr int LJ_I = 1;
 constexpr int LJ_TJ = 32;                    // j-records per warp iteration
 constexpr int LJ_CTAS_PER_SM = 3;
-constexpr int64_t LJ_MAX_ACT = 1024;         // n_act <= this -> lanes-over-j
+constexpr int64_t LJ_MAX_ACT = 16;           // n_act <= this -> lanes-over-j
+constexpr int64_t LIW_MAX_ACT = 96;          // n_act <= this -> lanes-over-i with 32-particle units (above, a 128-lane i-tile is >= 75 % full)
 
 struct ForceArgs {
     const double4* pj0; const double4* pj1; const double2* pj2;   // predicted records (padded)
     const int32_t* idx;      // active indices or nullptr (i = k)
     int n_act;
     int n_units;             // i-tiles (LI) or warp i-groups (LJ)
-    int n_split;             // S
+    int n_split;             // S: j-slices per unit
+    int n_planes;            // partial planes per unit = S x sub-slices (1: results are written directly)
     int slice_tiles;         // j-tiles per slice
     int n_tiles;             // total j-tiles (Npad / TJ)
     int n_items;             // n_units * n_split

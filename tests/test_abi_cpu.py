@@ -33,7 +33,7 @@ def test_struct_layouts_match_header(B):
     # nb_config: int, void*, void*, size_t, int, double, double, int, int  (natural alignment)
     assert C.sizeof(B.nb_config) == 64
     assert B.nb_config.workspace.offset == 16 and B.nb_config.eta.offset == 40 and B.nb_config.k_max.offset == 60
-    assert C.sizeof(B.nb_plan) == 40
+    assert C.sizeof(B.nb_plan) == 48 and B.nb_plan.waves.offset == 40
 
 
 def test_workspace_bytes(B):
@@ -47,18 +47,19 @@ def test_workspace_bytes(B):
 
 @pytest.mark.parametrize("N", [1, 2, 255, 1024, 5000, 65536, 262144, 1 << 20])
 def test_plan_invariants(B, N):
-    for n_act in sorted({1, 2, 7, 64, 512, 1024, 1025, 4096, 32768, N // 3 + 1, N} & set(range(1, N + 1)) | {N}):
+    for n_act in sorted({1, 2, 7, 16, 17, 64, 96, 97, 512, 1024, 1025, 4096, 32768, N // 3 + 1, N} & set(range(1, N + 1)) | {N}):
         for n_sm in (148, 132, 8):
             p = B.nb_plan_force(N, n_act, n_sm)
             Npad = (N + 255) // 256 * 256
-            assert p.kernel == (1 if n_act <= 1024 else 0)
+            assert p.kernel == (1 if n_act <= 16 else 2 if n_act <= 96 else 0)
+            assert p.sub == (4 if p.kernel == 2 else 1) and p.unit == (1 if p.kernel == 1 else 128 // p.sub)
             unit, n_tiles = p.unit, Npad // p.tile
             assert unit >= 1 and Npad % p.tile == 0 and p.n_units == (n_act + unit - 1) // unit
             assert 1 <= p.ctas_per_sm <= 32 and p.grid <= n_sm * p.ctas_per_sm
             S, st = p.n_split, p.slice_tiles
             assert S >= 1 and st >= 1 and p.grid >= 1
             assert S * st >= n_tiles and (S - 1) * st < n_tiles            # slices cover all j-tiles, none empty
-            assert S * p.n_units * unit <= 8 * Npad + (1 << 19)            # partial-sum buffer capacity
+            assert S * p.sub * p.n_units * unit <= 8 * Npad + (1 << 19)    # partial-sum buffer capacity
             # small active sets are split so that the device is filled
             resident = n_sm * p.ctas_per_sm * (8 if p.kernel == 1 else 1)
             if p.n_units < resident and n_tiles >= 16 * resident:

@@ -92,14 +92,14 @@ def test_force_parity_active_sets(B, oracle, N, eps, masses):
     g.nb_predict(2.0 ** -9); g.nb_force(outputs=False); g.nb_corrector(None, 2.0 ** -9)
     g.nb_predict(2.0 ** -9 + 2.0 ** -11)
     rng = np.random.default_rng(N)
-    sizes = sorted({1, 2, 3, 31, 33, 64, 255, 1023, 1024, 1025, 2049, N} & set(range(1, N + 1)) | {N})
+    sizes = sorted({1, 2, 3, 16, 17, 31, 33, 64, 96, 97, 129, 255, 1023, 1024, 1025, 2049, N} & set(range(1, N + 1)) | {N})
     for n_act in sizes:
         idx = None if n_act == N else rng.choice(N, n_act, replace=False).astype(np.int32)
         got = g.nb_force(idx)
         ref = oracle_on_gpu_records(oracle, g, eps, idx)
         assert_force_parity(got, ref)
         plan = B.nb_plan_force(N, n_act, 148)
-        assert plan.kernel == (1 if n_act <= 1024 else 0)
+        assert plan.kernel == (1 if n_act <= 16 else 2 if n_act <= 96 else 0)   # all three kernel shapes
     # permuted full list: row k <-> idx[k]
     perm = rng.permutation(N).astype(np.int32)
     got = g.nb_force(perm)
