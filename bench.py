@@ -31,10 +31,12 @@ from paper_1411_5234_b200 import workloads as W  # noqa: E402
 
 METRIC = "fp64 pairwise interactions/s (acc+jerk+snap) at N=2^20"
 UNIT = "interactions/s"
-FLOP_EXEC = 86   # 2*32 DFMA + 11 DMUL + 11 DADD per interaction, counted from the shipped SASS
+FLOP_EXEC = 86   # algorithmic flop per interaction: 2*32 FMA + 11 MUL + 11 ADD.  The shipped SASS executes 85 of them
+                 # on the FP64 pipe (32 DFMA + 11 DMUL + 10 DADD) and one (2 c1) as an exponent increment on the integer pipe
 FLOP_CONV = 97   # customary acc+jerk+snap operation count of the Hermite-6 literature (a labelled convention)
 FP64_LANES_PER_SM = 64
 DT_BENCH = 2.0 ** -14
+TRAFFIC_NCU_BYTES = 652.8e6 + 646.1e6   # per force launch at N = 2^20, from the committed ncu capture (profiles/)
 
 
 def n_cores() -> int:
@@ -259,13 +261,15 @@ def run_ours(args, cfg_dict):
     peak_measured, _ = B.nb_probe_fp64_peak(1.0, local)
     f_ms = float(np.mean(force_ms))
     achieved = FLOP_EXEC * inter_per_step / (f_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "force_li_kernel<false> (+ reduce_partials_kernel)", "achieved": achieved,
+    roofline = {"bound": "alu", "kernel": "force_li_kernel<false, 1> (+ reduce_partials_kernel)", "achieved": achieved,
                 "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
                 "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max_mhz:.0f} MHz (DESIGN.md)",
                 "peak_measured_dfma": peak_measured, "frac_of_measured_dfma": achieved / peak_measured,
                 "flop_per_interaction": FLOP_EXEC, "tflops_conv97": FLOP_CONV * inter_per_step / (f_ms * 1e-3) / 1e12,
                 "kernel_ms": f_ms, "kernel_share_of_step": f_ms * args.steps / ms,
-                "interactions_per_s_kernel": inter_per_step / (f_ms * 1e-3), "traffic": None}
+                "interactions_per_s_kernel": inter_per_step / (f_ms * 1e-3),
+                "traffic": TRAFFIC_NCU_BYTES if N == W.CONFIGS[4].N else None,
+                "traffic_source": "profiles/r01_force_li_full.md (dram__bytes_read.sum + dram__bytes_write.sum, one ncu --set full capture)"}
 
     # ---- the oracle timed beside it (rank 0, bounded sample)
     cpu_val, sample = time_oracle_sample(m, x, v, np.zeros_like(x), c.eps, args.cpu_seconds, 31)
@@ -296,7 +300,7 @@ def main():
                             "all N active; step = nb_predict + nb_force(all) + nb_corrector(all)",
                 "N": N, "n_act": N, "eps": 1e-4, "dt": DT_BENCH,
                 "parallelism": "single GPU" if args.gpus == 1 else f"{args.gpus} independent replicas",
-                "l2": "per-step working set (state 168 MB + j-records 84 MB + partial sums 335 MB + results 84 MB) exceeds the 126 MB L2"}
+                "l2": "per-step working set (state 168 MB + j-records 84 MB + partial sums 671 MB + results 84 MB) exceeds the 126 MB L2"}
     if args.impl == "reference":
         run_reference(args, cfg_dict)
     else:

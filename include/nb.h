@@ -96,6 +96,10 @@ size_t nb_workspace_bytes(int64_t N);
  * with n_sm multiprocessors.  NB_EINVAL on bad sizes. */
 int nb_plan_force(int64_t N, int64_t n_act, int n_sm, nb_plan* plan);
 
+/* Cap the j-split S of this context's nb_force / nb_run_blocks launches: 0 (default) = the cost model decides,
+ * 1 = no split (the "Bfactor off" arm of the paper's Fig. 1), k = at most k slices. */
+int nb_set_max_split(nb_ctx* ctx, int64_t max_split);
+
 /*
  * nb_init — create a system from the initial conditions of eq. (1): masses m[N],
  * positions x[N][3], velocities v[N][3] (h/d), softening eps >= 0 of eq. (2).
@@ -154,6 +158,20 @@ int nb_next_block(nb_ctx* ctx, double* t_next, int32_t* active_idx, int64_t* n_a
 /* Pass as active_idx to use the list the last nb_next_block left inside the context. */
 #define NB_ACTIVE_INTERNAL ((const int32_t*)(uintptr_t)1)
 
+/*
+ * nb_run_blocks — advance the system by whole block steps without the host in the loop:
+ * repeats { nb_next_block; stop if t_next > t_end; nb_predict(t_next); nb_force(internal list);
+ * nb_corrector(internal list, per-particle dt) } at most max_steps times.  Every decision of a step -
+ * t_next, the active list, n_act, the j-split of the force launch (reading R15; "determined
+ * step by step") - is taken on the device, and one step is one replay of a CUDA graph; the host enqueues
+ * batches of replays and reads the counters after each batch.  The arithmetic and its order are those of
+ * the separate calls: states agree bit for bit.
+ * steps_done, t_last (time of the last completed step; -1 if none), sum_n_act (sum of n_act over the
+ * steps: interactions = sum_n_act * (N - 1)): HOST pointers, any may be NULL.  Synchronises the stream.
+ */
+int nb_run_blocks(nb_ctx* ctx, double t_end, int64_t max_steps, int64_t* steps_done, double* t_last,
+                  int64_t* sum_n_act);
+
 /* Read / write one field for the particles idx[0..n) (h/d; NULL = the first n in index order). */
 int nb_get_state(nb_ctx* ctx, int field, const int32_t* idx, int64_t n, double* out);
 int nb_set_state(nb_ctx* ctx, int field, const int32_t* idx, int64_t n, const double* in);
@@ -173,6 +191,16 @@ int nb_energy(nb_ctx* ctx, double* kinetic, double* potential);
  */
 int nb_probe_fp64_peak(int device, void* stream, void* workspace, size_t workspace_bytes,
                        double seconds, double* tflops, int* n_sm);
+
+/*
+ * nb_probe_dfma_sources — measurement aid: cycles one warp-wide DFMA holds the FP64 pipe of an SM
+ * sub-partition, from a stream of independent DFMAs whose sources are (kind 0) one register and two
+ * constants, (kind 1) three different registers, (kind 2) three registers of which one is shared by
+ * the whole run, so that the operand-reuse cache can supply it.  sm_mhz: the SM clock to convert with.
+ * These are the numbers behind the pipe model of DESIGN.md section 6.  workspace: >= 64 KiB, device.
+ */
+int nb_probe_dfma_sources(int device, void* stream, void* workspace, size_t workspace_bytes, int kind,
+                          double sm_mhz, double* cycles);
 
 /* Kernel launches issued by this context so far (what bench.py reports as gpu_launches). */
 int64_t nb_launch_count(const nb_ctx* ctx);

@@ -20,8 +20,8 @@ FIELDS = dict(M=0, X=1, V=2, A=3, J=4, S=5, C=6, T=7, DT=8, XP=9, VP=10, AP=11)
 _WIDTH = {0: 1, 7: 1, 8: 1}
 ACTIVE_INTERNAL = C.c_void_p(1)
 
-EXPORTS = ["nb_workspace_bytes", "nb_plan_force", "nb_init", "nb_predict", "nb_force", "nb_corrector",
-           "nb_next_block", "nb_get_state", "nb_set_state", "nb_energy", "nb_probe_fp64_peak",
+EXPORTS = ["nb_workspace_bytes", "nb_plan_force", "nb_set_max_split", "nb_init", "nb_predict", "nb_force", "nb_corrector",
+           "nb_next_block", "nb_run_blocks", "nb_get_state", "nb_set_state", "nb_energy", "nb_probe_fp64_peak", "nb_probe_dfma_sources",
            "nb_launch_count", "nb_last_force_ms", "nb_strerror", "nb_last_error", "nb_free"]
 
 
@@ -58,16 +58,20 @@ def lib() -> C.CDLL:
     vp, i64, dbl = C.c_void_p, C.c_int64, C.c_double
     L.nb_workspace_bytes.argtypes = [i64]; L.nb_workspace_bytes.restype = C.c_size_t
     L.nb_plan_force.argtypes = [i64, i64, C.c_int, C.POINTER(nb_plan)]; L.nb_plan_force.restype = C.c_int
+    L.nb_set_max_split.argtypes = [vp, i64]; L.nb_set_max_split.restype = C.c_int
     L.nb_init.argtypes = [C.POINTER(vp), i64, vp, vp, vp, dbl, C.POINTER(nb_config)]; L.nb_init.restype = C.c_int
     L.nb_predict.argtypes = [vp, dbl]; L.nb_predict.restype = C.c_int
     L.nb_force.argtypes = [vp, vp, i64, vp, vp, vp, vp]; L.nb_force.restype = C.c_int
     L.nb_corrector.argtypes = [vp, vp, i64, dbl]; L.nb_corrector.restype = C.c_int
     L.nb_next_block.argtypes = [vp, C.POINTER(dbl), vp, C.POINTER(i64)]; L.nb_next_block.restype = C.c_int
+    L.nb_run_blocks.argtypes = [vp, dbl, i64, C.POINTER(i64), C.POINTER(dbl), C.POINTER(i64)]; L.nb_run_blocks.restype = C.c_int
     L.nb_get_state.argtypes = [vp, C.c_int, vp, i64, vp]; L.nb_get_state.restype = C.c_int
     L.nb_set_state.argtypes = [vp, C.c_int, vp, i64, vp]; L.nb_set_state.restype = C.c_int
     L.nb_energy.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl)]; L.nb_energy.restype = C.c_int
     L.nb_probe_fp64_peak.argtypes = [C.c_int, vp, vp, C.c_size_t, dbl, C.POINTER(dbl), C.POINTER(C.c_int)]
     L.nb_probe_fp64_peak.restype = C.c_int
+    L.nb_probe_dfma_sources.argtypes = [C.c_int, vp, vp, C.c_size_t, C.c_int, dbl, C.POINTER(dbl)]
+    L.nb_probe_dfma_sources.restype = C.c_int
     L.nb_launch_count.argtypes = [vp]; L.nb_launch_count.restype = i64
     L.nb_last_force_ms.argtypes = [vp]; L.nb_last_force_ms.restype = dbl
     L.nb_strerror.argtypes = [C.c_int]; L.nb_strerror.restype = C.c_char_p
@@ -183,6 +187,9 @@ class System:
             n, ip = int(active_idx.shape[0]), _ptr(active_idx)
         self._check(self.L.nb_corrector(self.ctx, ip, n, float(dt)))
 
+    def nb_set_max_split(self, max_split):
+        self._check(self.L.nb_set_max_split(self.ctx, int(max_split)))
+
     def nb_next_block(self, want_list=True):
         t, n = C.c_double(), C.c_int64()
         if not want_list:
@@ -194,6 +201,12 @@ class System:
             buf = self._torch.empty(self.N, dtype=self._torch.int32, device=f"cuda:{self.device}")
         self._check(self.L.nb_next_block(self.ctx, C.byref(t), _ptr(buf), C.byref(n)))
         return t.value, n.value, buf[:n.value]
+
+    def nb_run_blocks(self, t_end, max_steps=1 << 62):
+        """Returns (steps_done, t_last, sum_n_act)."""
+        steps, t_last, sum_act = C.c_int64(), C.c_double(), C.c_int64()
+        self._check(self.L.nb_run_blocks(self.ctx, float(t_end), int(max_steps), C.byref(steps), C.byref(t_last), C.byref(sum_act)))
+        return steps.value, t_last.value, sum_act.value
 
     def nb_get_state(self, field, idx=None, n=None):
         f = FIELDS[field] if isinstance(field, str) else field
@@ -248,3 +261,20 @@ def nb_probe_fp64_peak(seconds=1.0, device=0):
     if rc != NB_OK:
         raise NBError(rc, lib().nb_strerror(rc).decode())
     return tf.value, nsm.value
+
+
+def nb_probe_dfma_sources(sm_mhz, device=0):
+    """Cycles per warp-wide DFMA and SM sub-partition for 2-source, 3-source and 3-source-with-reuse streams."""
+    import torch
+    torch.cuda.set_device(device)
+    ws = torch.empty(65536 + 256, dtype=torch.uint8, device=f"cuda:{device}")
+    base = (ws.data_ptr() + 255) // 256 * 256
+    out = {}
+    for kind, name in enumerate(("two_sources", "three_sources", "three_sources_one_reused")):
+        cyc = C.c_double()
+        rc = lib().nb_probe_dfma_sources(device, C.c_void_p(torch.cuda.current_stream(device).cuda_stream), C.c_void_p(base), 65536,
+                                         kind, float(sm_mhz), C.byref(cyc))
+        if rc != NB_OK:
+            raise NBError(rc, lib().nb_strerror(rc).decode())
+        out[name] = cyc.value
+    return out

@@ -8,13 +8,14 @@
 #include <new>
 
 #include "nb_internal.h"
+#include "nb_plan.h"
 
 namespace {
 
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t x, size_t a = ALIGN) { return (x + a - 1) / a * a; }
-inline int64_t pad_n(int64_t N) { return (N + NB_PAD - 1) / NB_PAD * NB_PAD; }
-inline int64_t partial_rows(int64_t Npad) { return 8 * Npad + (int64_t(1) << 19); }
+inline int64_t pad_n(int64_t N) { return nb_pad_n(N); }
+inline int64_t partial_rows(int64_t Npad) { return nb_partial_rows(Npad); }
 inline size_t scratch_bytes(int64_t Npad) { return 65536 + (size_t)Npad / 8; }
 
 struct Carve {
@@ -33,6 +34,7 @@ struct Layout {
     double* stage;                      // staging for host <-> device transfers, 10 doubles per particle
     char* scratch;
     int* queue;                         // work queue of the force kernels (2 counters)
+    DevPlan* devplan;                   // plan and counters of the device-planned block steps (nb_run_blocks)
     size_t bytes;
     Layout(void* base, int64_t Npad)
     {
@@ -46,6 +48,7 @@ struct Layout {
         stage = c.take<double>(10 * Npad);
         scratch = c.take<char>(scratch_bytes(Npad));
         queue = c.take<int>(64);
+        devplan = c.take<DevPlan>(1);
         bytes = c.off;
     }
 };
@@ -60,6 +63,7 @@ struct nb_ctx {
     double eps = 0, eta = 0.45, eta_s = 0.01;
     int k_min = -20, k_max = -3;
     int n_sm = 148;
+    int64_t max_split = 0;         // cap on the j-split (0: the cost model decides)
     Layout L{nullptr, 0};
     double t_pred = 0;
     bool predicted = false;        // predicted records are valid
@@ -67,6 +71,7 @@ struct nb_ctx {
     int64_t sched_n = -1;          // length of the internal active list (-1: none)
     int64_t launches = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    cudaGraphExec_t step_graph = nullptr;   // one device-planned block step (built on first use)
     bool ev_valid = false;
     char err[256] = {0};
 };
@@ -79,6 +84,49 @@ int fail_cuda(nb_ctx* c, cudaError_t e, const char* where)
     return NB_ECUDA;
 }
 #define CU(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail_cuda(ctx, e_, where); } while (0)
+
+// the fields of ForceArgs that do not depend on the plan
+ForceArgs base_force_args(const nb_ctx* ctx)
+{
+    ForceArgs A{};
+    A.pj0 = ctx->L.s.pj0; A.pj1 = ctx->L.s.pj1; A.pj2 = ctx->L.s.pj2;
+    A.eps2 = ctx->eps * ctx->eps;
+    A.partial = ctx->L.partial;
+    A.queue = ctx->L.queue;                                 // zeroed by nb_init, left at 0 by every launch
+    A.out_a = ctx->L.fa; A.out_j = ctx->L.fj; A.out_s = ctx->L.fs; A.out_p = ctx->L.fp;
+    return A;
+}
+
+// One block step with every decision taken on the device, captured once as a CUDA graph: scheduler (+ plan of the
+// force launch) -> predictor -> the three force kernel shapes (two of them return at once) -> reduction -> corrector.
+constexpr int STEP_GRAPH_KERNELS = 9;
+
+int build_step_graph(nb_ctx* ctx)
+{
+    cudaStream_t cs;                                        // capture needs a non-default stream; nothing runs on it
+    CU(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking), "capture stream");
+    cudaGraph_t graph = nullptr;
+    int launches = 0;
+    cudaError_t e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
+    if (e == cudaSuccess) {
+        ForceArgs A = base_force_args(ctx);
+        A.idx = ctx->L.idx_sched;
+        A.n_tiles = 0;                                      // set per kernel below
+        A.dp = ctx->L.devplan;
+        e = nb_launch_devstep_head(ctx->L.s, ctx->N, ctx->Npad, ctx->n_sm, ctx->L.idx_sched, ctx->L.scratch, ctx->L.devplan, cs, &launches);
+        if (e == cudaSuccess) e = nb_launch_force_devplan(A, ctx->eps == 0.0, ctx->n_sm, (int)ctx->Npad, cs, &launches);
+        if (e == cudaSuccess)
+            e = nb_launch_devstep_tail(ctx->L.s, ctx->n_sm, ctx->L.idx_sched, ctx->L.scratch, ctx->L.devplan, ctx->L.fa, ctx->L.fj, ctx->L.fs,
+                                       ctx->eta, ctx->k_min, ctx->k_max, cs, &launches);
+        const cudaError_t e2 = cudaStreamEndCapture(cs, &graph);
+        if (e == cudaSuccess) e = e2;
+    }
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&ctx->step_graph, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    cudaStreamDestroy(cs);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "block-step graph");
+    return launches == STEP_GRAPH_KERNELS ? NB_OK : NB_ECUDA;
+}
 
 // device pointer to n_act indices: uploads a host list into `buf`, or passes a device list through
 int resolve_idx(nb_ctx* ctx, const int32_t* idx, int64_t n, int32_t* buf, const int32_t** out)
@@ -103,30 +151,6 @@ int copy_out(nb_ctx* ctx, double* dst, const double* src, size_t count)
     return NB_OK;
 }
 
-// Split chosen by a cost model (reading R15), in units of one j-tile of work on one work slot.  Work items
-// (unit, slice) are pulled from a queue by `resident` workers (CTAs or warps); an item costs
-// slice_tiles + fixed.  Up to a few rounds the last round is counted whole; beyond that the queue balances
-// the workers up to a tail of about one item.
-void choose_split(int64_t n_units, int64_t n_tiles, int64_t resident, int64_t s_max, int fixed, nb_plan* p)
-{
-    int64_t best_S = 1, best_tiles = n_tiles;
-    double best_cost = 1e300;
-    s_max = std::max<int64_t>(1, std::min(s_max, n_tiles));
-    for (int64_t S = 1; S <= s_max; ++S) {
-        const int64_t st = (n_tiles + S - 1) / S;
-        const int64_t S_eff = (n_tiles + st - 1) / st;           // slices that are not empty
-        if (S_eff != S) continue;
-        const int64_t items = n_units * S;
-        const double rounds = items <= 4 * resident ? (double)((items + resident - 1) / resident)
-                                                    : (double)items / (double)resident + 0.7;
-        const double cost = rounds * (double)(st + fixed);
-        if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best_S = S; best_tiles = st; }
-    }
-    p->n_split = (int)best_S;
-    p->slice_tiles = (int)best_tiles;
-    p->waves = (double)(n_units * best_S) / (double)resident;
-}
-
 }  // namespace
 
 extern "C" {
@@ -137,37 +161,31 @@ size_t nb_workspace_bytes(int64_t N)
     return Layout(nullptr, pad_n(N)).bytes;
 }
 
-int nb_plan_force(int64_t N, int64_t n_act, int n_sm, nb_plan* plan)
+static int plan_force(int64_t N, int64_t n_act, int n_sm, int64_t max_split, nb_plan* plan)
 {
-    if (!plan || N < 1 || n_act < 1 || n_act > N || n_sm < 1 || N > (int64_t(1) << 30)) return NB_EINVAL;
-    const int64_t Npad = pad_n(N);
-    const int64_t rows = partial_rows(Npad);
+    if (!plan || N < 1 || n_act < 1 || n_act > N || n_sm < 1 || N > (int64_t(1) << 30) || max_split < 0) return NB_EINVAL;
+    const PlanShape sh = nb_plan_shape(pad_n(N), n_act, n_sm, max_split);
+    double cost;
+    const int64_t S = nb_best_split(sh, 1, 1, &cost);
+    int64_t st;
+    nb_split_cost(sh, S, &st);
     nb_plan p{};
-    if (n_act <= LJ_MAX_ACT) {
-        // lanes-over-j: a work item is (warp i-group, j-slice); resident = warps on the device
-        p.kernel = 1; p.unit = LJ_I; p.tile = LJ_TJ; p.ctas_per_sm = LJ_CTAS_PER_SM; p.sub = 1;
-        p.n_units = (int)((n_act + LJ_I - 1) / LJ_I);
-        const int64_t n_tiles = Npad / LJ_TJ;
-        const int64_t resident = (int64_t)n_sm * LJ_CTAS_PER_SM * LJ_WARPS;
-        const int64_t s_cap = rows / ((int64_t)p.n_units * LJ_I);
-        choose_split(p.n_units, n_tiles, resident, std::min<int64_t>(s_cap, n_tiles / 4), 6, &p);
-        const int64_t items = (int64_t)p.n_units * p.n_split;
-        p.grid = (int)std::min<int64_t>((items + LJ_WARPS - 1) / LJ_WARPS, (int64_t)n_sm * LJ_CTAS_PER_SM);
-    } else {
-        // lanes-over-i: a work item is (i-tile, j-slice); resident = CTAs on the device.  Up to LIW_MAX_ACT active
-        // particles the i-tile is 32 particles and the CTA's warps each take a part of every j-tile (sub > 1).
-        const bool small = n_act <= LIW_MAX_ACT;
-        p.kernel = small ? 2 : 0; p.sub = small ? LI_W : 1;
-        p.unit = LI_UNIT / p.sub; p.tile = LI_TJ; p.ctas_per_sm = LI_CTAS_PER_SM;
-        p.n_units = (int)((n_act + p.unit - 1) / p.unit);
-        const int64_t n_tiles = Npad / LI_TJ;
-        const int64_t resident = (int64_t)n_sm * LI_CTAS_PER_SM;
-        const int64_t s_cap = rows / ((int64_t)p.n_units * p.unit * p.sub);
-        choose_split(p.n_units, n_tiles, resident, std::min<int64_t>(std::min<int64_t>(s_cap, 256), n_tiles / 2), 2, &p);
-        const int64_t items = (int64_t)p.n_units * p.n_split;
-        p.grid = (int)std::min<int64_t>(items, resident);
-    }
+    p.kernel = sh.kernel; p.unit = sh.unit; p.tile = sh.tile; p.sub = sh.sub; p.ctas_per_sm = sh.ctas_per_sm;
+    p.n_units = (int)sh.n_units; p.n_split = (int)S; p.slice_tiles = (int)st;
+    const int64_t items = sh.n_units * S;
+    p.waves = (double)items / (double)sh.resident;
+    p.grid = sh.kernel == 1 ? (int)std::min<int64_t>((items + LJ_WARPS - 1) / LJ_WARPS, (int64_t)n_sm * LJ_CTAS_PER_SM)
+                            : (int)std::min<int64_t>(items, sh.resident);
     *plan = p;
+    return NB_OK;
+}
+
+int nb_plan_force(int64_t N, int64_t n_act, int n_sm, nb_plan* plan) { return plan_force(N, n_act, n_sm, 0, plan); }
+
+int nb_set_max_split(nb_ctx* ctx, int64_t max_split)
+{
+    if (!ctx || max_split < 0) return NB_EINVAL;
+    ctx->max_split = max_split;
     return NB_OK;
 }
 
@@ -247,11 +265,10 @@ int nb_force(nb_ctx* ctx, const int32_t* active_idx, int64_t n_act, double* a, d
     if (rc != NB_OK) return rc;
 
     nb_plan plan;
-    rc = nb_plan_force(ctx->N, n_act, ctx->n_sm, &plan);
+    rc = plan_force(ctx->N, n_act, ctx->n_sm, ctx->max_split, &plan);
     if (rc != NB_OK) return rc;
 
-    ForceArgs A{};
-    A.pj0 = ctx->L.s.pj0; A.pj1 = ctx->L.s.pj1; A.pj2 = ctx->L.s.pj2;
+    ForceArgs A = base_force_args(ctx);
     A.idx = didx;
     A.n_act = (int)n_act;
     A.n_units = plan.n_units; A.n_split = plan.n_split; A.slice_tiles = plan.slice_tiles;
@@ -259,10 +276,6 @@ int nb_force(nb_ctx* ctx, const int32_t* active_idx, int64_t n_act, double* a, d
     A.n_items = plan.n_units * plan.n_split;
     A.n_planes = plan.n_split * plan.sub;
     A.ld = plan.n_units * plan.unit;
-    A.eps2 = ctx->eps * ctx->eps;
-    A.partial = ctx->L.partial;
-    A.queue = ctx->L.queue;                                 // zeroed by nb_init, left at 0 by every launch
-    A.out_a = ctx->L.fa; A.out_j = ctx->L.fj; A.out_s = ctx->L.fs; A.out_p = ctx->L.fp;
 
     int launches = 0;
     CU(cudaEventRecord(ctx->ev0, ctx->stream), "event record");
@@ -313,6 +326,38 @@ int nb_next_block(nb_ctx* ctx, double* t_next, int32_t* active_idx, int64_t* n_a
                            ctx->on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream), "active list");
         if (!ctx->on_device) CU(cudaStreamSynchronize(ctx->stream), "nb_next_block");
     }
+    return NB_OK;
+}
+
+int nb_run_blocks(nb_ctx* ctx, double t_end, int64_t max_steps, int64_t* steps_done, double* t_last, int64_t* sum_n_act)
+{
+    if (!ctx || !(t_end == t_end) || max_steps < 0) return NB_EINVAL;
+    if (!ctx->step_graph) {
+        const int rc = build_step_graph(ctx);
+        if (rc != NB_OK) return rc;
+    }
+    DevPlan h{};
+    h.t_end = t_end; h.steps_left = max_steps; h.t_last = -1.0; h.max_split = ctx->max_split;
+    CU(cudaMemcpyAsync(ctx->L.devplan, &h, sizeof h, cudaMemcpyHostToDevice, ctx->stream), "upload step control");
+    CU(cudaMemsetAsync(ctx->L.scratch, 0xff, 8, ctx->stream), "reset t_next");
+    ctx->predicted = false; ctx->forced_n = -1; ctx->sched_n = -1;
+    // The host cannot know when the device stops, so it enqueues batches of steps and looks at the counters after each;
+    // steps enqueued after the stop flag is up return at once (every kernel checks it).
+    int64_t enqueued = 0;
+    int batch = 8;
+    while (max_steps > 0) {
+        const int64_t n = std::min<int64_t>(batch, max_steps - enqueued);
+        for (int64_t k = 0; k < n; ++k) CU(cudaGraphLaunch(ctx->step_graph, ctx->stream), "block-step graph launch");
+        enqueued += n;
+        ctx->launches += n * STEP_GRAPH_KERNELS;
+        CU(cudaMemcpyAsync(&h, ctx->L.devplan, sizeof h, cudaMemcpyDeviceToHost, ctx->stream), "read step control");
+        CU(cudaStreamSynchronize(ctx->stream), "nb_run_blocks");
+        if (h.stop || enqueued >= max_steps) break;
+        if (batch < 64) batch *= 2;
+    }
+    if (steps_done) *steps_done = h.steps_done;
+    if (t_last) *t_last = h.t_last;
+    if (sum_n_act) *sum_n_act = h.sum_act;
     return NB_OK;
 }
 
@@ -412,6 +457,31 @@ int nb_probe_fp64_peak(int device, void* stream, void* workspace, size_t workspa
     return NB_OK;
 }
 
+int nb_probe_dfma_sources(int device, void* stream, void* workspace, size_t workspace_bytes, int kind, double sm_mhz, double* cycles)
+{
+    if (!workspace || workspace_bytes < 65536 || !cycles || kind < 0 || kind > 2 || !(sm_mhz > 0)) return NB_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    int n_sm = 0;
+    if (cudaSetDevice(device) != cudaSuccess) return NB_ECUDA;
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return NB_ECUDA;
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return NB_ECUDA;
+    const int iters = 40000;
+    float ms = 0;
+    int rc = NB_OK;
+    for (int round = 0; round < 2 && rc == NB_OK; ++round) {       // the first launch warms up
+        cudaEventRecord(e0, st);
+        if (nb_launch_dfma_source_probe((double*)workspace, n_sm, kind, iters, st) != cudaSuccess) rc = NB_ECUDA;
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess || cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) rc = NB_ECUDA;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    if (rc != NB_OK) return rc;
+    // 3 x 8 warps per SM = 6 per sub-partition, 64 DFMAs per iteration each
+    *cycles = (double)ms * 1e-3 * sm_mhz * 1e6 / (6.0 * 64.0 * iters);
+    return NB_OK;
+}
+
 int64_t nb_launch_count(const nb_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 double nb_last_force_ms(nb_ctx* ctx)
@@ -442,6 +512,7 @@ void nb_free(nb_ctx* ctx)
     if (!ctx) return;
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    if (ctx->step_graph) cudaGraphExecDestroy(ctx->step_graph);
     delete ctx;
 }
 

@@ -16,6 +16,7 @@
 // long tail of under-occupied SMs.  Where an item's sums are stored depends only on the item, so the
 // results stay bitwise reproducible.
 #include "nb_internal.h"
+#include "nb_plan.h"
 
 namespace {
 
@@ -289,6 +290,18 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
     } while (!done);
 }
 
+// Device-planned launch (nb_run_blocks): take the plan the scheduler left in device memory.  False: this kernel shape
+// is not the one the plan names (or the step is not taken) and the whole grid returns.
+__device__ __forceinline__ bool take_devplan(ForceArgs& A, int kernel_id)
+{
+    if (!A.dp) return true;
+    const DevPlan* d = A.dp;
+    if (d->stop || d->kernel != kernel_id) return false;
+    A.n_act = d->n_act; A.n_units = d->n_units; A.n_split = d->n_split; A.slice_tiles = d->slice_tiles;
+    A.n_items = d->n_items; A.ld = d->ld; A.n_planes = d->n_planes;
+    return true;
+}
+
 // The CTA (or warp) that finds the queue empty last puts both counters back to 0 for the next launch.
 __device__ __forceinline__ void queue_retire(int* queue, int n_workers)
 {
@@ -306,8 +319,10 @@ static_assert(LI_TJ % 2 == 0, "pair2 takes two j-records at a time");
 // warps hold the SAME 32 particles and each takes its own quarter of every j-tile, so an item is (32 particles,
 // j-slice) and writes four partial planes (slice * 4 + warp) that the reduction adds like any other slices.
 template <bool EPS0, int W>
-__global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(const ForceArgs A)
+__global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(const ForceArgs A_)
 {
+    ForceArgs A = A_;
+    if (!take_devplan(A, W == 1 ? 0 : 2)) return;
     constexpr int UNIT = LI_UNIT / W;                      // active particles per work item
     constexpr int TJW = LI_TJ / W;                         // records of each j-tile one warp group takes
     static_assert(W == 1 || (LI_I == 1 && UNIT == 32 && TJW % 2 == 0), "W > 1: one warp per group");
@@ -417,8 +432,10 @@ __device__ __forceinline__ double warp_sum(double v)
 }
 
 template <bool EPS0>
-__global__ void __launch_bounds__(LJ_THREADS, LJ_CTAS_PER_SM) force_lj_kernel(const ForceArgs A)
+__global__ void __launch_bounds__(LJ_THREADS, LJ_CTAS_PER_SM) force_lj_kernel(const ForceArgs A_)
 {
+    ForceArgs A = A_;
+    if (!take_devplan(A, 1)) return;
     const int lane = threadIdx.x & 31;
     for (;;) {
         int wi = 0;
@@ -474,42 +491,48 @@ __global__ void __launch_bounds__(LJ_THREADS, LJ_CTAS_PER_SM) force_lj_kernel(co
 // tree in shared memory.  The order depends only on (S, T): bitwise reproducible.  T = 1 is the plain loop over
 // slices (large active sets, few slices: the loads of neighbouring threads coalesce over k).
 // ---------------------------------------------------------------------------------------------
-constexpr int RED_THREADS = 256;
-
-__global__ void __launch_bounds__(RED_THREADS) reduce_partials_kernel(const ForceArgs A, const int T)
+__global__ void __launch_bounds__(RED_THREADS) reduce_partials_kernel(const ForceArgs A_, int T)
 {
     __shared__ double sm[10][RED_THREADS];
-    const int R = RED_THREADS / T;                         // active particles per block
+    ForceArgs A = A_;
+    if (A.dp) {                                            // device-planned: any kernel shape, T from the plan
+        if (A.dp->stop) return;
+        A.n_act = A.dp->n_act; A.ld = A.dp->ld; A.n_planes = A.dp->n_planes; T = A.dp->red_T;
+        if (A.n_planes <= 1) return;                       // the force kernel wrote the results itself
+    }
+    const int R = RED_THREADS / T;                         // active particles per block and pass
     const int kl = threadIdx.x % R, lane = threadIdx.x / R;
-    const int k = blockIdx.x * R + kl;
-    double r[10];
+    for (int k0 = blockIdx.x * R; k0 < A.n_act; k0 += gridDim.x * R) {      // uniform over the block
+        const int k = k0 + kl;
+        double r[10];
 #pragma unroll
-    for (int c = 0; c < 10; ++c) r[c] = 0.0;
-    if (k < A.n_act) {
-        const size_t plane = (size_t)10 * A.ld;
-        const double* P = A.partial + (size_t)lane * plane + k;
-        for (int s = lane; s < A.n_planes; s += T, P += (size_t)T * plane) {
+        for (int c = 0; c < 10; ++c) r[c] = 0.0;
+        if (k < A.n_act) {
+            const size_t plane = (size_t)10 * A.ld;
+            const double* P = A.partial + (size_t)lane * plane + k;
+            for (int s = lane; s < A.n_planes; s += T, P += (size_t)T * plane) {
 #pragma unroll
-            for (int c = 0; c < 10; ++c) r[c] += P[(size_t)c * A.ld];
+                for (int c = 0; c < 10; ++c) r[c] += P[(size_t)c * A.ld];
+            }
         }
+        for (int off = T >> 1; off > 0; off >>= 1) {
+            if (lane >= off && lane < 2 * off) {
+#pragma unroll
+                for (int c = 0; c < 10; ++c) sm[c][threadIdx.x] = r[c];
+            }
+            __syncthreads();
+            if (lane < off) {
+#pragma unroll
+                for (int c = 0; c < 10; ++c) r[c] += sm[c][threadIdx.x + off * R];
+            }
+            __syncthreads();
+        }
+        if (lane != 0 || k >= A.n_act) continue;
+        A.out_a[3 * k] = r[0]; A.out_a[3 * k + 1] = r[1]; A.out_a[3 * k + 2] = r[2];
+        A.out_j[3 * k] = r[3]; A.out_j[3 * k + 1] = r[4]; A.out_j[3 * k + 2] = r[5];
+        A.out_s[3 * k] = r[6]; A.out_s[3 * k + 1] = r[7]; A.out_s[3 * k + 2] = r[8];
+        A.out_p[k] = -r[9];
     }
-    for (int off = T >> 1; off > 0; off >>= 1) {           // uniform over the block
-        if (lane >= off && lane < 2 * off) {
-#pragma unroll
-            for (int c = 0; c < 10; ++c) sm[c][threadIdx.x] = r[c];
-        }
-        __syncthreads();
-        if (lane < off) {
-#pragma unroll
-            for (int c = 0; c < 10; ++c) r[c] += sm[c][threadIdx.x + off * R];
-        }
-        __syncthreads();
-    }
-    if (lane != 0 || k >= A.n_act) return;
-    A.out_a[3 * k] = r[0]; A.out_a[3 * k + 1] = r[1]; A.out_a[3 * k + 2] = r[2];
-    A.out_j[3 * k] = r[3]; A.out_j[3 * k + 1] = r[4]; A.out_j[3 * k + 2] = r[5];
-    A.out_s[3 * k] = r[6]; A.out_s[3 * k + 1] = r[7]; A.out_s[3 * k + 2] = r[8];
-    A.out_p[k] = -r[9];
 }
 
 }  // namespace
@@ -530,15 +553,32 @@ cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (args.n_planes > 1) {
-        // threads per particle: enough to spread S slices, few enough that large active sets keep coalesced rows
-        int T = 1;
-        while (T < RED_THREADS && T * 4 <= args.n_planes && (int64_t)args.n_act * T < (int64_t)1 << 18) T <<= 1;
+        const int T = nb_reduce_threads(args.n_act, args.n_planes);
         const int R = RED_THREADS / T;
         reduce_partials_kernel<<<(args.n_act + R - 1) / R, RED_THREADS, 0, st>>>(args, T);
         ++*launches;
         e = cudaGetLastError();
     }
     return e;
+}
+
+cudaError_t nb_launch_force_devplan(const ForceArgs& args_, bool eps_is_zero, int n_sm, int Npad, cudaStream_t st, int* launches)
+{
+    ForceArgs args = args_, args_lj = args_;
+    args.n_tiles = Npad / LI_TJ; args_lj.n_tiles = Npad / LJ_TJ;
+    const int g_li = n_sm * LI_CTAS_PER_SM, g_lj = n_sm * LJ_CTAS_PER_SM;
+    if (eps_is_zero) {
+        force_lj_kernel<true><<<g_lj, LJ_THREADS, 0, st>>>(args_lj);
+        force_li_kernel<true, LI_W><<<g_li, LI_THREADS, 0, st>>>(args);
+        force_li_kernel<true, 1><<<g_li, LI_THREADS, 0, st>>>(args);
+    } else {
+        force_lj_kernel<false><<<g_lj, LJ_THREADS, 0, st>>>(args_lj);
+        force_li_kernel<false, LI_W><<<g_li, LI_THREADS, 0, st>>>(args);
+        force_li_kernel<false, 1><<<g_li, LI_THREADS, 0, st>>>(args);
+    }
+    reduce_partials_kernel<<<n_sm * 4, RED_THREADS, 0, st>>>(args, 1);
+    *launches += 4;
+    return cudaGetLastError();
 }
 
 void nb_force_occupancy(int* li, int* lj)

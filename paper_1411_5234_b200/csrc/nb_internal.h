@@ -49,7 +49,10 @@ constexpr int LJ_I = 1;
 constexpr int LJ_TJ = 32;                    // j-records per warp iteration
 constexpr int LJ_CTAS_PER_SM = 3;
 constexpr int64_t LJ_MAX_ACT = 16;           // n_act <= this -> lanes-over-j
+constexpr int RED_THREADS = 256;             // threads per block of the partial-sum reduction
 constexpr int64_t LIW_MAX_ACT = 96;          // n_act <= this -> lanes-over-i with 32-particle units (above, a 128-lane i-tile is >= 75 % full)
+
+struct DevPlan;   // nb_plan.h
 
 struct ForceArgs {
     const double4* pj0; const double4* pj1; const double2* pj2;   // predicted records (padded)
@@ -64,12 +67,15 @@ struct ForceArgs {
     int ld;                  // rows of the partial buffer per (slice, component) plane
     double eps2;
     double* partial;         // [S][10][ld] when S > 1
+    const DevPlan* dp;       // non-null: the launch was planned on the device (nb_run_blocks); overrides the plan fields above
     int* queue;              // work queue: [0] next item, [1] finished CTAs (both 0 between launches)
     double* out_a; double* out_j; double* out_s; double* out_p;   // [n_act][3] x3, [n_act]
 };
 
 // nb_force.cu
 cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps_is_zero, cudaStream_t st, int* launches);
+// device-planned: all three kernel shapes and the reduction at their largest grids; the ones the plan does not name return at once
+cudaError_t nb_launch_force_devplan(const ForceArgs& args, bool eps_is_zero, int n_sm, int Npad, cudaStream_t st, int* launches);
 void nb_force_occupancy(int* li_ctas_per_sm, int* lj_ctas_per_sm);
 
 // nb_step.cu
@@ -85,5 +91,12 @@ cudaError_t nb_launch_get(const StateArrays& s, int field, const int32_t* idx, i
 cudaError_t nb_launch_set(const StateArrays& s, int field, const int32_t* idx, int64_t n, const double* in, cudaStream_t st);
 // scheduler: scratch = >= 64 KiB; result: scratch_out[0] = t_next (double), ((int64*)scratch_out)[1] = n_act
 cudaError_t nb_launch_next_block(const StateArrays& s, int64_t N, int32_t* active, void* scratch, cudaStream_t st, int* launches);
+// the O(N) / O(n_act) kernels of one device-planned block step (nb_run_blocks): scheduler + plan, predictor; corrector
+cudaError_t nb_launch_devstep_head(const StateArrays& s, int64_t N, int64_t Npad, int n_sm, int32_t* active, void* scratch, DevPlan* dp,
+                                   cudaStream_t st, int* launches);
+cudaError_t nb_launch_devstep_tail(const StateArrays& s, int n_sm, const int32_t* active, void* scratch, DevPlan* dp, const double* fa,
+                                   const double* fj, const double* fs, double eta, int k_min, int k_max, cudaStream_t st, int* launches);
 cudaError_t nb_launch_energy(const StateArrays& s, int64_t N, const double* pot, double* scratch, cudaStream_t st, int* launches);
 cudaError_t nb_launch_fp64_probe(double* out, int n_sm, int iters, cudaStream_t st);
+// 3 CTAs x 256 threads per SM, 64 DFMAs per thread and iteration; kind: see nb_step.cu
+cudaError_t nb_launch_dfma_source_probe(double* out, int n_sm, int kind, int iters, cudaStream_t st);

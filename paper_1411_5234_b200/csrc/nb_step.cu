@@ -2,6 +2,7 @@
 // a4, a5, a6): predictor, corrector with the time-step criterion, block scheduler, state I/O,
 // energy.  All are HBM-bandwidth bound; see DESIGN.md for the bytes per particle of each.
 #include "nb_internal.h"
+#include "nb_plan.h"
 
 namespace {
 
@@ -37,8 +38,12 @@ __global__ void init_state_kernel(StateArrays s, int64_t N, int64_t Npad, const 
 
 // ------------------------------------------------------------------ a1: predictor (reading R6)
 // Reads 160 B, writes 80 B per particle.  own_time: D = 0 for every particle (records := stored state).
-__global__ void __launch_bounds__(TPB) predict_kernel(StateArrays s, int64_t N, double t, bool own_time)
+__global__ void __launch_bounds__(TPB) predict_kernel(StateArrays s, int64_t N, double t, bool own_time, const DevPlan* dp)
 {
+    if (dp) {                                              // device-planned block step: the time comes from the scheduler
+        if (dp->stop) return;
+        t = dp->t_next;
+    }
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const double4 p = s.st0[i], q = s.st1[i], r = s.st2[i], u = s.st3[i], w = s.st4[i];
@@ -99,12 +104,9 @@ __global__ void startup_kernel(StateArrays s, int64_t N, const double* fa, const
 
 // ------------------------------------------------------------------ a4 + a5: corrector (reading R10, R11, R12)
 // Per active particle: reads 160 B state + 8 B dt + 72 B new a, jerk, snap; writes 160 B + 8 B.
-__global__ void __launch_bounds__(TPB) corrector_kernel(StateArrays s, const int32_t* idx, int64_t n_act, double dt_shared,
-                                                        double t_new, const double* fa, const double* fj, const double* fs,
-                                                        double eta3, int k_min, int k_max)
+__device__ __forceinline__ void corrector_one(const StateArrays& s, const int32_t* idx, int64_t k, double dt_shared, double t_new,
+                                              const double* fa, const double* fj, const double* fs, double eta3, int k_min, int k_max)
 {
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= n_act) return;
     const int64_t i = idx ? (int64_t)idx[k] : k;
     const double4 p = s.st0[i], q = s.st1[i], r = s.st2[i], u = s.st3[i], w = s.st4[i];
     const double dt_old = s.dt[i];
@@ -156,6 +158,22 @@ __global__ void __launch_bounds__(TPB) corrector_kernel(StateArrays s, const int
         if (m == rint(m)) k_new = k_old + 1;                // grow only on the doubled grid
     }
     s.dt[i] = scalbn(1.0, k_new);
+}
+
+__global__ void __launch_bounds__(TPB) corrector_kernel(StateArrays s, const int32_t* idx, int64_t n_act, double dt_shared,
+                                                        double t_new, const double* fa, const double* fj, const double* fs,
+                                                        double eta3, int k_min, int k_max, DevPlan* dp, unsigned long long* tmin_bits)
+{
+    if (dp) {                                              // device-planned block step
+        if (dp->stop) return;
+        n_act = dp->n_act; t_new = dp->t_next;
+        if (blockIdx.x == 0 && threadIdx.x == 0) {         // last kernel of the step: book-keeping nobody else reads now
+            dp->steps_done += 1; dp->steps_left -= 1; dp->sum_act += n_act; dp->t_last = t_new;
+            *tmin_bits = ~0ull;                            // "+infinity" for the next step's atomicMin
+        }
+    }
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n_act; k += (int64_t)gridDim.x * blockDim.x)
+        corrector_one(s, idx, k, dt_shared, t_new, fa, fj, fs, eta3, k_min, k_max);
 }
 
 // ------------------------------------------------------------------ state I/O
@@ -223,8 +241,9 @@ __device__ __forceinline__ double block_min(double v)
     return v;   // valid in thread 0
 }
 
-__global__ void __launch_bounds__(1024) sched_min_kernel(StateArrays s, int64_t N, unsigned long long* tmin_bits)
+__global__ void __launch_bounds__(1024) sched_min_kernel(StateArrays s, int64_t N, unsigned long long* tmin_bits, const DevPlan* dp)
 {
+    if (dp && dp->stop) return;
     double v = INFINITY;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
         v = fmin(v, s.st1[i].w + s.dt[i]);
@@ -235,10 +254,12 @@ __global__ void __launch_bounds__(1024) sched_min_kernel(StateArrays s, int64_t 
 constexpr int SCHED_TPB = 1024;
 
 __global__ void __launch_bounds__(SCHED_TPB) sched_count_kernel(StateArrays s, int64_t N, const unsigned long long* tmin_bits,
-                                                               unsigned int* counts, unsigned int* done, long long* n_act_out)
+                                                               unsigned int* counts, unsigned int* done, long long* n_act_out,
+                                                               DevPlan* dp, int64_t Npad, int n_sm)
 {
     __shared__ unsigned int warp_cnt[32];
     __shared__ bool last;
+    if (dp && dp->stop) return;
     const double tn = __longlong_as_double((long long)*tmin_bits);
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool act = i < N && (s.st1[i].w + s.dt[i] == tn);
@@ -275,12 +296,45 @@ __global__ void __launch_bounds__(SCHED_TPB) sched_count_kernel(StateArrays s, i
         int b2 = threadIdx.x * per + q;
         if (b2 < nb) { unsigned int v = __ldcg(counts + b2); counts[b2] = run; run += v; }
     }
+    if (!dp) return;
+    // device-planned block step (nb_run_blocks): decide whether the step is taken, and plan the force launch for its
+    // n_act with the functions the host uses (nb_plan.h); the candidates S are spread over the block's threads.
+    __syncthreads();
+    __shared__ double best_c[SCHED_TPB];
+    __shared__ int best_s[SCHED_TPB];
+    const long long n_act = *n_act_out;
+    const bool stop = tn > dp->t_end || dp->steps_left <= 0 || n_act <= 0;
+    if (stop) {
+        if (threadIdx.x == 0) { dp->stop = 1; dp->n_act = 0; }
+        return;
+    }
+    const PlanShape sh = nb_plan_shape(Npad, n_act, n_sm, dp->max_split);
+    double c;
+    const int64_t S = nb_best_split(sh, 1 + threadIdx.x, SCHED_TPB, &c);
+    best_c[threadIdx.x] = c; best_s[threadIdx.x] = (int)S;       // S = 0: this thread had no candidate (c = 1e300)
+    __syncthreads();
+    for (int o = SCHED_TPB / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) {
+            const double c2 = best_c[threadIdx.x + o];
+            const int s2 = best_s[threadIdx.x + o];
+            const double c1 = best_c[threadIdx.x];
+            const int s1 = best_s[threadIdx.x];
+            // least cost; on ties the smaller S (as the host's ascending scan)
+            if (s2 != 0 && (s1 == 0 || c2 < c1 || (c2 == c1 && s2 < s1))) { best_c[threadIdx.x] = c2; best_s[threadIdx.x] = s2; }
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        nb_fill_devplan(dp, sh, best_s[0], n_act);
+        dp->t_next = tn;
+    }
 }
 
 __global__ void __launch_bounds__(SCHED_TPB) sched_scatter_kernel(StateArrays s, int64_t N, const unsigned long long* tmin_bits,
-                                                                 const unsigned int* offsets, int32_t* active)
+                                                                 const unsigned int* offsets, int32_t* active, const DevPlan* dp)
 {
     __shared__ unsigned int warp_off[32];
+    if (dp && dp->stop) return;
     const double tn = __longlong_as_double((long long)*tmin_bits);
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool act = i < N && (s.st1[i].w + s.dt[i] == tn);
@@ -347,7 +401,47 @@ __global__ void __launch_bounds__(256) fp64_probe_kernel(double* out, int iters)
     if (r == 12345.678) out[blockIdx.x] = r;     // never true; keeps the chains alive
 }
 
+// Operand-source probes: 8 independent chains, 64 DFMAs per loop iteration, in three flavours.
+//   0: acc = acc * m + c, m and c loop constants       -> two cycles per DFMA (the pipe's rate)
+//   1: acc_k = b_k * d_k + acc_k, three register pairs  -> three cycles
+//   2: acc_k = q * d_k + acc_k, q shared by the run     -> two cycles where the operand-reuse cache supplies q
+#define PROBE_FMA(d, a, b, c) asm volatile("fma.rn.f64 %0, %1, %2, %3;" : "=d"(d) : "d"(a), "d"(b), "d"(c))
+template <int KIND>
+__global__ void __launch_bounds__(256) dfma_source_probe_kernel(double* out, int iters, double seed)
+{
+    double a[8], b[8], d[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        a[k] = threadIdx.x + k; b[k] = seed * (k + 1) + threadIdx.x * 1e-9; d[k] = seed * 0.1 * (k + 2) + threadIdx.x * 1e-9;
+    }
+    const double q = seed + threadIdx.x * 1e-9;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                if (KIND == 0) PROBE_FMA(a[k], a[k], 0.999999, 1e-7);
+                if (KIND == 1) PROBE_FMA(a[k], b[k], d[k], a[k]);
+                if (KIND == 2) PROBE_FMA(a[k], q, d[k], a[k]);
+            }
+        }
+    }
+    double r = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) r += a[k];
+    if (r == 12345.678) out[blockIdx.x] = r;     // never true; keeps the chains alive
+}
+
 }  // namespace
+
+cudaError_t nb_launch_dfma_source_probe(double* out, int n_sm, int kind, int iters, cudaStream_t st)
+{
+    const double seed = 1e-3;
+    if (kind == 0) dfma_source_probe_kernel<0><<<n_sm * 3, 256, 0, st>>>(out, iters, seed);
+    else if (kind == 1) dfma_source_probe_kernel<1><<<n_sm * 3, 256, 0, st>>>(out, iters, seed);
+    else dfma_source_probe_kernel<2><<<n_sm * 3, 256, 0, st>>>(out, iters, seed);
+    return cudaGetLastError();
+}
 
 cudaError_t nb_launch_init_state(const StateArrays& s, int64_t N, int64_t Npad, const double* m, const double* x, const double* v, cudaStream_t st)
 {
@@ -357,7 +451,7 @@ cudaError_t nb_launch_init_state(const StateArrays& s, int64_t N, int64_t Npad, 
 
 cudaError_t nb_launch_predict(const StateArrays& s, int64_t N, double t, bool own_time, cudaStream_t st)
 {
-    predict_kernel<<<nblocks(N), TPB, 0, st>>>(s, N, t, own_time);
+    predict_kernel<<<nblocks(N), TPB, 0, st>>>(s, N, t, own_time, nullptr);
     return cudaGetLastError();
 }
 
@@ -372,7 +466,7 @@ cudaError_t nb_launch_corrector(const StateArrays& s, const int32_t* idx, int64_
                                 const double* fa, const double* fj, const double* fs, double eta, int k_min, int k_max,
                                 cudaStream_t st)
 {
-    corrector_kernel<<<nblocks(n_act), TPB, 0, st>>>(s, idx, n_act, dt_shared, t_new, fa, fj, fs, eta * eta * eta, k_min, k_max);
+    corrector_kernel<<<nblocks(n_act), TPB, 0, st>>>(s, idx, n_act, dt_shared, t_new, fa, fj, fs, eta * eta * eta, k_min, k_max, nullptr, nullptr);
     return cudaGetLastError();
 }
 
@@ -398,11 +492,37 @@ cudaError_t nb_launch_next_block(const StateArrays& s, int64_t N, int32_t* activ
     if (e != cudaSuccess) return e;
     // 0xffff... as an unsigned is larger than the bit pattern of +inf (0x7ff0...), so it is a valid "+infinity"
     const int nb_min = (int)((N + 4095) / 4096) < 1024 ? (int)((N + 4095) / 4096) : 1024;
-    sched_min_kernel<<<nb_min, 1024, 0, st>>>(s, N, tmin);
+    sched_min_kernel<<<nb_min, 1024, 0, st>>>(s, N, tmin, nullptr);
     const int nb = nblocks(N, SCHED_TPB);
-    sched_count_kernel<<<nb, SCHED_TPB, 0, st>>>(s, N, tmin, counts, done, n_act);
-    sched_scatter_kernel<<<nb, SCHED_TPB, 0, st>>>(s, N, tmin, counts, active);
+    sched_count_kernel<<<nb, SCHED_TPB, 0, st>>>(s, N, tmin, counts, done, n_act, nullptr, 0, 0);
+    sched_scatter_kernel<<<nb, SCHED_TPB, 0, st>>>(s, N, tmin, counts, active, nullptr);
     *launches += 3;
+    return cudaGetLastError();
+}
+
+cudaError_t nb_launch_devstep_head(const StateArrays& s, int64_t N, int64_t Npad, int n_sm, int32_t* active, void* scratch, DevPlan* dp,
+                                   cudaStream_t st, int* launches)
+{
+    unsigned long long* tmin = (unsigned long long*)scratch;         // all ones on entry (memset by the caller, then by the corrector)
+    long long* n_act = (long long*)scratch + 1;
+    unsigned int* done = (unsigned int*)((char*)scratch + 16);
+    unsigned int* counts = (unsigned int*)((char*)scratch + 64);
+    const int nb_min = (int)((N + 4095) / 4096) < 1024 ? (int)((N + 4095) / 4096) : 1024;
+    sched_min_kernel<<<nb_min, 1024, 0, st>>>(s, N, tmin, dp);
+    const int nb = nblocks(N, SCHED_TPB);
+    sched_count_kernel<<<nb, SCHED_TPB, 0, st>>>(s, N, tmin, counts, done, n_act, dp, Npad, n_sm);
+    sched_scatter_kernel<<<nb, SCHED_TPB, 0, st>>>(s, N, tmin, counts, active, dp);
+    predict_kernel<<<nblocks(N), TPB, 0, st>>>(s, N, 0.0, false, dp);
+    *launches += 4;
+    return cudaGetLastError();
+}
+
+cudaError_t nb_launch_devstep_tail(const StateArrays& s, int n_sm, const int32_t* active, void* scratch, DevPlan* dp, const double* fa,
+                                   const double* fj, const double* fs, double eta, int k_min, int k_max, cudaStream_t st, int* launches)
+{
+    corrector_kernel<<<n_sm * 8, TPB, 0, st>>>(s, active, 0, 0.0, 0.0, fa, fj, fs, eta * eta * eta, k_min, k_max, dp,
+                                               (unsigned long long*)scratch);
+    *launches += 1;
     return cudaGetLastError();
 }
 

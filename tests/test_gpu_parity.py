@@ -308,6 +308,37 @@ def test_config2_sampled_and_steps(B, oracle):
     g.nb_free()
 
 
+def test_run_blocks_is_bitwise_the_separate_calls(B):
+    """nb_run_blocks (scheduler, plan and step on the device, CUDA graph) against the same steps driven call by call:
+    identical schedules, bit-identical states; step budget and t_end respected; eps = 0 variant."""
+    for N, eps, masses in ((3000, 1e-4, "kroupa"), (300, 0.0, "equal")):
+        m, x, v = W.plummer(N, 77 + N, masses)
+        g1 = B.System(m, x, v, eps)
+        g2 = B.System(m, x, v, eps)
+        t_end = 2.0 ** -5
+        steps, acts = 0, 0
+        while True:
+            t, n, act = g1.nb_next_block()
+            if t > t_end:
+                break
+            g1.nb_predict(t); g1.nb_force(act, outputs=False); g1.nb_corrector(act, 0.0)
+            steps += 1; acts += n
+        # in three instalments: a step budget, then a time limit, then the rest
+        s_a, t_a, n_a = g2.nb_run_blocks(t_end, max_steps=5)
+        assert s_a == 5 and t_a > 0
+        s_b, t_b, n_b = g2.nb_run_blocks(t_end / 2)
+        assert t_b <= t_end / 2
+        s_c, t_c, n_c = g2.nb_run_blocks(t_end)
+        assert s_a + s_b + s_c == steps and n_a + n_b + n_c == acts and t_c == t_end
+        assert g2.nb_run_blocks(t_end) == (0, -1.0, 0)                    # nothing left below t_end
+        for f in ("X", "V", "A", "J", "S", "C", "T", "DT"):
+            assert np.array_equal(g1.nb_get_state(f), g2.nb_get_state(f)), f
+        # the separate calls still work on a context that has run the graph
+        t1, n1, a1 = g1.nb_next_block(); t2, n2, a2 = g2.nb_next_block()
+        assert t1 == t2 and np.array_equal(a1, a2)
+        g1.nb_free(); g2.nb_free()
+
+
 def test_config3_reduced_twin_block_steps(B, oracle):
     """Config 3's recipe at N = 2048 run end to end to t = 1/8 on both sides."""
     _, m, x, v = W.config_inputs(3, N=2048)
