@@ -259,13 +259,14 @@ def run_ours(args, cfg_dict):
     sm_max_mhz = float(peaks.get("sm_max_mhz") or (clocks or {}).get("sm_max_mhz") or 1965.0)
     peak_nominal = n_sm * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12       # TFLOP/s, all-FMA
     peak_measured, _ = B.nb_probe_fp64_peak(1.0, local)
+    pipe_probe = B.nb_probe_dfma_sources(sm_max_mhz, local)   # cycles per DFMA: 2 / 3 / 3-with-reuse register sources
     f_ms = float(np.mean(force_ms))
     achieved = FLOP_EXEC * inter_per_step / (f_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "force_li_kernel<false, 1> (+ reduce_partials_kernel)", "achieved": achieved,
                 "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
                 "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max_mhz:.0f} MHz (DESIGN.md)",
                 "peak_measured_dfma": peak_measured, "frac_of_measured_dfma": achieved / peak_measured,
-                "flop_per_interaction": FLOP_EXEC, "tflops_conv97": FLOP_CONV * inter_per_step / (f_ms * 1e-3) / 1e12,
+                "flop_per_interaction": FLOP_EXEC, "pipe_probe": pipe_probe, "tflops_conv97": FLOP_CONV * inter_per_step / (f_ms * 1e-3) / 1e12,
                 "kernel_ms": f_ms, "kernel_share_of_step": f_ms * args.steps / ms,
                 "interactions_per_s_kernel": inter_per_step / (f_ms * 1e-3),
                 "traffic": TRAFFIC_NCU_BYTES if N == W.CONFIGS[4].N else None,

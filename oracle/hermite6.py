@@ -118,6 +118,21 @@ class OracleSystem:
         self.pot0 = p2
         self.L.oracle_startup_levels(N, _p(self.a), _p(self.j), eta_s, k_min, k_max, _p(self.dt))
 
+    @classmethod
+    def from_state(cls, m, x, v, a, j, s, c, t, dt, eps, eta=0.45, eta_s=0.01, k_min=-20, k_max=-3, kind="ld"):
+        """A system that continues from a given state (no startup evaluation): for checks at sizes where the two
+        O(N^2) startup passes are out of reach."""
+        o = cls.__new__(cls)
+        o.L, o.kind = lib(kind), kind
+        o.N = N = int(m.shape[0])
+        o.eps, o.eta, o.eta_s, o.k_min, o.k_max = float(eps), eta, eta_s, k_min, k_max
+        o.m = _f64(m, (N,)).copy()
+        o.x, o.v, o.a, o.j, o.s, o.c = (_f64(q, (N, 3)).copy() for q in (x, v, a, j, s, c))
+        o.t, o.dt = _f64(t, (N,)).copy(), _f64(dt, (N,)).copy()
+        o.xp, o.vp, o.ap = np.zeros((N, 3)), np.zeros((N, 3)), np.zeros((N, 3))
+        o.t_pred, o.f = 0.0, None
+        return o
+
     def predict(self, t):
         self.L.oracle_predict(self.N, float(t), _p(self.t), _p(self.x), _p(self.v), _p(self.a),
                               _p(self.j), _p(self.s), _p(self.c), _p(self.xp), _p(self.vp), _p(self.ap))

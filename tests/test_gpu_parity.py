@@ -308,6 +308,49 @@ def test_config2_sampled_and_steps(B, oracle):
     g.nb_free()
 
 
+def test_config3_full_size_sampled_block_steps(B, oracle):
+    """Config 3 at its full size (N = 262144, Kroupa masses, block steps): advance on the GPU, then check sampled
+    block steps piece by piece against the oracle started from the GPU's state - scheduler bit-exact, predictor on all
+    N, the pairwise evaluation on up to 48 of the active particles (all N j-particles), corrector + time-step levels on
+    all active particles from identical inputs."""
+    import torch
+    c, m, x, v = W.config_inputs(3)
+    N = m.shape[0]
+    dev = "cuda:0"
+    g = B.System(torch.tensor(m, device=dev), torch.tensor(x, device=dev), torch.tensor(v, device=dev), c.eps, host=False)
+    K0, W0 = g.nb_energy()
+    steps, t_last, _ = g.nb_run_blocks(2.0 ** -8)
+    assert steps > 50 and t_last == 2.0 ** -8
+    get = lambda f: g.nb_get_state(f).cpu().numpy()
+    o = oracle.OracleSystem.from_state(m, *(get(f) for f in ("X", "V", "A", "J", "S", "C", "T", "DT")), c.eps)
+    rng = np.random.default_rng(3)
+    kernels = set()
+    for step in range(40):
+        tg, ng, actg = g.nb_next_block()
+        to, acto = o.next_block()
+        actg = actg.cpu().numpy()
+        assert tg == to and np.array_equal(actg, acto)                           # bit-exact schedule
+        kernels.add(B.nb_plan_force(N, ng, 148).kernel)
+        g.nb_predict(tg); o.predict(to)
+        for f, ref in (("XP", o.xp), ("VP", o.vp), ("AP", o.ap)):
+            assert relvec(get(f), ref).max() <= 1e-12, f
+        got = tuple(q.cpu().numpy() for q in g.nb_force(torch.tensor(actg, device=dev)))
+        rows = np.arange(ng) if ng <= 48 else np.sort(rng.choice(ng, 48, replace=False))
+        ref = oracle.hermite6.force(m, o.xp, o.vp, o.ap, c.eps, acto[rows])
+        assert_force_parity(tuple(q[rows] for q in got), ref)
+        # corrector and time-step criterion on identical inputs: the oracle takes the GPU's a, jerk, snap
+        o.f = got
+        g.nb_corrector(torch.tensor(actg, device=dev), 0.0); o.corrector(acto, 0.0)
+        for f, ref, tol in (("X", o.x, 1e-14), ("V", o.v, 1e-13), ("A", o.a, 0), ("J", o.j, 0), ("S", o.s, 0)):
+            assert relvec(get(f)[acto], ref[acto]).max() <= tol, f
+        assert np.array_equal(get("T"), o.t)
+        assert np.array_equal(get("DT"), o.dt), "time-step levels"
+        # resynchronise the oracle's x, v, crackle with the GPU's (round-off level) so that the next schedule stays comparable
+        o.x[acto], o.v[acto], o.c[acto] = get("X")[acto], get("V")[acto], get("C")[acto]
+    assert 1 in kernels                                                          # the tiny-active-set shape was exercised
+    g.nb_free()
+
+
 def test_run_blocks_is_bitwise_the_separate_calls(B):
     """nb_run_blocks (scheduler, plan and step on the device, CUDA graph) against the same steps driven call by call:
     identical schedules, bit-identical states; step budget and t_end respected; eps = 0 variant."""
