@@ -57,6 +57,13 @@ def lib(kind: str = "ld") -> C.CDLL:
     L.oracle_aarseth6_dt.restype = C.c_double
     L.oracle_hermite_derivs.argtypes = [C.c_double] + [_d] * 7
     L.oracle_hermite_derivs.restype = None
+    L.oracle_predict4.argtypes = [C.c_int64, C.c_double, _d] + [_d] * 4 + [_d] * 2
+    L.oracle_predict4.restype = None
+    L.oracle_correct4.argtypes = [C.c_int64, _i32, C.c_int64, C.c_double, C.c_double, _d, _d,
+                                  _d, _d, _d, _d, _d, _d, _d, _d, C.c_double, C.c_int, C.c_int]
+    L.oracle_correct4.restype = None
+    L.oracle_aarseth4_dt.argtypes = [_d, C.c_double]
+    L.oracle_aarseth4_dt.restype = C.c_double
     L.oracle_next_block.argtypes = [C.c_int64, _d, _d, _d, _i32]
     L.oracle_next_block.restype = C.c_int64
     L.oracle_energy.argtypes = [C.c_int64, _d, _d, _d, _d, _d]
@@ -97,9 +104,12 @@ def force(m, xp, vp, ap, eps, idx=None, kind="ld", want=("a", "j", "s", "p")):
 class OracleSystem:
     """Mirror of the C ABI (include/nb.h) on the CPU: init / predict / force / corrector / next_block."""
 
-    def __init__(self, m, x, v, eps, eta=0.45, eta_s=0.01, k_min=-20, k_max=-3, kind="ld"):
+    def __init__(self, m, x, v, eps, eta=None, eta_s=0.01, k_min=-20, k_max=-3, kind="ld", order=6):
+        assert order in (4, 6)
+        eta = {4: 0.14, 6: 0.45}[order] if eta is None else eta
         self.L = lib(kind)
         self.kind = kind
+        self.order = order
         self.N = N = int(m.shape[0])
         self.eps, self.eta, self.eta_s, self.k_min, self.k_max = float(eps), eta, eta_s, k_min, k_max
         self.m = _f64(m, (N,)).copy()
@@ -112,18 +122,22 @@ class OracleSystem:
         self.f = None
         # Startup (R8): pass 1 with a := 0 gives a, jerk; pass 2 with that a gives snap; a''' := 0.
         zero = np.zeros((N, 3))
-        a1, j1, _, _ = force(self.m, self.x, self.v, zero, self.eps, kind=kind)
-        a2, j2, s2, p2 = force(self.m, self.x, self.v, a1, self.eps, kind=kind)
-        self.a[:], self.j[:], self.s[:] = a2, j2, s2
-        self.pot0 = p2
+        a1, j1, _, p1 = force(self.m, self.x, self.v, zero, self.eps, kind=kind)
+        if order == 4:                                      # a and jerk need no second pass; snap, crackle := 0
+            self.a[:], self.j[:] = a1, j1
+            self.pot0 = p1
+        else:
+            a2, j2, s2, p2 = force(self.m, self.x, self.v, a1, self.eps, kind=kind)
+            self.a[:], self.j[:], self.s[:] = a2, j2, s2
+            self.pot0 = p2
         self.L.oracle_startup_levels(N, _p(self.a), _p(self.j), eta_s, k_min, k_max, _p(self.dt))
 
     @classmethod
-    def from_state(cls, m, x, v, a, j, s, c, t, dt, eps, eta=0.45, eta_s=0.01, k_min=-20, k_max=-3, kind="ld"):
+    def from_state(cls, m, x, v, a, j, s, c, t, dt, eps, eta=0.45, eta_s=0.01, k_min=-20, k_max=-3, kind="ld", order=6):
         """A system that continues from a given state (no startup evaluation): for checks at sizes where the two
         O(N^2) startup passes are out of reach."""
         o = cls.__new__(cls)
-        o.L, o.kind = lib(kind), kind
+        o.L, o.kind, o.order = lib(kind), kind, order
         o.N = N = int(m.shape[0])
         o.eps, o.eta, o.eta_s, o.k_min, o.k_max = float(eps), eta, eta_s, k_min, k_max
         o.m = _f64(m, (N,)).copy()
@@ -134,12 +148,19 @@ class OracleSystem:
         return o
 
     def predict(self, t):
+        if self.order == 4:
+            self.L.oracle_predict4(self.N, float(t), _p(self.t), _p(self.x), _p(self.v), _p(self.a), _p(self.j),
+                                   _p(self.xp), _p(self.vp))
+            self.ap[:] = 0.0                                # not used by a and jerk
+            self.t_pred = float(t)
+            return
         self.L.oracle_predict(self.N, float(t), _p(self.t), _p(self.x), _p(self.v), _p(self.a),
                               _p(self.j), _p(self.s), _p(self.c), _p(self.xp), _p(self.vp), _p(self.ap))
         self.t_pred = float(t)
 
     def force(self, idx=None):
-        self.f = force(self.m, self.xp, self.vp, self.ap, self.eps, idx, kind=self.kind)
+        want = ("a", "j", "p") if self.order == 4 else ("a", "j", "s", "p")
+        self.f = force(self.m, self.xp, self.vp, self.ap, self.eps, idx, kind=self.kind, want=want)
         return self.f
 
     def corrector(self, idx=None, dt=0.0):
@@ -148,6 +169,11 @@ class OracleSystem:
         n = self.N if idx is None else idx.shape[0]
         a1, j1, s1, _ = self.f
         assert a1.shape[0] == n
+        if self.order == 4:
+            self.L.oracle_correct4(self.N, _pi(idx), n, float(dt), self.t_pred, _p(a1), _p(j1),
+                                   _p(self.x), _p(self.v), _p(self.a), _p(self.j), _p(self.s), _p(self.c),
+                                   _p(self.t), _p(self.dt), self.eta, self.k_min, self.k_max)
+            return
         self.L.oracle_correct(self.N, _pi(idx), n, float(dt), self.t_pred, _p(a1), _p(j1), _p(s1),
                               _p(self.x), _p(self.v), _p(self.a), _p(self.j), _p(self.s), _p(self.c),
                               _p(self.t), _p(self.dt), self.eta, self.k_min, self.k_max)

@@ -255,6 +255,85 @@ void oracle_hermite_derivs(double h, const double* a0, const double* j0, const d
 }
 
 /*
+ * ---- 4th-order variant ("Hermite time integrators (4th, 6th and 8th order)"; formulas: DESIGN.md R21) ----
+ * The pairwise evaluation is O1 restricted to a and jerk (neither depends on the predicted accelerations).
+ *
+ * O2/4 - predictor:  x_p = x + D v + D^2/2 a + D^3/6 j,   v_p = v + D a + D^2/2 j.
+ */
+void oracle_predict4(int64_t N, double t, const double* ti, const double* x, const double* v,
+                     const double* a, const double* j, double* xp, double* vp)
+{
+    for (int64_t i = 0; i < N; ++i) {
+        const real D = (real)t - (real)ti[i];
+        const real D2 = D * D, D3 = D2 * D;
+        for (int k = 0; k < 3; ++k) {
+            const int64_t e = 3 * i + k;
+            xp[e] = (double)((real)x[e] + D * v[e] + D2 / 2 * a[e] + D3 / 6 * j[e]);
+            vp[e] = (double)((real)v[e] + D * a[e] + D2 / 2 * j[e]);
+        }
+    }
+}
+
+/* O4/4 - generalised Aarseth criterion for a 4th-order scheme: dt_crit = eta A1/A2,
+ * Ak = sqrt(|a^(k-1)| |a^(k+1)| + |a^(k)|^2); d[0..3] = a, a', a'', a''' at the new time. */
+static real aarseth4_dt(real d[4][3], double eta)
+{
+    const real n0 = norm3(d[0]), n1 = norm3(d[1]), n2 = norm3(d[2]), n3 = norm3(d[3]);
+    return (real)eta * R_SQRT(n0 * n2 + n1 * n1) / R_SQRT(n1 * n3 + n2 * n2);
+}
+
+double oracle_aarseth4_dt(const double* d12, double eta)
+{
+    real d[4][3];
+    for (int r = 0; r < 4; ++r) for (int q = 0; q < 3; ++q) d[r][q] = d12[3 * r + q];
+    return (double)aarseth4_dt(d, eta);
+}
+
+/*
+ * O3/4 - corrector: the two-point cubic Hermite quadrature
+ *   v1 = v0 + h/2 (a1 + a0) - h^2/12 (j1 - j0),   x1 = x0 + h/2 (v1 + v0) - h^2/12 (a1 - a0)
+ * and the cubic Hermite interpolant of a(t) through (a0, j0) and (a1, j1):
+ *   d3a/dt3     = (12 (a0 - a1) + 6 h (j0 + j1)) / h^3        (constant over the step)
+ *   d2a/dt2(t1) = (6 (a0 - a1) + h (2 j0 + 4 j1)) / h^2
+ * Stored afterwards: x1, v1, a1, j1, s := d2a/dt2(t1), c := d3a/dt3, t_i := t_new; dt_i as in O3.
+ */
+void oracle_correct4(int64_t N, const int32_t* idx, int64_t n_act, double dt_shared, double t_new,
+                     const double* a1, const double* j1,
+                     double* x, double* v, double* a, double* j, double* s, double* c,
+                     double* ti, double* dt, double eta, int k_min, int k_max)
+{
+    (void)N;
+    for (int64_t k = 0; k < n_act; ++k) {
+        const int64_t i = idx ? (int64_t)idx[k] : k;
+        const real h = dt_shared > 0 ? (real)dt_shared : (real)dt[i];
+        real d[4][3];
+        for (int q = 0; q < 3; ++q) {
+            const int64_t e = 3 * i + q, f = 3 * k + q;
+            const real A0 = a[e], J0 = j[e], A1 = a1[f], J1 = j1[f];
+            const real v0 = v[e], x0 = x[e];
+            const real v1 = v0 + h / 2 * (A1 + A0) - h * h / 12 * (J1 - J0);
+            const real x1 = x0 + h / 2 * (v1 + v0) - h * h / 12 * (A1 - A0);
+            d[0][q] = A1; d[1][q] = J1;
+            d[2][q] = (6 * (A0 - A1) + h * (2 * J0 + 4 * J1)) / (h * h);
+            d[3][q] = (12 * (A0 - A1) + 6 * h * (J0 + J1)) / (h * h * h);
+            x[e] = (double)x1; v[e] = (double)v1;
+            a[e] = (double)A1; j[e] = (double)J1; s[e] = (double)d[2][q]; c[e] = (double)d[3][q];
+        }
+        ti[i] = t_new;
+        if (dt_shared > 0) {
+            dt[i] = dt_shared;
+        } else {
+            int k_old = (int)lrint(log2(dt[i]));
+            int k_crit = level_clamp(aarseth4_dt(d, eta), k_min, k_max);
+            int k_new = k_old;
+            if (k_crit < k_old) k_new = k_crit;
+            else if (k_crit > k_old && k_old < k_max && fmod(t_new, ldexp(1.0, k_old + 1)) == 0.0) k_new = k_old + 1;
+            dt[i] = ldexp(1.0, k_new);
+        }
+    }
+}
+
+/*
  * O6 — block scheduler ("blocks that share the same time step"):
  * t_next = min_i (t_i + dt_i); active = { i : t_i + dt_i == t_next } in index order.
  * All times are dyadic rationals, so the fp64 sums and the equality are exact.

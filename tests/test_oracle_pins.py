@@ -323,3 +323,82 @@ def test_f64_variant_agrees_with_long_double(oracle):
     for r, f in zip(ref[:3], f64[:3]):
         assert (np.linalg.norm(r - f, axis=1) / np.linalg.norm(r, axis=1)).max() < 1e-12
     assert np.abs(ref[3] / f64[3] - 1).max() < 1e-13
+
+
+# ---------------------------------------------------------------- 4th-order variant (R21)
+def test_o4_predictor_and_corrector_polynomial_exactness(oracle):
+    """Predictor exact for cubic x(t); corrector exact in v and in the recovered a'', a''' for cubic a(t), exact in x for
+    quadratic a(t) (two-point cubic Hermite quadrature)."""
+    rng = np.random.default_rng(14)
+    L = oracle.lib("ld")
+    P = oracle.hermite6._p
+    N = 5
+    coef = rng.normal(size=(4, N, 3))                       # x, v, a, j at t_i
+    ti = rng.choice([0.0, 0.25, 0.5], N)
+    t = 0.75
+    xp, vp = np.zeros((N, 3)), np.zeros((N, 3))
+    L.oracle_predict4(N, t, P(ti), *[P(np.ascontiguousarray(c)) for c in coef], P(xp), P(vp))
+    D = (t - ti)[:, None]
+    np.testing.assert_allclose(xp, coef[0] + D * coef[1] + D ** 2 / 2 * coef[2] + D ** 3 / 6 * coef[3], rtol=0, atol=2e-15)
+    np.testing.assert_allclose(vp, coef[1] + D * coef[2] + D ** 2 / 2 * coef[3], rtol=0, atol=2e-15)
+    for deg in (2, 3):
+        h, t0 = 0.25, 0.5
+        pa = [np.polynomial.Polynomial(rng.normal(size=deg + 1)) for _ in range(3)]
+        pv = [p.integ() + rng.normal() for p in pa]
+        px = [p.integ() + rng.normal() for p in pv]
+        ev = lambda polys, k, tt: np.array([[p.deriv(k)(tt) if k else p(tt) for p in polys]])
+        x, v, a, j = ev(px, 0, t0), ev(pv, 0, t0), ev(pa, 0, t0), ev(pa, 1, t0)
+        s, c = np.zeros((1, 3)), np.zeros((1, 3))
+        t1 = t0 + h
+        a1, j1 = ev(pa, 0, t1), ev(pa, 1, t1)
+        tt, dt = np.array([t0]), np.array([h])
+        L.oracle_correct4(1, None, 1, h, t1, P(a1), P(j1), P(x), P(v), P(a), P(j), P(s), P(c), P(tt), P(dt), 0.14, -20, -3)
+        np.testing.assert_allclose(v, ev(pv, 0, t1), rtol=0, atol=1e-14)
+        if deg == 2:
+            np.testing.assert_allclose(x, ev(px, 0, t1), rtol=0, atol=1e-14)
+        np.testing.assert_allclose(s, ev(pa, 2, t1), rtol=0, atol=1e-12)
+        np.testing.assert_allclose(c, ev(pa, 3, t1), rtol=0, atol=1e-11)
+        assert tt[0] == t1 and dt[0] == h and np.array_equal(a, a1) and np.array_equal(j, j1)
+
+
+def test_o4_kepler_orbit_fourth_order_convergence(oracle):
+    """The e = 0.5 orbit of P5 with the 4th-order scheme: halving dt divides the error by ~2^4, not 2^6."""
+    e = 0.5
+    m = np.array([0.5, 0.5])
+    x = np.array([[0.75, 0, 0], [-0.75, 0, 0]])
+    vy = 0.5 * np.sqrt((1 - e) / (1 + e))
+    v = np.array([[0, vy, 0], [0, -vy, 0]])
+    dx, dE = [], []
+    for n in (512, 1024, 2048):
+        o = oracle.OracleSystem(m, x, v, 0.0, order=4)
+        E0 = sum(o.energy())
+        for _ in range(n):
+            o.shared_step(2 * np.pi / n)
+        dx.append(np.abs(o.x - x).max()); dE.append(abs(sum(o.energy()) / E0 - 1))
+    assert dx[0] < 1e-4 and dx[2] < 1e-6
+    assert 12 < dx[0] / dx[1] < 20 and 12 < dx[1] / dx[2] < 20
+    assert 12 < dE[0] / dE[1] < 40 and 12 < dE[1] / dE[2] < 40
+
+
+def test_o4_criterion_closed_form_and_block_steps(oracle):
+    L = oracle.lib("ld")
+    P = oracle.hermite6._p
+    # |a^(k)| = w^k |a|  =>  A1 = sqrt2 w |a|, A2 = sqrt2 w^2 |a|  =>  dt_crit = eta / w
+    for w_ in (0.7, 3.0, 41.0):
+        d = np.zeros((4, 3))
+        for k in range(4):
+            d[k, k % 3] = 2.5 * w_ ** k
+        assert abs(L.oracle_aarseth4_dt(P(d), 0.14) * w_ / 0.14 - 1) < 1e-15
+    # block steps on a small Plummer sphere stay on the dyadic grid and conserve energy
+    m, x, v = W.plummer(96, 11)
+    o = oracle.OracleSystem(m, x, v, 1e-2, order=4)
+    E0 = sum(o.energy())
+    n = 0
+    while True:
+        tn, act = o.next_block()
+        if tn > 0.125:
+            break
+        o.predict(tn); o.force(act); o.corrector(act, 0.0)
+        n += 1
+    assert np.all(o.t == 0.125) and n > 10
+    assert abs(sum(o.energy()) / E0 - 1) < 1e-5
