@@ -51,9 +51,13 @@ typedef struct {
     void* workspace;        /* DEVICE memory, 256-B aligned, >= nb_workspace_bytes(N) bytes, owned by the caller */
     size_t workspace_bytes;
     int ptrs_on_device;     /* 0: (h/d) pointers are host pointers; 1: device pointers */
-    double eta;             /* accuracy parameter of the time-step criterion (reading R11); 0 -> 0.45 */
+    double eta;             /* accuracy parameter of the time-step criterion (reading R11); 0 -> 0.45 (order 6), 0.14 (order 4) */
     double eta_s;           /* same, for the startup step dt = eta_s |a|/|jerk|;             0 -> 0.01 */
     int k_min, k_max;       /* allowed levels: dt = 2^k, k_min <= k <= k_max; both 0 -> -20, -3 */
+    int order;              /* Hermite order ("4th, 6th and 8th order"): 0 or 6 = the 6th-order scheme of the
+                               north star; 4 = the 4th-order variant (reading R21): nb_force evaluates a, jerk and pot (snap
+                               is returned as 0), the predictor stops at the jerk term, nb_corrector is the cubic Hermite
+                               quadrature and the criterion dt = eta A1/A2.  8 is not built (NB_EINVAL). */
 } nb_config;
 
 /* Selectors of nb_get_state / nb_set_state.  Width = doubles per particle. */

@@ -28,7 +28,7 @@ EXPORTS = ["nb_workspace_bytes", "nb_plan_force", "nb_set_max_split", "nb_init",
 class nb_config(C.Structure):
     _fields_ = [("device", C.c_int), ("stream", C.c_void_p), ("workspace", C.c_void_p),
                 ("workspace_bytes", C.c_size_t), ("ptrs_on_device", C.c_int),
-                ("eta", C.c_double), ("eta_s", C.c_double), ("k_min", C.c_int), ("k_max", C.c_int)]
+                ("eta", C.c_double), ("eta_s", C.c_double), ("k_min", C.c_int), ("k_max", C.c_int), ("order", C.c_int)]
 
 
 class nb_plan(C.Structure):
@@ -113,7 +113,7 @@ class System:
     host=False: array arguments are torch CUDA tensors (DEVICE pointers; calls are asynchronous).
     """
 
-    def __init__(self, m, x, v, eps, host=True, device=0, eta=0.0, eta_s=0.0, k_min=0, k_max=0, stream=None):
+    def __init__(self, m, x, v, eps, host=True, device=0, eta=0.0, eta_s=0.0, k_min=0, k_max=0, stream=None, order=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1411_5234_b200 needs a CUDA device; there is no CPU fallback")
@@ -129,7 +129,7 @@ class System:
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=f"cuda:{device}")
         base = (self.workspace.data_ptr() + 255) // 256 * 256
         self.cfg = nb_config(device, C.c_void_p(self.stream.cuda_stream), C.c_void_p(base), nbytes,
-                             0 if host else 1, eta, eta_s, k_min, k_max)
+                             0 if host else 1, eta, eta_s, k_min, k_max, order)
         m, x, v = self._in(m, (self.N,)), self._in(x, (self.N, 3)), self._in(v, (self.N, 3))
         self._check(self.L.nb_init(C.byref(self.ctx), self.N, _ptr(m), _ptr(x), _ptr(v), float(eps), C.byref(self.cfg)))
 

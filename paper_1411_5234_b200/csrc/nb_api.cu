@@ -62,6 +62,7 @@ struct nb_ctx {
     int64_t N = 0, Npad = 0;
     double eps = 0, eta = 0.45, eta_s = 0.01;
     int k_min = -20, k_max = -3;
+    int order = 6;
     int n_sm = 148;
     int64_t max_split = 0;         // cap on the j-split (0: the cost model decides)
     Layout L{nullptr, 0};
@@ -114,7 +115,7 @@ int build_step_graph(nb_ctx* ctx)
         A.n_tiles = 0;                                      // set per kernel below
         A.dp = ctx->L.devplan;
         e = nb_launch_devstep_head(ctx->L.s, ctx->N, ctx->Npad, ctx->n_sm, ctx->L.idx_sched, ctx->L.scratch, ctx->L.devplan, cs, &launches);
-        if (e == cudaSuccess) e = nb_launch_force_devplan(A, ctx->eps == 0.0, ctx->n_sm, (int)ctx->Npad, cs, &launches);
+        if (e == cudaSuccess) e = nb_launch_force_devplan(A, ctx->eps == 0.0, ctx->order, ctx->n_sm, (int)ctx->Npad, cs, &launches);
         if (e == cudaSuccess)
             e = nb_launch_devstep_tail(ctx->L.s, ctx->n_sm, ctx->L.idx_sched, ctx->L.scratch, ctx->L.devplan, ctx->L.fa, ctx->L.fj, ctx->L.fs,
                                        ctx->eta, ctx->k_min, ctx->k_max, cs, &launches);
@@ -195,6 +196,7 @@ int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const dou
     const int k_min = (cfg->k_min == 0 && cfg->k_max == 0) ? -20 : cfg->k_min;
     const int k_max = (cfg->k_min == 0 && cfg->k_max == 0) ? -3 : cfg->k_max;
     if (k_min > k_max || k_min < -1000 || k_max > 1000 || cfg->eta < 0 || cfg->eta_s < 0) return NB_EINVAL;
+    if (cfg->order != 0 && cfg->order != 4 && cfg->order != 6) return NB_EINVAL;
     const int64_t Npad = pad_n(N);
     if (!cfg->workspace || ((uintptr_t)cfg->workspace % ALIGN) != 0 || cfg->workspace_bytes < Layout(nullptr, Npad).bytes)
         return NB_ENOMEM;
@@ -206,10 +208,12 @@ int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const dou
     ctx->stream = (cudaStream_t)cfg->stream;
     ctx->on_device = cfg->ptrs_on_device != 0;
     ctx->N = N; ctx->Npad = Npad; ctx->eps = eps;
-    ctx->eta = cfg->eta > 0 ? cfg->eta : 0.45;
+    ctx->order = cfg->order == 0 ? 6 : cfg->order;
+    ctx->eta = cfg->eta > 0 ? cfg->eta : (ctx->order == 4 ? 0.14 : 0.45);
     ctx->eta_s = cfg->eta_s > 0 ? cfg->eta_s : 0.01;
     ctx->k_min = k_min; ctx->k_max = k_max;
     ctx->L = Layout(cfg->workspace, Npad);
+    ctx->L.s.order = ctx->order;
 
     CU(cudaSetDevice(ctx->device), "cudaSetDevice");
     CU(cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, ctx->device), "device attribute");
@@ -230,7 +234,7 @@ int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const dou
     ctx->launches += 1;
 
     // startup (reading R8): two all-active evaluations at t = 0
-    for (int pass = 1; pass <= 2; ++pass) {
+    for (int pass = 1; pass <= (ctx->order == 4 ? 1 : 2); ++pass) {
         CU(nb_launch_predict(ctx->L.s, N, 0.0, true, ctx->stream), "predict");
         ctx->launches += 1;
         ctx->predicted = true; ctx->t_pred = 0.0;
@@ -279,7 +283,7 @@ int nb_force(nb_ctx* ctx, const int32_t* active_idx, int64_t n_act, double* a, d
 
     int launches = 0;
     CU(cudaEventRecord(ctx->ev0, ctx->stream), "event record");
-    CU(nb_launch_force(plan, A, ctx->eps == 0.0, ctx->stream, &launches), "force kernel");
+    CU(nb_launch_force(plan, A, ctx->eps == 0.0, ctx->order, ctx->stream, &launches), "force kernel");
     CU(cudaEventRecord(ctx->ev1, ctx->stream), "event record");
     ctx->ev_valid = true;
     ctx->launches += launches;

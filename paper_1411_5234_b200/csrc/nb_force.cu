@@ -238,6 +238,100 @@ __device__ __forceinline__ void pair2(const IPart& pi, const JRec (&J)[2], const
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// 4th-order variant (R21): acceleration, jerk and potential only.  32 FP64-pipe instructions per
+// pair (17 DFMA + 8 DMUL + 7 DADD) + 1 MUFU.RSQ64H; the snap sums stay 0.
+// ---------------------------------------------------------------------------------------------
+template <bool EPS0, bool MASK = true>
+__device__ __forceinline__ void pair_o4(const IPart& pi, const double4 p0, const double4 p1, const double eps2, const bool self, Sums& S)
+{
+    const double dx = p0.x - pi.x, dy = p0.y - pi.y, dz = p0.z - pi.z;
+    const double dvx = p1.x - pi.vx, dvy = p1.y - pi.vy, dvz = p1.z - pi.vz;
+    double s = F(dx, dx, F(dy, dy, F(dz, dz, eps2)));
+    if (EPS0 && MASK) s = self ? 1.0 : s;
+    const double y0 = rsqrt_seed(s);
+    const double e = F(-s, M(y0, y0), 1.0);
+    const double y = F(M(y0, e), F(e, 0.375, 0.5), y0);
+    const double rv = F(dx, dvx, F(dy, dvy, M(dz, dvz)));
+    const double yy = M(y, y);
+    const double mr = M(y, p0.w);
+    const double q = M(yy, mr);
+    const double c1 = M(M(yy, -3.0), rv);                // -3 alpha
+    const double ux = F(c1, dx, dvx), uy = F(c1, dy, dvy), uz = F(c1, dz, dvz);
+    S.ax = F(q, dx, S.ax); S.ay = F(q, dy, S.ay); S.az = F(q, dz, S.az);
+    S.jx = F(q, ux, S.jx); S.jy = F(q, uy, S.jy); S.jz = F(q, uz, S.jz);
+    S.p += (MASK && self) ? 0.0 : mr;
+}
+
+// two j-records at a time, FP64 instruction order as in pair2 (the nine three-source DFMAs of a pair in one pinned run)
+template <bool EPS0, bool MASK>
+__device__ __forceinline__ void pair2_o4(const IPart& pi, const JRec (&J)[2], const double eps2, const bool (&self)[2], Sums& S)
+{
+    double dx[2], dy[2], dz[2], dvx[2], dvy[2], dvz[2];
+    double s[2], rv[2], y0[2], t[2], e[2], h[2], y[2], yy[2], mr[2], z[2], q[2], c1[2];
+#pragma unroll
+    BOTH { VSUB(dz[k], J[k].p0.z, pi.z); VSUB(dvz[k], J[k].p1.z, pi.vz); }
+#pragma unroll
+    BOTH { VSUB(dy[k], J[k].p0.y, pi.y); VSUB(dvy[k], J[k].p1.y, pi.vy); }
+#pragma unroll
+    BOTH { VSUB(dx[k], J[k].p0.x, pi.x); VSUB(dvx[k], J[k].p1.x, pi.vx); }
+#pragma unroll
+    BOTH { VFMA(s[k], dz[k], dz[k], eps2); VMUL(rv[k], dz[k], dvz[k]); }
+#pragma unroll
+    BOTH { VFMA(s[k], dy[k], dy[k], s[k]); VFMA(rv[k], dy[k], dvy[k], rv[k]); }
+#pragma unroll
+    BOTH { VFMA(s[k], dx[k], dx[k], s[k]); VFMA(rv[k], dx[k], dvx[k], rv[k]); }
+    if (EPS0 && MASK) {
+#pragma unroll
+        BOTH s[k] = self[k] ? 1.0 : s[k];
+    }
+#pragma unroll
+    BOTH VRSQ(y0[k], s[k]);
+#pragma unroll
+    BOTH VMUL(t[k], y0[k], y0[k]);
+#pragma unroll
+    BOTH VFNMA(e[k], s[k], t[k], 1.0);
+#pragma unroll
+    BOTH VFMA(h[k], e[k], 0.375, 0.5);
+#pragma unroll
+    BOTH VMUL(t[k], e[k], h[k]);
+#pragma unroll
+    BOTH VFMA(y[k], y0[k], t[k], y0[k]);
+#pragma unroll
+    BOTH VMUL(yy[k], y[k], y[k]);
+#pragma unroll
+    BOTH VMUL(mr[k], y[k], J[k].p0.w);
+#pragma unroll
+    BOTH VMUL(z[k], yy[k], -3.0);
+#pragma unroll
+    BOTH VMUL(q[k], mr[k], yy[k]);
+#pragma unroll
+    BOTH VMUL(c1[k], z[k], rv[k]);
+    {
+        const double m0 = (MASK && self[0]) ? 0.0 : mr[0];
+        VADD(S.p, S.p, m0);
+    }
+    PIN(s[0])
+#pragma unroll
+    BOTH {
+        double ux, uy, uz;
+        VFMA(ux, c1[k], dx[k], dvx[k]);
+        VFMA(uy, c1[k], dy[k], dvy[k]);
+        VFMA(uz, c1[k], dz[k], dvz[k]);
+        VFMA(S.az, q[k], dz[k], S.az);
+        VFMA(S.ay, q[k], dy[k], S.ay);
+        VFMA(S.ax, q[k], dx[k], S.ax);
+        VFMA(S.jx, q[k], ux, S.jx);
+        VFMA(S.jy, q[k], uy, S.jy);
+        VFMA(S.jz, q[k], uz, S.jz);
+        PIN(yy[k])
+        if (k == 0) {
+            const double m1 = (MASK && self[1]) ? 0.0 : mr[1];
+            VADD(S.p, S.p, m1);
+        }
+    }
+}
+
 __device__ __forceinline__ IPart load_ipart(const ForceArgs& A, int i)
 {
     const double4 a = A.pj0[i], b = A.pj1[i];
@@ -318,7 +412,7 @@ static_assert(LI_TJ % 2 == 0, "pair2 takes two j-records at a time");
 // W = 1: a work item is (i-tile of LI_THREADS particles, j-slice).  W = 4 (17..96 active particles): the CTA's four
 // warps hold the SAME 32 particles and each takes its own quarter of every j-tile, so an item is (32 particles,
 // j-slice) and writes four partial planes (slice * 4 + warp) that the reduction adds like any other slices.
-template <bool EPS0, int W>
+template <bool EPS0, int W, int ORDER>
 __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(const ForceArgs A_)
 {
     ForceArgs A = A_;
@@ -398,7 +492,8 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
 #pragma unroll
                     for (int q = 0; q < LI_I; ++q) {
                         const bool self[2] = {jbase + jj == ii[q], jbase + jj + 1 == ii[q]};
-                        pair2<EPS0, true>(pi[q], J, A.eps2, self, acc[q]);
+                        if (ORDER == 4) pair2_o4<EPS0, true>(pi[q], J, A.eps2, self, acc[q]);
+                        else pair2<EPS0, true>(pi[q], J, A.eps2, self, acc[q]);
                     }
                 }
             } else {
@@ -407,7 +502,10 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
                     const JRec J[2] = {{t0p[jj], t1p[jj], t2p[jj]}, {t0p[jj + 1], t1p[jj + 1], t2p[jj + 1]}};
                     const bool self[2] = {false, false};
 #pragma unroll
-                    for (int q = 0; q < LI_I; ++q) pair2<EPS0, false>(pi[q], J, A.eps2, self, acc[q]);
+                    for (int q = 0; q < LI_I; ++q) {
+                        if (ORDER == 4) pair2_o4<EPS0, false>(pi[q], J, A.eps2, self, acc[q]);
+                        else pair2<EPS0, false>(pi[q], J, A.eps2, self, acc[q]);
+                    }
                 }
             }
             __syncthreads();                                   // every warp is done with stage st
@@ -431,7 +529,7 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
-template <bool EPS0>
+template <bool EPS0, int ORDER>
 __global__ void __launch_bounds__(LJ_THREADS, LJ_CTAS_PER_SM) force_lj_kernel(const ForceArgs A_)
 {
     ForceArgs A = A_;
@@ -468,7 +566,10 @@ __global__ void __launch_bounds__(LJ_THREADS, LJ_CTAS_PER_SM) force_lj_kernel(co
             const double2 p2 = n2;
             if (t + 1 < nt) { n0 = A.pj0[j + LJ_TJ]; n1 = A.pj1[j + LJ_TJ]; n2 = A.pj2[j + LJ_TJ]; }   // prefetch
 #pragma unroll
-            for (int q = 0; q < LJ_I; ++q) pair<EPS0>(pi[q], p0, p1, p2, A.eps2, j == ii[q], acc[q]);
+            for (int q = 0; q < LJ_I; ++q) {
+                if (ORDER == 4) pair_o4<EPS0>(pi[q], p0, p1, A.eps2, j == ii[q], acc[q]);
+                else pair<EPS0>(pi[q], p0, p1, p2, A.eps2, j == ii[q], acc[q]);
+            }
             j += LJ_TJ;
         }
 
@@ -537,18 +638,24 @@ __global__ void __launch_bounds__(RED_THREADS) reduce_partials_kernel(const Forc
 
 }  // namespace
 
-cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps_is_zero, cudaStream_t st, int* launches)
+// kernel instantiation for (eps == 0, order)
+#define NB_DISPATCH(CALL)                                               \
+    do {                                                                \
+        if (order == 4) { if (eps_is_zero) { CALL(true, 4); } else { CALL(false, 4); } } \
+        else            { if (eps_is_zero) { CALL(true, 6); } else { CALL(false, 6); } } \
+    } while (0)
+
+cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps_is_zero, int order, cudaStream_t st, int* launches)
 {
-    if (plan.kernel == 0) {
-        if (eps_is_zero) force_li_kernel<true, 1><<<plan.grid, LI_THREADS, 0, st>>>(args);
-        else             force_li_kernel<false, 1><<<plan.grid, LI_THREADS, 0, st>>>(args);
-    } else if (plan.kernel == 2) {
-        if (eps_is_zero) force_li_kernel<true, LI_W><<<plan.grid, LI_THREADS, 0, st>>>(args);
-        else             force_li_kernel<false, LI_W><<<plan.grid, LI_THREADS, 0, st>>>(args);
-    } else {
-        if (eps_is_zero) force_lj_kernel<true><<<plan.grid, LJ_THREADS, 0, st>>>(args);
-        else             force_lj_kernel<false><<<plan.grid, LJ_THREADS, 0, st>>>(args);
-    }
+#define LI1(E, O) force_li_kernel<E, 1, O><<<plan.grid, LI_THREADS, 0, st>>>(args)
+#define LIW(E, O) force_li_kernel<E, LI_W, O><<<plan.grid, LI_THREADS, 0, st>>>(args)
+#define LJ(E, O) force_lj_kernel<E, O><<<plan.grid, LJ_THREADS, 0, st>>>(args)
+    if (plan.kernel == 0) NB_DISPATCH(LI1);
+    else if (plan.kernel == 2) NB_DISPATCH(LIW);
+    else NB_DISPATCH(LJ);
+#undef LI1
+#undef LIW
+#undef LJ
     ++*launches;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -562,20 +669,17 @@ cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps
     return e;
 }
 
-cudaError_t nb_launch_force_devplan(const ForceArgs& args_, bool eps_is_zero, int n_sm, int Npad, cudaStream_t st, int* launches)
+cudaError_t nb_launch_force_devplan(const ForceArgs& args_, bool eps_is_zero, int order, int n_sm, int Npad, cudaStream_t st, int* launches)
 {
     ForceArgs args = args_, args_lj = args_;
     args.n_tiles = Npad / LI_TJ; args_lj.n_tiles = Npad / LJ_TJ;
     const int g_li = n_sm * LI_CTAS_PER_SM, g_lj = n_sm * LJ_CTAS_PER_SM;
-    if (eps_is_zero) {
-        force_lj_kernel<true><<<g_lj, LJ_THREADS, 0, st>>>(args_lj);
-        force_li_kernel<true, LI_W><<<g_li, LI_THREADS, 0, st>>>(args);
-        force_li_kernel<true, 1><<<g_li, LI_THREADS, 0, st>>>(args);
-    } else {
-        force_lj_kernel<false><<<g_lj, LJ_THREADS, 0, st>>>(args_lj);
-        force_li_kernel<false, LI_W><<<g_li, LI_THREADS, 0, st>>>(args);
-        force_li_kernel<false, 1><<<g_li, LI_THREADS, 0, st>>>(args);
-    }
+#define ALL3(E, O)                                                      \
+    force_lj_kernel<E, O><<<g_lj, LJ_THREADS, 0, st>>>(args_lj);        \
+    force_li_kernel<E, LI_W, O><<<g_li, LI_THREADS, 0, st>>>(args);     \
+    force_li_kernel<E, 1, O><<<g_li, LI_THREADS, 0, st>>>(args)
+    NB_DISPATCH(ALL3);
+#undef ALL3
     reduce_partials_kernel<<<n_sm * 4, RED_THREADS, 0, st>>>(args, 1);
     *launches += 4;
     return cudaGetLastError();
@@ -583,6 +687,6 @@ cudaError_t nb_launch_force_devplan(const ForceArgs& args_, bool eps_is_zero, in
 
 void nb_force_occupancy(int* li, int* lj)
 {
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(li, force_li_kernel<false, 1>, LI_THREADS, 0);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(lj, force_lj_kernel<false>, LJ_THREADS, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(li, force_li_kernel<false, 1, 6>, LI_THREADS, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(lj, force_lj_kernel<false, 6>, LJ_THREADS, 0);
 }

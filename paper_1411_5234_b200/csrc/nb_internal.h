@@ -73,13 +73,13 @@ struct ForceArgs {
 };
 
 // nb_force.cu
-cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps_is_zero, cudaStream_t st, int* launches);
+cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps_is_zero, int order, cudaStream_t st, int* launches);
 // device-planned: all three kernel shapes and the reduction at their largest grids; the ones the plan does not name return at once
-cudaError_t nb_launch_force_devplan(const ForceArgs& args, bool eps_is_zero, int n_sm, int Npad, cudaStream_t st, int* launches);
+cudaError_t nb_launch_force_devplan(const ForceArgs& args, bool eps_is_zero, int order, int n_sm, int Npad, cudaStream_t st, int* launches);
 void nb_force_occupancy(int* li_ctas_per_sm, int* lj_ctas_per_sm);
 
 // nb_step.cu
-struct StateArrays { double4 *st0, *st1, *st2, *st3, *st4; double* dt; double4 *pj0, *pj1; double2* pj2; };
+struct StateArrays { double4 *st0, *st1, *st2, *st3, *st4; double* dt; double4 *pj0, *pj1; double2* pj2; int order; /* 4 or 6 */ };
 cudaError_t nb_launch_init_state(const StateArrays& s, int64_t N, int64_t Npad, const double* m, const double* x, const double* v, cudaStream_t st);
 cudaError_t nb_launch_predict(const StateArrays& s, int64_t N, double t, bool own_time, cudaStream_t st);
 cudaError_t nb_launch_startup(const StateArrays& s, int64_t N, const double* fa, const double* fj, const double* fs, int pass,

@@ -52,11 +52,20 @@ __global__ void __launch_bounds__(TPB) predict_kernel(StateArrays s, int64_t N, 
     const double x[3] = {p.x, p.y, p.z}, v[3] = {q.x, q.y, q.z}, a[3] = {r.x, r.y, r.z};
     const double j[3] = {r.w, u.x, u.y}, sn[3] = {u.z, u.w, w.x}, c[3] = {w.y, w.z, w.w};
     double xp[3], vp[3], ap[3];
+    if (s.order == 4) {                                    // 4th-order variant (R21): x to the jerk term, v to D^2/2 jerk
 #pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        xp[k] = fma(D, fma(D2, fma(D3, fma(D4, fma(D5, c[k], sn[k]), j[k]), a[k]), v[k]), x[k]);
-        vp[k] = fma(D, fma(D2, fma(D3, fma(D4, c[k], sn[k]), j[k]), a[k]), v[k]);
-        ap[k] = fma(D, fma(D2, fma(D3, c[k], sn[k]), j[k]), a[k]);
+        for (int k = 0; k < 3; ++k) {
+            xp[k] = fma(D, fma(D2, fma(D3, j[k], a[k]), v[k]), x[k]);
+            vp[k] = fma(D, fma(D2, j[k], a[k]), v[k]);
+            ap[k] = 0.0;                                   // a and jerk do not read it
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            xp[k] = fma(D, fma(D2, fma(D3, fma(D4, fma(D5, c[k], sn[k]), j[k]), a[k]), v[k]), x[k]);
+            vp[k] = fma(D, fma(D2, fma(D3, fma(D4, c[k], sn[k]), j[k]), a[k]), v[k]);
+            ap[k] = fma(D, fma(D2, fma(D3, c[k], sn[k]), j[k]), a[k]);
+        }
     }
     s.pj0[i] = make_double4(xp[0], xp[1], xp[2], p.w);
     s.pj1[i] = make_double4(vp[0], vp[1], vp[2], ap[0]);
@@ -85,12 +94,14 @@ __global__ void startup_kernel(StateArrays s, int64_t N, const double* fa, const
     if (i >= N) return;
     const double ax = fa[3 * i], ay = fa[3 * i + 1], az = fa[3 * i + 2];
     const double jx = fj[3 * i], jy = fj[3 * i + 1], jz = fj[3 * i + 2];
-    if (pass == 1) {
+    if (pass == 1 && s.order != 4) {
         s.st2[i] = make_double4(ax, ay, az, jx);
         s.st3[i] = make_double4(jy, jz, 0.0, 0.0);
         return;
     }
-    const double sx = fs[3 * i], sy = fs[3 * i + 1], sz = fs[3 * i + 2];
+    // 4th-order variant: a and jerk are complete after one evaluation; snap := 0
+    const bool o4 = s.order == 4;
+    const double sx = o4 ? 0.0 : fs[3 * i], sy = o4 ? 0.0 : fs[3 * i + 1], sz = o4 ? 0.0 : fs[3 * i + 2];
     s.st2[i] = make_double4(ax, ay, az, jx);
     s.st3[i] = make_double4(jy, jz, sx, sy);
     s.st4[i] = make_double4(sz, 0.0, 0.0, 0.0);
@@ -114,6 +125,43 @@ __device__ __forceinline__ void corrector_one(const StateArrays& s, const int32_
     const double hh = 0.5 * h;
     const double x0[3] = {p.x, p.y, p.z}, v0[3] = {q.x, q.y, q.z};
     const double a0[3] = {r.x, r.y, r.z}, j0[3] = {r.w, u.x, u.y}, s0[3] = {u.z, u.w, w.x};
+    if (s.order == 4) {
+        // 4th-order variant (R21): cubic Hermite quadrature; d2a/dt2 at the end of the step and d3a/dt3 from the interpolant
+        double a1[3], j1[3], x1[3], v1[3], d2[3], d3[3];
+        const double h2_12 = h * h * (1.0 / 12.0), ih = 1.0 / h, ih2 = ih * ih;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            a1[c] = fa[3 * k + c]; j1[c] = fj[3 * k + c];
+            v1[c] = v0[c] + hh * (a1[c] + a0[c]) - h2_12 * (j1[c] - j0[c]);
+            x1[c] = x0[c] + hh * (v1[c] + v0[c]) - h2_12 * (a1[c] - a0[c]);
+            const double Am = a0[c] - a1[c];
+            d2[c] = (6.0 * Am + h * (2.0 * j0[c] + 4.0 * j1[c])) * ih2;
+            d3[c] = (12.0 * Am + 6.0 * h * (j0[c] + j1[c])) * (ih2 * ih);
+        }
+        s.st0[i] = make_double4(x1[0], x1[1], x1[2], p.w);
+        s.st1[i] = make_double4(v1[0], v1[1], v1[2], t_new);
+        s.st2[i] = make_double4(a1[0], a1[1], a1[2], j1[0]);
+        s.st3[i] = make_double4(j1[1], j1[2], d2[0], d2[1]);
+        s.st4[i] = make_double4(d2[2], d3[0], d3[1], d3[2]);
+        if (dt_shared > 0.0) { s.dt[i] = dt_shared; return; }
+        // dt_crit = eta A1/A2 (eta3 carries eta itself for this order)
+        const double n0 = norm3(a1[0], a1[1], a1[2]), n1 = norm3(j1[0], j1[1], j1[2]);
+        const double n2 = norm3(d2[0], d2[1], d2[2]), n3 = norm3(d3[0], d3[1], d3[2]);
+        const double r1 = eta3 * (sqrt(fma(n0, n2, n1 * n1)) / sqrt(fma(n1, n3, n2 * n2)));
+        int k_crit;
+        if (!(r1 < INFINITY)) k_crit = k_max;
+        else if (!(r1 > 0.0)) k_crit = k_min;
+        else k_crit = clampi(ilog2_pos(r1), k_min, k_max);
+        const int k_old = ilog2_pos(dt_old);
+        int k_new = k_old;
+        if (k_crit < k_old) k_new = k_crit;
+        else if (k_crit > k_old && k_old < k_max) {
+            const double mm = scalbn(t_new, -(k_old + 1));
+            if (mm == rint(mm)) k_new = k_old + 1;
+        }
+        s.dt[i] = scalbn(1.0, k_new);
+        return;
+    }
     double a1[3], j1[3], s1[3], x1[3], v1[3], d3[3], d4[3], d5[3];
     const double h2_10 = h * h * 0.1, h3_120 = h * h * h * (1.0 / 120.0);
     const double ihh = 1.0 / hh, ihh3 = ihh * ihh * ihh;
@@ -466,7 +514,8 @@ cudaError_t nb_launch_corrector(const StateArrays& s, const int32_t* idx, int64_
                                 const double* fa, const double* fj, const double* fs, double eta, int k_min, int k_max,
                                 cudaStream_t st)
 {
-    corrector_kernel<<<nblocks(n_act), TPB, 0, st>>>(s, idx, n_act, dt_shared, t_new, fa, fj, fs, eta * eta * eta, k_min, k_max, nullptr, nullptr);
+    corrector_kernel<<<nblocks(n_act), TPB, 0, st>>>(s, idx, n_act, dt_shared, t_new, fa, fj, fs, s.order == 4 ? eta : eta * eta * eta, k_min, k_max,
+                                                     nullptr, nullptr);
     return cudaGetLastError();
 }
 
@@ -520,7 +569,7 @@ cudaError_t nb_launch_devstep_head(const StateArrays& s, int64_t N, int64_t Npad
 cudaError_t nb_launch_devstep_tail(const StateArrays& s, int n_sm, const int32_t* active, void* scratch, DevPlan* dp, const double* fa,
                                    const double* fj, const double* fs, double eta, int k_min, int k_max, cudaStream_t st, int* launches)
 {
-    corrector_kernel<<<n_sm * 8, TPB, 0, st>>>(s, active, 0, 0.0, 0.0, fa, fj, fs, eta * eta * eta, k_min, k_max, dp,
+    corrector_kernel<<<n_sm * 8, TPB, 0, st>>>(s, active, 0, 0.0, 0.0, fa, fj, fs, s.order == 4 ? eta : eta * eta * eta, k_min, k_max, dp,
                                                (unsigned long long*)scratch);
     *launches += 1;
     return cudaGetLastError();

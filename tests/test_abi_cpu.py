@@ -31,7 +31,7 @@ def test_library_exports_every_declared_symbol(B):
 
 def test_struct_layouts_match_header(B):
     # nb_config: int, void*, void*, size_t, int, double, double, int, int  (natural alignment)
-    assert C.sizeof(B.nb_config) == 64
+    assert C.sizeof(B.nb_config) == 72 and B.nb_config.order.offset == 64
     assert B.nb_config.workspace.offset == 16 and B.nb_config.eta.offset == 40 and B.nb_config.k_max.offset == 60
     assert C.sizeof(B.nb_plan) == 48 and B.nb_plan.waves.offset == 40
 

@@ -410,3 +410,74 @@ def test_config3_reduced_twin_block_steps(B, oracle):
     assert abs((Kg + Wg) - (Ko + Wo)) / abs(Ko + Wo) < 1e-10
     assert abs((Kg + Wg) / (Kg0 + Wg0) - 1) < 1e-5
     g.nb_free()
+
+
+# ------------------------------------------------------------------ 4th-order variant (nb_config.order = 4; R21)
+def test_order4_force_steps_and_block_steps(B, oracle):
+    N, eps = 1500, 1e-3
+    m, x, v = W.plummer(N, 4004, "kroupa")
+    g = B.System(m, x, v, eps, order=4)
+    o = oracle.OracleSystem(m, x, v, eps, order=4)
+    # startup: one evaluation gives a and jerk; snap = crackle = 0; same levels
+    for f, ref in (("A", o.a), ("J", o.j)):
+        assert relvec(g.nb_get_state(f), ref).max() <= TOL
+    assert not g.nb_get_state("S").any() and not g.nb_get_state("C").any()
+    assert np.array_equal(g.nb_get_state("DT"), o.dt)
+    # shared steps: predictor, force (all three kernel shapes), corrector
+    dt = 2.0 ** -9
+    rng = np.random.default_rng(44)
+    for step in range(1, 5):
+        g.nb_predict(step * dt); o.predict(step * dt)
+        for f, ref in (("XP", o.xp), ("VP", o.vp)):
+            assert relvec(g.nb_get_state(f), ref).max() <= 1e-13, f
+        if step == 2:
+            for n_act in (1, 7, 16, 17, 64, 96, 97, 300):
+                idx = rng.choice(N, n_act, replace=False).astype(np.int32)
+                ga, gj, gs, gp = g.nb_force(idx)
+                oa, oj, _, op = oracle_on_gpu_records(oracle, g, eps, idx)
+                assert relvec(ga, oa).max() <= TOL and relvec(gj, oj).max() <= TOL and np.abs(gp / op - 1).max() <= TOL
+                assert not gs.any()                                           # snap is not evaluated at this order
+        ga, gj, gs, gp = g.nb_force()
+        oa, oj, _, op = o.force()
+        assert relvec(ga, oa).max() <= 1e-10 and relvec(gj, oj).max() <= 1e-10        # states differ at round-off after a step
+        g.nb_corrector(None, dt); o.corrector(None, dt)
+    for f, ref, tol in (("X", o.x, 1e-13), ("V", o.v, 1e-12), ("A", o.a, 1e-10), ("J", o.j, 1e-10)):
+        assert relvec(g.nb_get_state(f), ref).max() <= tol, f
+    # the interpolant's a'' and a''' amplify a force difference delta by 6/h^2 and 12/h^3 (see the crackle bound above)
+    nrm = lambda q: np.linalg.norm(q, axis=-1)
+    delta = 1e-11
+    scale = nrm(o.a) + dt * nrm(o.j)
+    assert np.all(nrm(g.nb_get_state("S") - o.s) <= delta * 12 * scale / dt ** 2)
+    assert np.all(nrm(g.nb_get_state("C") - o.c) <= delta * 24 * scale / dt ** 3)
+    Kg, Wg = g.nb_energy(); Ko, Wo = o.energy()
+    assert abs((Kg + Wg) - (Ko + Wo)) / abs(Ko + Wo) < 1e-10
+    g.nb_free()
+    # block steps: same schedule on both sides, then nb_run_blocks bit-identical to the separate calls
+    N = 384
+    m, x, v = W.plummer(N, 4005, "kroupa")
+    g, g2 = B.System(m, x, v, eps, order=4), B.System(m, x, v, eps, order=4)
+    o = oracle.OracleSystem(m, x, v, eps, order=4)
+    steps = 0
+    while True:
+        tg, ng, actg = g.nb_next_block()
+        to, acto = o.next_block()
+        assert tg == to and np.array_equal(actg, acto)
+        if to > 2.0 ** -5:
+            break
+        g.nb_predict(tg); g.nb_force(actg, outputs=False); g.nb_corrector(actg, 0.0)
+        o.predict(to); o.force(acto); o.corrector(acto, 0.0)
+        assert np.array_equal(g.nb_get_state("DT"), o.dt)
+        steps += 1
+    assert steps > 20
+    assert relvec(g.nb_get_state("X"), o.x).max() <= 1e-12
+    s2, t2, _ = g2.nb_run_blocks(2.0 ** -5)
+    assert s2 == steps and t2 == 2.0 ** -5
+    for f in ("X", "V", "A", "J", "S", "C", "T", "DT"):
+        assert np.array_equal(g.nb_get_state(f), g2.nb_get_state(f)), f
+    g.nb_free(); g2.nb_free()
+
+
+def test_order_is_validated(B):
+    m, x, v = W.plummer(64, 1)
+    with pytest.raises(B.NBError):
+        B.System(m, x, v, 1e-3, order=8)
