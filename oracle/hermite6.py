@@ -64,6 +64,17 @@ def lib(kind: str = "ld") -> C.CDLL:
     L.oracle_correct4.restype = None
     L.oracle_aarseth4_dt.argtypes = [_d, C.c_double]
     L.oracle_aarseth4_dt.restype = C.c_double
+    L.oracle_force8.argtypes = [C.c_int64, _d, _d, _d, _d, _d, C.c_double, _i32, C.c_int64, _d, _d, _d, _d, _d]
+    L.oracle_force8.restype = None
+    L.oracle_predict8.argtypes = [C.c_int64, C.c_double, _d] + [_d] * 8 + [_d] * 4
+    L.oracle_predict8.restype = None
+    L.oracle_correct8.argtypes = [C.c_int64, _i32, C.c_int64, C.c_double, C.c_double, _d, _d, _d, _d,
+                                  _d, _d, _d, _d, _d, _d, _d, _d, _d, _d, C.c_double, C.c_int, C.c_int]
+    L.oracle_correct8.restype = None
+    L.oracle_hermite8_derivs.argtypes = [C.c_double] + [_d] * 9
+    L.oracle_hermite8_derivs.restype = None
+    L.oracle_aarseth8_dt.argtypes = [_d, C.c_double]
+    L.oracle_aarseth8_dt.restype = C.c_double
     L.oracle_next_block.argtypes = [C.c_int64, _d, _d, _d, _i32]
     L.oracle_next_block.restype = C.c_int64
     L.oracle_energy.argtypes = [C.c_int64, _d, _d, _d, _d, _d]
@@ -101,12 +112,24 @@ def force(m, xp, vp, ap, eps, idx=None, kind="ld", want=("a", "j", "s", "p")):
     return acc, jerk, snap, pot
 
 
+def force8(m, xp, vp, ap, jp, eps, idx=None, kind="ld"):
+    """O1/8 on explicit arrays: (acc, jerk, snap, crackle [n,3], pot[n]) for the active rows."""
+    N = m.shape[0]
+    m, xp, vp, ap, jp = _f64(m, (N,)), _f64(xp, (N, 3)), _f64(vp, (N, 3)), _f64(ap, (N, 3)), _f64(jp, (N, 3))
+    if idx is not None:
+        idx = np.ascontiguousarray(idx, dtype=np.int32)
+    n = N if idx is None else idx.shape[0]
+    out = [np.zeros((n, 3)) for _ in range(4)] + [np.zeros(n)]
+    lib(kind).oracle_force8(N, _p(m), _p(xp), _p(vp), _p(ap), _p(jp), float(eps), _pi(idx), n, *[_p(o) for o in out])
+    return tuple(out)
+
+
 class OracleSystem:
     """Mirror of the C ABI (include/nb.h) on the CPU: init / predict / force / corrector / next_block."""
 
     def __init__(self, m, x, v, eps, eta=None, eta_s=0.01, k_min=-20, k_max=-3, kind="ld", order=6):
-        assert order in (4, 6)
-        eta = {4: 0.14, 6: 0.45}[order] if eta is None else eta
+        assert order in (4, 6, 8)
+        eta = {4: 0.14, 6: 0.45, 8: 0.75}[order] if eta is None else eta
         self.L = lib(kind)
         self.kind = kind
         self.order = order
@@ -118,6 +141,7 @@ class OracleSystem:
         self.t = np.zeros(N)
         self.dt = np.zeros(N)
         self.xp, self.vp, self.ap = np.zeros((N, 3)), np.zeros((N, 3)), np.zeros((N, 3))
+        self.a4, self.a5, self.jp = np.zeros((N, 3)), np.zeros((N, 3)), np.zeros((N, 3))      # 8th order only
         self.t_pred = 0.0
         self.f = None
         # Startup (R8): pass 1 with a := 0 gives a, jerk; pass 2 with that a gives snap; a''' := 0.
@@ -126,6 +150,11 @@ class OracleSystem:
         if order == 4:                                      # a and jerk need no second pass; snap, crackle := 0
             self.a[:], self.j[:] = a1, j1
             self.pot0 = p1
+        elif order == 8:                                    # R22: a third pass with a and jerk gives crackle; a4 = a5 := 0
+            a2, j2, _, _, _ = force8(self.m, self.x, self.v, a1, zero, self.eps, kind=kind)
+            a3, j3, s3, c3, p3 = force8(self.m, self.x, self.v, a2, j2, self.eps, kind=kind)
+            self.a[:], self.j[:], self.s[:], self.c[:] = a3, j3, s3, c3
+            self.pot0 = p3
         else:
             a2, j2, s2, p2 = force(self.m, self.x, self.v, a1, self.eps, kind=kind)
             self.a[:], self.j[:], self.s[:] = a2, j2, s2
@@ -144,10 +173,16 @@ class OracleSystem:
         o.x, o.v, o.a, o.j, o.s, o.c = (_f64(q, (N, 3)).copy() for q in (x, v, a, j, s, c))
         o.t, o.dt = _f64(t, (N,)).copy(), _f64(dt, (N,)).copy()
         o.xp, o.vp, o.ap = np.zeros((N, 3)), np.zeros((N, 3)), np.zeros((N, 3))
+        o.a4, o.a5, o.jp = np.zeros((N, 3)), np.zeros((N, 3)), np.zeros((N, 3))
         o.t_pred, o.f = 0.0, None
         return o
 
     def predict(self, t):
+        if self.order == 8:
+            self.L.oracle_predict8(self.N, float(t), _p(self.t), _p(self.x), _p(self.v), _p(self.a), _p(self.j), _p(self.s),
+                                   _p(self.c), _p(self.a4), _p(self.a5), _p(self.xp), _p(self.vp), _p(self.ap), _p(self.jp))
+            self.t_pred = float(t)
+            return
         if self.order == 4:
             self.L.oracle_predict4(self.N, float(t), _p(self.t), _p(self.x), _p(self.v), _p(self.a), _p(self.j),
                                    _p(self.xp), _p(self.vp))
@@ -159,6 +194,10 @@ class OracleSystem:
         self.t_pred = float(t)
 
     def force(self, idx=None):
+        if self.order == 8:                                 # (a, jerk, snap, pot, crackle): crackle last, so f[:4] reads as at order 6
+            a, j, s, c, p = force8(self.m, self.xp, self.vp, self.ap, self.jp, self.eps, idx, kind=self.kind)
+            self.f = (a, j, s, p, c)
+            return self.f
         want = ("a", "j", "p") if self.order == 4 else ("a", "j", "s", "p")
         self.f = force(self.m, self.xp, self.vp, self.ap, self.eps, idx, kind=self.kind, want=want)
         return self.f
@@ -167,8 +206,13 @@ class OracleSystem:
         if idx is not None:
             idx = np.ascontiguousarray(idx, dtype=np.int32)
         n = self.N if idx is None else idx.shape[0]
-        a1, j1, s1, _ = self.f
+        a1, j1, s1 = self.f[:3]
         assert a1.shape[0] == n
+        if self.order == 8:
+            self.L.oracle_correct8(self.N, _pi(idx), n, float(dt), self.t_pred, _p(a1), _p(j1), _p(s1), _p(self.f[4]),
+                                   _p(self.x), _p(self.v), _p(self.a), _p(self.j), _p(self.s), _p(self.c), _p(self.a4), _p(self.a5),
+                                   _p(self.t), _p(self.dt), self.eta, self.k_min, self.k_max)
+            return
         if self.order == 4:
             self.L.oracle_correct4(self.N, _pi(idx), n, float(dt), self.t_pred, _p(a1), _p(j1),
                                    _p(self.x), _p(self.v), _p(self.a), _p(self.j), _p(self.s), _p(self.c),

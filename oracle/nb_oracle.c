@@ -32,11 +32,13 @@
 #define R_CBRT cbrtl
 #define R_LOG2 log2l
 #define R_FLOOR floorl
+#define R_POW powl
 #else
 #define R_SQRT sqrt
 #define R_CBRT cbrt
 #define R_LOG2 log2
 #define R_FLOOR floor
+#define R_POW pow
 #endif
 typedef REAL real;
 
@@ -325,6 +327,182 @@ void oracle_correct4(int64_t N, const int32_t* idx, int64_t n_act, double dt_sha
         } else {
             int k_old = (int)lrint(log2(dt[i]));
             int k_crit = level_clamp(aarseth4_dt(d, eta), k_min, k_max);
+            int k_new = k_old;
+            if (k_crit < k_old) k_new = k_crit;
+            else if (k_crit > k_old && k_old < k_max && fmod(t_new, ldexp(1.0, k_old + 1)) == 0.0) k_new = k_old + 1;
+            dt[i] = ldexp(1.0, k_new);
+        }
+    }
+}
+
+/*
+ * ---- 8th-order variant ("Hermite time integrators (4th, 6th and 8th order)"; formulas: DESIGN.md R22) ----
+ *
+ * O1/8 - pairwise evaluation with the third time derivative ("crackle") added.  With dj = j_j - j_i (predicted
+ * jerks), alpha and beta as in O1 and
+ *   gamma = (3 dv.da + dx.dj)/s + alpha (3 beta - 4 alpha^2),
+ *   u = dv - 3 alpha dx,  w = da - 6 alpha u - 3 beta dx   (jerk and snap terms per unit q = m_j s^(-3/2)),
+ *   crackle_i = d3/dt3 a_i = sum q (dj - 9 alpha w - 9 beta u - 3 gamma dx).
+ */
+void oracle_force8(int64_t N, const double* m, const double* xp, const double* vp, const double* ap, const double* jp,
+                   double eps, const int32_t* idx, int64_t n_act,
+                   double* acc, double* jerk, double* snap, double* crackle, double* pot)
+{
+    const real e2 = (real)eps * (real)eps;
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t k = 0; k < n_act; ++k) {
+        const int64_t i = idx ? (int64_t)idx[k] : k;
+        real A[3] = {0, 0, 0}, J[3] = {0, 0, 0}, S[3] = {0, 0, 0}, C[3] = {0, 0, 0}, P = 0;
+        for (int64_t j = 0; j < N; ++j) {
+            if (j == i) continue;
+            real dx[3], dv[3], da[3], dj[3];
+            for (int q = 0; q < 3; ++q) {
+                dx[q] = (real)xp[3 * j + q] - (real)xp[3 * i + q];
+                dv[q] = (real)vp[3 * j + q] - (real)vp[3 * i + q];
+                da[q] = (real)ap[3 * j + q] - (real)ap[3 * i + q];
+                dj[q] = (real)jp[3 * j + q] - (real)jp[3 * i + q];
+            }
+            const real s = dx[0] * dx[0] + dx[1] * dx[1] + dx[2] * dx[2] + e2;
+            const real rho2 = 1 / s, rho = R_SQRT(rho2);
+            const real q_ = (real)m[j] * rho * rho2;
+            const real xv = dx[0] * dv[0] + dx[1] * dv[1] + dx[2] * dv[2];
+            const real vv = dv[0] * dv[0] + dv[1] * dv[1] + dv[2] * dv[2];
+            const real xa = dx[0] * da[0] + dx[1] * da[1] + dx[2] * da[2];
+            const real va = dv[0] * da[0] + dv[1] * da[1] + dv[2] * da[2];
+            const real xj = dx[0] * dj[0] + dx[1] * dj[1] + dx[2] * dj[2];
+            const real alpha = xv * rho2;
+            const real beta = (vv + xa) * rho2 + alpha * alpha;
+            const real gamma = (3 * va + xj) * rho2 + alpha * (3 * beta - 4 * alpha * alpha);
+            for (int c = 0; c < 3; ++c) {
+                const real u = dv[c] - 3 * alpha * dx[c];
+                const real w = da[c] - 6 * alpha * u - 3 * beta * dx[c];
+                A[c] += q_ * dx[c];
+                J[c] += q_ * u;
+                S[c] += q_ * w;
+                C[c] += q_ * (dj[c] - 9 * alpha * w - 9 * beta * u - 3 * gamma * dx[c]);
+            }
+            P -= (real)m[j] * rho;
+        }
+        for (int c = 0; c < 3; ++c) {
+            if (acc) acc[3 * k + c] = (double)A[c];
+            if (jerk) jerk[3 * k + c] = (double)J[c];
+            if (snap) snap[3 * k + c] = (double)S[c];
+            if (crackle) crackle[3 * k + c] = (double)C[c];
+        }
+        if (pot) pot[k] = (double)P;
+    }
+}
+
+/*
+ * O2/8 - predictor: x_p to D^7/5040 a5, v_p to D^6/720 a5, a_p to D^5/120 a5, j_p to D^4/24 a5, where
+ * a4 = d4a/dt4 and a5 = d5a/dt5 come from the previous corrector's interpolant (0 before the first step).
+ */
+void oracle_predict8(int64_t N, double t, const double* ti, const double* x, const double* v, const double* a,
+                     const double* j, const double* s, const double* c, const double* a4, const double* a5,
+                     double* xp, double* vp, double* ap, double* jp)
+{
+    for (int64_t i = 0; i < N; ++i) {
+        const real D = (real)t - (real)ti[i];
+        const real D2 = D * D, D3 = D2 * D, D4 = D3 * D, D5 = D4 * D, D6 = D5 * D, D7 = D6 * D;
+        for (int k = 0; k < 3; ++k) {
+            const int64_t e = 3 * i + k;
+            xp[e] = (double)((real)x[e] + D * v[e] + D2 / 2 * a[e] + D3 / 6 * j[e] + D4 / 24 * s[e] + D5 / 120 * c[e]
+                             + D6 / 720 * a4[e] + D7 / 5040 * a5[e]);
+            vp[e] = (double)((real)v[e] + D * a[e] + D2 / 2 * j[e] + D3 / 6 * s[e] + D4 / 24 * c[e] + D5 / 120 * a4[e]
+                             + D6 / 720 * a5[e]);
+            ap[e] = (double)((real)a[e] + D * j[e] + D2 / 2 * s[e] + D3 / 6 * c[e] + D4 / 24 * a4[e] + D5 / 120 * a5[e]);
+            jp[e] = (double)((real)j[e] + D * s[e] + D2 / 2 * c[e] + D3 / 6 * a4[e] + D4 / 24 * a5[e]);
+        }
+    }
+}
+
+/*
+ * The septic Hermite interpolant of a(t) through (a, j, s, c) at both ends of a step of length h, about the mid-point in
+ * tau = (t - t_mid)/hh, hh = h/2.  With Am = a1 - a0, Jp = hh (j1 + j0), Jm = hh (j1 - j0), Sp = hh^2 (s1 + s0),
+ * Sm = hh^2 (s1 - s0), Cp = hh^3 (c1 + c0), Cm = hh^3 (c1 - c0), its derivatives at the END of the step are
+ *   hh^4 a4 = (-105 Am + 105 Jp + 15 Jm - 45 Sm - 15 Sp)/2 + 5 Cp + 3 Cm
+ *   hh^5 a5 = -315 Am + 315 Jp + (45 Jm - 255 Sm - 45 Sp + 45 Cp + 15 Cm)/2
+ *   hh^6 a6 = (-1575 Am + 1575 Jp + 45 Jm - 45 Sp + 105 Cp + 15 Cm)/2 - 315 Sm
+ *   hh^7 a7 = (-1575 Am + 1575 Jp + 105 Cp)/2 - 315 Sm
+ * (solved from the eight end-point conditions; checked by the polynomial-exactness pin).
+ */
+static void hermite8_end_derivs(real hh, real A0, real J0, real S0, real C0, real A1, real J1, real S1, real C1, real out[4])
+{
+    const real Am = A1 - A0;
+    const real Jp = hh * (J1 + J0), Jm = hh * (J1 - J0);
+    const real Sp = hh * hh * (S1 + S0), Sm = hh * hh * (S1 - S0);
+    const real Cp = hh * hh * hh * (C1 + C0), Cm = hh * hh * hh * (C1 - C0);
+    const real h4 = hh * hh * hh * hh;
+    out[0] = ((-105 * Am + 105 * Jp + 15 * Jm - 45 * Sm - 15 * Sp) / 2 + 5 * Cp + 3 * Cm) / h4;
+    out[1] = (-315 * Am + 315 * Jp + (45 * Jm - 255 * Sm - 45 * Sp + 45 * Cp + 15 * Cm) / 2) / (h4 * hh);
+    out[2] = ((-1575 * Am + 1575 * Jp + 45 * Jm - 45 * Sp + 105 * Cp + 15 * Cm) / 2 - 315 * Sm) / (h4 * hh * hh);
+    out[3] = ((-1575 * Am + 1575 * Jp + 105 * Cp) / 2 - 315 * Sm) / (h4 * hh * hh * hh);
+}
+
+void oracle_hermite8_derivs(double h, const double* a0, const double* j0, const double* s0, const double* c0,
+                            const double* a1, const double* j1, const double* s1, const double* c1, double* d4567)
+{
+    for (int q = 0; q < 3; ++q) {
+        real o[4];
+        hermite8_end_derivs((real)h / 2, a0[q], j0[q], s0[q], c0[q], a1[q], j1[q], s1[q], c1[q], o);
+        for (int r = 0; r < 4; ++r) d4567[3 * r + q] = (double)o[r];
+    }
+}
+
+/* O4/8 - generalised Aarseth criterion for an 8th-order scheme: dt_crit = eta (A1/A6)^(1/5);
+ * d[0..7] = a, a', ..., a^(7) at the new time. */
+static real aarseth8_dt(real d[8][3], double eta)
+{
+    const real n0 = norm3(d[0]), n1 = norm3(d[1]), n2 = norm3(d[2]);
+    const real n5 = norm3(d[5]), n6 = norm3(d[6]), n7 = norm3(d[7]);
+    const real r = R_SQRT(n0 * n2 + n1 * n1) / R_SQRT(n5 * n7 + n6 * n6);
+    return (real)eta * R_POW(r, (real)1 / 5);
+}
+
+double oracle_aarseth8_dt(const double* d24, double eta)
+{
+    real d[8][3];
+    for (int r = 0; r < 8; ++r) for (int q = 0; q < 3; ++q) d[r][q] = d24[3 * r + q];
+    return (double)aarseth8_dt(d, eta);
+}
+
+/*
+ * O3/8 - corrector: the two-point septic Hermite quadrature
+ *   v1 = v0 + h/2 (a1 + a0) - 3 h^2/28 (j1 - j0) + h^3/84 (s1 + s0) - h^4/1680 (c1 - c0)
+ *   x1 = x0 + h/2 (v1 + v0) - 3 h^2/28 (a1 - a0) + h^3/84 (j1 + j0) - h^4/1680 (s1 - s0)
+ * Stored afterwards: x1, v1, a1, j1, s1, c1 (evaluated at the predicted state), a4, a5 := the interpolant's at t1.
+ */
+void oracle_correct8(int64_t N, const int32_t* idx, int64_t n_act, double dt_shared, double t_new,
+                     const double* a1, const double* j1, const double* s1, const double* c1,
+                     double* x, double* v, double* a, double* j, double* s, double* c, double* a4, double* a5,
+                     double* ti, double* dt, double eta, int k_min, int k_max)
+{
+    (void)N;
+    for (int64_t k = 0; k < n_act; ++k) {
+        const int64_t i = idx ? (int64_t)idx[k] : k;
+        const real h = dt_shared > 0 ? (real)dt_shared : (real)dt[i];
+        real d[8][3];
+        for (int q = 0; q < 3; ++q) {
+            const int64_t e = 3 * i + q, f = 3 * k + q;
+            const real A0 = a[e], J0 = j[e], S0 = s[e], C0 = c[e], A1 = a1[f], J1 = j1[f], S1 = s1[f], C1 = c1[f];
+            const real v0 = v[e], x0 = x[e];
+            const real h2 = h * h, h3 = h2 * h, h4 = h3 * h;
+            const real v1 = v0 + h / 2 * (A1 + A0) - 3 * h2 / 28 * (J1 - J0) + h3 / 84 * (S1 + S0) - h4 / 1680 * (C1 - C0);
+            const real x1 = x0 + h / 2 * (v1 + v0) - 3 * h2 / 28 * (A1 - A0) + h3 / 84 * (J1 + J0) - h4 / 1680 * (S1 - S0);
+            real o[4];
+            hermite8_end_derivs(h / 2, A0, J0, S0, C0, A1, J1, S1, C1, o);
+            d[0][q] = A1; d[1][q] = J1; d[2][q] = S1; d[3][q] = C1;
+            d[4][q] = o[0]; d[5][q] = o[1]; d[6][q] = o[2]; d[7][q] = o[3];
+            x[e] = (double)x1; v[e] = (double)v1;
+            a[e] = (double)A1; j[e] = (double)J1; s[e] = (double)S1; c[e] = (double)C1;
+            a4[e] = (double)o[0]; a5[e] = (double)o[1];
+        }
+        ti[i] = t_new;
+        if (dt_shared > 0) {
+            dt[i] = dt_shared;
+        } else {
+            int k_old = (int)lrint(log2(dt[i]));
+            int k_crit = level_clamp(aarseth8_dt(d, eta), k_min, k_max);
             int k_new = k_old;
             if (k_crit < k_old) k_new = k_crit;
             else if (k_crit > k_old && k_old < k_max && fmod(t_new, ldexp(1.0, k_old + 1)) == 0.0) k_new = k_old + 1;

@@ -402,3 +402,129 @@ def test_o4_criterion_closed_form_and_block_steps(oracle):
         n += 1
     assert np.all(o.t == 0.125) and n > 10
     assert abs(sum(o.energy()) / E0 - 1) < 1e-5
+
+
+# ---------------------------------------------------------------- 8th-order variant (R22)
+@pytest.mark.parametrize("N,eps,seed", [(2, 0.0, 21), (3, 0.05, 22), (4, 0.3, 23)])
+def test_o8_crackle_against_mpmath_differentiation(oracle, N, eps, seed):
+    """a, jerk, snap, crackle of O1/8 = a(tau) and its first three derivatives along
+    x(tau) = x + v tau + a_p tau^2/2 + j_p tau^3/6, in 50-digit arithmetic: pins alpha, beta, gamma and every coefficient."""
+    mp.mp.dps = 50
+    rng = np.random.default_rng(seed)
+    m = rng.uniform(0.2, 1.0, N)
+    x, v, ap, jp = (rng.normal(size=(N, 3)) for _ in range(4))
+    idx = np.arange(N, dtype=np.int32)[::-1].copy()
+    acc, jerk, snap, crk, pot = oracle.hermite6.force8(m, x, v, ap, jp, eps, idx)
+    a6, j6, s6, p6 = oracle.hermite6.force(m, x, v, ap, eps, idx)
+    assert np.array_equal(acc, a6) and np.array_equal(jerk, j6) and np.array_equal(pot, p6)
+    np.testing.assert_allclose(snap, s6, rtol=1e-14)
+
+    def pos(i, k, tau):
+        return mp.mpf(x[i, k]) + mp.mpf(v[i, k]) * tau + mp.mpf(ap[i, k]) * tau ** 2 / 2 + mp.mpf(jp[i, k]) * tau ** 3 / 6
+
+    def a_of_tau(i, c, tau):
+        tot = mp.mpf(0)
+        for jj in range(N):
+            if jj == i:
+                continue
+            d = [pos(jj, k, tau) - pos(i, k, tau) for k in range(3)]
+            s = d[0] ** 2 + d[1] ** 2 + d[2] ** 2 + mp.mpf(eps) ** 2
+            tot += mp.mpf(m[jj]) * d[c] / s ** mp.mpf(1.5)
+        return tot
+
+    for k, i in enumerate(idx):
+        for c in range(3):
+            c_ref = mp.diff(lambda t: a_of_tau(i, c, t), 0, 3)
+            s_ref = mp.diff(lambda t: a_of_tau(i, c, t), 0, 2)
+            assert abs(crk[k, c] - float(c_ref)) <= 1e-15 * max(abs(float(c_ref)), np.abs(crk[k]).max())
+            assert abs(snap[k, c] - float(s_ref)) <= 4e-16 * max(abs(float(s_ref)), np.abs(snap[k]).max())
+
+
+def test_o8_newtons_third_law_and_startup(oracle):
+    m, x, v = W.plummer(48, 8, "kroupa")
+    o = oracle.OracleSystem(m, x, v, 1e-2, order=8)
+    for arr in (o.a, o.j, o.s, o.c):                         # crackle obeys it only if dj uses the same jerk array for i and j
+        total = (m[:, None] * arr).sum(0)
+        assert np.abs(total).max() <= 1e-15 * (m[:, None] * np.abs(arr)).sum()
+    o6 = oracle.OracleSystem(m, x, v, 1e-2, order=6)
+    assert np.array_equal(o.a, o6.a) and np.array_equal(o.j, o6.j)
+    np.testing.assert_allclose(o.s, o6.s, rtol=1e-14)          # same sum, another order of the operations
+
+
+def test_o8_predictor_and_corrector_polynomial_exactness(oracle):
+    rng = np.random.default_rng(18)
+    L = oracle.lib("ld")
+    P = oracle.hermite6._p
+    N = 5
+    coef = rng.normal(size=(8, N, 3))                       # x, v, a, j, s, c, a4, a5 at t_i
+    ti = rng.choice([0.0, 0.25, 0.5], N)
+    t = 0.75
+    out = [np.zeros((N, 3)) for _ in range(4)]
+    L.oracle_predict8(N, t, P(ti), *[P(np.ascontiguousarray(c)) for c in coef], *[P(o) for o in out])
+    D = (t - ti)[:, None]
+    fact = [1, 1, 2, 6, 24, 120, 720, 5040]
+    for lo, got in enumerate(out):                           # x_p, v_p, a_p, j_p
+        ref = sum(coef[k] * D ** (k - lo) / fact[k - lo] for k in range(lo, 8))
+        np.testing.assert_allclose(got, ref, rtol=0, atol=4e-15)
+    for deg in (6, 7):
+        h, t0 = 0.25, 0.5
+        pa = [np.polynomial.Polynomial(rng.normal(size=deg + 1)) for _ in range(3)]
+        pv = [p.integ() + rng.normal() for p in pa]
+        px = [p.integ() + rng.normal() for p in pv]
+        ev = lambda polys, k, tt: np.array([[p.deriv(k)(tt) if k else p(tt) for p in polys]])
+        x, v = ev(px, 0, t0), ev(pv, 0, t0)
+        a, j, s, c = (ev(pa, k, t0) for k in range(4))
+        a4, a5 = np.zeros((1, 3)), np.zeros((1, 3))
+        t1 = t0 + h
+        a1, j1, s1, c1 = (ev(pa, k, t1) for k in range(4))
+        d = np.zeros(12)
+        L.oracle_hermite8_derivs(h, P(a), P(j), P(s), P(c), P(a1), P(j1), P(s1), P(c1), P(d))
+        for r, tol in zip(range(4), (1e-9, 1e-8, 1e-6, 1e-5)):
+            np.testing.assert_allclose(d[3 * r:3 * r + 3], ev(pa, 4 + r, t1)[0], rtol=0, atol=tol)
+        tt, dt = np.array([t0]), np.array([h])
+        L.oracle_correct8(1, None, 1, h, t1, P(a1), P(j1), P(s1), P(c1), P(x), P(v), P(a), P(j), P(s), P(c), P(a4), P(a5),
+                          P(tt), P(dt), 0.75, -20, -3)
+        np.testing.assert_allclose(v, ev(pv, 0, t1), rtol=0, atol=1e-14)
+        if deg == 6:
+            np.testing.assert_allclose(x, ev(px, 0, t1), rtol=0, atol=1e-14)
+        np.testing.assert_allclose(a4, ev(pa, 4, t1), rtol=0, atol=1e-9)
+        np.testing.assert_allclose(a5, ev(pa, 5, t1), rtol=0, atol=1e-8)
+        assert tt[0] == t1 and np.array_equal(c, c1)
+
+
+def test_o8_kepler_orbit_eighth_order_convergence(oracle):
+    e = 0.5
+    m = np.array([0.5, 0.5])
+    x = np.array([[0.75, 0, 0], [-0.75, 0, 0]])
+    vy = 0.5 * np.sqrt((1 - e) / (1 + e))
+    v = np.array([[0, vy, 0], [0, -vy, 0]])
+    dx = []
+    for n in (64, 128, 256):
+        o = oracle.OracleSystem(m, x, v, 0.0, order=8)
+        for _ in range(n):
+            o.shared_step(2 * np.pi / n)
+        dx.append(np.abs(o.x - x).max())
+    assert dx[0] < 1e-4 and dx[2] < 1e-9
+    assert dx[0] / dx[1] > 150 and dx[1] / dx[2] > 150           # ~2^8 per halving: 8th order (6th gives ~64)
+
+
+def test_o8_criterion_closed_form_and_block_steps(oracle):
+    L = oracle.lib("ld")
+    P = oracle.hermite6._p
+    for w_ in (0.7, 3.0, 41.0):                                   # |a^(k)| = w^k |a|  =>  (A1/A6)^(1/5) = 1/w
+        d = np.zeros((8, 3))
+        for k in range(8):
+            d[k, k % 3] = 2.5 * w_ ** k
+        assert abs(L.oracle_aarseth8_dt(P(d), 0.75) * w_ / 0.75 - 1) < 1e-15
+    m, x, v = W.plummer(96, 11)
+    o = oracle.OracleSystem(m, x, v, 1e-2, order=8)
+    E0 = sum(o.energy())
+    n = 0
+    while True:
+        tn, act = o.next_block()
+        if tn > 0.125:
+            break
+        o.predict(tn); o.force(act); o.corrector(act, 0.0)
+        n += 1
+    assert np.all(o.t == 0.125) and n > 10
+    assert abs(sum(o.energy()) / E0 - 1) < 1e-6
