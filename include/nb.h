@@ -57,7 +57,10 @@ typedef struct {
     int order;              /* Hermite order ("4th, 6th and 8th order"): 0 or 6 = the 6th-order scheme of the
                                north star; 4 = the 4th-order variant (reading R21): nb_force evaluates a, jerk and pot (snap
                                is returned as 0), the predictor stops at the jerk term, nb_corrector is the cubic Hermite
-                               quadrature and the criterion dt = eta A1/A2.  8 is not built (NB_EINVAL). */
+                               quadrature and the criterion dt = eta A1/A2;
+                               8 = the 8th-order variant (reading R22): nb_force also evaluates crackle = d3a/dt3 (read it with
+                               nb_force_crackle), the predictor runs to d5a/dt5 and predicts the jerk, nb_corrector is the
+                               septic Hermite quadrature, criterion dt = eta (A1/A6)^(1/5), eta -> 0.75, three startup passes. */
 } nb_config;
 
 /* Selectors of nb_get_state / nb_set_state.  Width = doubles per particle. */
@@ -73,7 +76,10 @@ typedef enum {
     NB_DT = 8,  /* particle step dt_i (a power of two), 1 */
     NB_XP = 9,  /* predicted position at the time of the last nb_predict, 3 (get only) */
     NB_VP = 10, /* predicted velocity, 3 (get only) */
-    NB_AP = 11  /* predicted acceleration, 3 (get only) */
+    NB_AP = 11, /* predicted acceleration, 3 (get only) */
+    NB_A4 = 12, /* d4a/dt4 from the corrector's interpolant, 3 (8th order only) */
+    NB_A5 = 13, /* d5a/dt5, 3 (8th order only) */
+    NB_JP = 14  /* predicted jerk, 3 (get only; 8th order only) */
 } nb_field;
 
 /* How nb_force maps an evaluation onto the GPU (reading R15; "Bfactor"). */
@@ -138,6 +144,9 @@ int nb_predict(nb_ctx* ctx, double t);
  */
 int nb_force(nb_ctx* ctx, const int32_t* active_idx, int64_t n_act,
              double* a, double* jerk, double* snap, double* pot);
+
+/* 8th order only: crackle [n_act][3] (h/d) of the last nb_force, row k <-> active_idx[k].  NB_ESTATE otherwise. */
+int nb_force_crackle(nb_ctx* ctx, double* crackle);
 
 /*
  * nb_corrector — finish the Hermite-6 step (formulas: reading R10) for the active

@@ -16,11 +16,11 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libnb.so")
 
 NB_OK, NB_EINVAL, NB_ENOMEM, NB_ESTATE, NB_ECUDA = 0, -1, -2, -3, -4
-FIELDS = dict(M=0, X=1, V=2, A=3, J=4, S=5, C=6, T=7, DT=8, XP=9, VP=10, AP=11)
+FIELDS = dict(M=0, X=1, V=2, A=3, J=4, S=5, C=6, T=7, DT=8, XP=9, VP=10, AP=11, A4=12, A5=13, JP=14)
 _WIDTH = {0: 1, 7: 1, 8: 1}
 ACTIVE_INTERNAL = C.c_void_p(1)
 
-EXPORTS = ["nb_workspace_bytes", "nb_plan_force", "nb_set_max_split", "nb_init", "nb_predict", "nb_force", "nb_corrector",
+EXPORTS = ["nb_workspace_bytes", "nb_plan_force", "nb_set_max_split", "nb_init", "nb_predict", "nb_force", "nb_force_crackle", "nb_corrector",
            "nb_next_block", "nb_run_blocks", "nb_get_state", "nb_set_state", "nb_energy", "nb_probe_fp64_peak", "nb_probe_dfma_sources",
            "nb_launch_count", "nb_last_force_ms", "nb_strerror", "nb_last_error", "nb_free"]
 
@@ -62,6 +62,7 @@ def lib() -> C.CDLL:
     L.nb_init.argtypes = [C.POINTER(vp), i64, vp, vp, vp, dbl, C.POINTER(nb_config)]; L.nb_init.restype = C.c_int
     L.nb_predict.argtypes = [vp, dbl]; L.nb_predict.restype = C.c_int
     L.nb_force.argtypes = [vp, vp, i64, vp, vp, vp, vp]; L.nb_force.restype = C.c_int
+    L.nb_force_crackle.argtypes = [vp, vp]; L.nb_force_crackle.restype = C.c_int
     L.nb_corrector.argtypes = [vp, vp, i64, dbl]; L.nb_corrector.restype = C.c_int
     L.nb_next_block.argtypes = [vp, C.POINTER(dbl), vp, C.POINTER(i64)]; L.nb_next_block.restype = C.c_int
     L.nb_run_blocks.argtypes = [vp, dbl, i64, C.POINTER(i64), C.POINTER(dbl), C.POINTER(i64)]; L.nb_run_blocks.restype = C.c_int
@@ -176,6 +177,12 @@ class System:
             a = j = s = p = None
         self._check(self.L.nb_force(self.ctx, ip, n, _ptr(a), _ptr(j), _ptr(s), _ptr(p)))
         return a, j, s, p
+
+    def nb_force_crackle(self, n):
+        """Crackle [n, 3] of the last nb_force over n active particles (8th order)."""
+        out = self._out(n, 3)
+        self._check(self.L.nb_force_crackle(self.ctx, _ptr(out)))
+        return out
 
     def nb_corrector(self, active_idx=None, dt=0.0, n_act=None):
         if active_idx is None:

@@ -28,7 +28,7 @@ struct Carve {
 // one place that defines the workspace layout, used for sizing (base = nullptr) and for carving
 struct Layout {
     StateArrays s;
-    double *fa, *fj, *fs, *fp;          // force results, row k <-> active_idx[k]
+    double *fa, *fj, *fs, *fp, *fc;     // force results (fc: crackle, 8th order), row k <-> active_idx[k]
     double* partial;
     int32_t *idx_user, *idx_sched, *idx_tmp;
     double* stage;                      // staging for host <-> device transfers, 10 doubles per particle
@@ -42,8 +42,10 @@ struct Layout {
         s.st0 = c.take<double4>(Npad); s.st1 = c.take<double4>(Npad); s.st2 = c.take<double4>(Npad);
         s.st3 = c.take<double4>(Npad); s.st4 = c.take<double4>(Npad); s.dt = c.take<double>(Npad);
         s.pj0 = c.take<double4>(Npad); s.pj1 = c.take<double4>(Npad); s.pj2 = c.take<double2>(Npad);
+        s.st5 = c.take<double4>(Npad); s.st6 = c.take<double4>(Npad); s.pj3 = c.take<double4>(Npad);
         fa = c.take<double>(3 * Npad); fj = c.take<double>(3 * Npad); fs = c.take<double>(3 * Npad); fp = c.take<double>(Npad);
-        partial = c.take<double>(10 * partial_rows(Npad));
+        fc = c.take<double>(3 * Npad); s.fc = fc; s.order = 6;
+        partial = c.take<double>(13 * partial_rows(Npad));   // 10 components, 13 at the 8th order
         idx_user = c.take<int32_t>(Npad); idx_sched = c.take<int32_t>(Npad); idx_tmp = c.take<int32_t>(Npad);
         stage = c.take<double>(10 * Npad);
         scratch = c.take<char>(scratch_bytes(Npad));
@@ -90,11 +92,11 @@ int fail_cuda(nb_ctx* c, cudaError_t e, const char* where)
 ForceArgs base_force_args(const nb_ctx* ctx)
 {
     ForceArgs A{};
-    A.pj0 = ctx->L.s.pj0; A.pj1 = ctx->L.s.pj1; A.pj2 = ctx->L.s.pj2;
+    A.pj0 = ctx->L.s.pj0; A.pj1 = ctx->L.s.pj1; A.pj2 = ctx->L.s.pj2; A.pj3 = ctx->L.s.pj3;
     A.eps2 = ctx->eps * ctx->eps;
     A.partial = ctx->L.partial;
     A.queue = ctx->L.queue;                                 // zeroed by nb_init, left at 0 by every launch
-    A.out_a = ctx->L.fa; A.out_j = ctx->L.fj; A.out_s = ctx->L.fs; A.out_p = ctx->L.fp;
+    A.out_a = ctx->L.fa; A.out_j = ctx->L.fj; A.out_s = ctx->L.fs; A.out_p = ctx->L.fp; A.out_c = ctx->L.fc;
     return A;
 }
 
@@ -196,7 +198,7 @@ int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const dou
     const int k_min = (cfg->k_min == 0 && cfg->k_max == 0) ? -20 : cfg->k_min;
     const int k_max = (cfg->k_min == 0 && cfg->k_max == 0) ? -3 : cfg->k_max;
     if (k_min > k_max || k_min < -1000 || k_max > 1000 || cfg->eta < 0 || cfg->eta_s < 0) return NB_EINVAL;
-    if (cfg->order != 0 && cfg->order != 4 && cfg->order != 6) return NB_EINVAL;
+    if (cfg->order != 0 && cfg->order != 4 && cfg->order != 6 && cfg->order != 8) return NB_EINVAL;
     const int64_t Npad = pad_n(N);
     if (!cfg->workspace || ((uintptr_t)cfg->workspace % ALIGN) != 0 || cfg->workspace_bytes < Layout(nullptr, Npad).bytes)
         return NB_ENOMEM;
@@ -209,7 +211,7 @@ int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const dou
     ctx->on_device = cfg->ptrs_on_device != 0;
     ctx->N = N; ctx->Npad = Npad; ctx->eps = eps;
     ctx->order = cfg->order == 0 ? 6 : cfg->order;
-    ctx->eta = cfg->eta > 0 ? cfg->eta : (ctx->order == 4 ? 0.14 : 0.45);
+    ctx->eta = cfg->eta > 0 ? cfg->eta : (ctx->order == 4 ? 0.14 : ctx->order == 8 ? 0.75 : 0.45);
     ctx->eta_s = cfg->eta_s > 0 ? cfg->eta_s : 0.01;
     ctx->k_min = k_min; ctx->k_max = k_max;
     ctx->L = Layout(cfg->workspace, Npad);
@@ -234,7 +236,7 @@ int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const dou
     ctx->launches += 1;
 
     // startup (reading R8): two all-active evaluations at t = 0
-    for (int pass = 1; pass <= (ctx->order == 4 ? 1 : 2); ++pass) {
+    for (int pass = 1; pass <= (ctx->order == 4 ? 1 : ctx->order == 8 ? 3 : 2); ++pass) {
         CU(nb_launch_predict(ctx->L.s, N, 0.0, true, ctx->stream), "predict");
         ctx->launches += 1;
         ctx->predicted = true; ctx->t_pred = 0.0;
@@ -294,6 +296,16 @@ int nb_force(nb_ctx* ctx, const int32_t* active_idx, int64_t n_act, double* a, d
     if ((rc = copy_out(ctx, snap, ctx->L.fs, 3 * n_act)) != NB_OK) return rc;
     if ((rc = copy_out(ctx, pot, ctx->L.fp, n_act)) != NB_OK) return rc;
     if (!ctx->on_device) CU(cudaStreamSynchronize(ctx->stream), "nb_force");
+    return NB_OK;
+}
+
+int nb_force_crackle(nb_ctx* ctx, double* crackle)
+{
+    if (!ctx || !crackle) return NB_EINVAL;
+    if (ctx->order != 8 || ctx->forced_n < 0) return NB_ESTATE;
+    const int rc = copy_out(ctx, crackle, ctx->L.fc, 3 * (size_t)ctx->forced_n);
+    if (rc != NB_OK) return rc;
+    if (!ctx->on_device) CU(cudaStreamSynchronize(ctx->stream), "nb_force_crackle");
     return NB_OK;
 }
 
@@ -369,7 +381,7 @@ static int field_width_host(int f) { return (f == NB_M || f == NB_T || f == NB_D
 
 int nb_get_state(nb_ctx* ctx, int field, const int32_t* idx, int64_t n, double* out)
 {
-    if (!ctx || !out || n < 0 || n > ctx->N || field < NB_M || field > NB_AP) return NB_EINVAL;
+    if (!ctx || !out || n < 0 || n > ctx->N || field < NB_M || field > NB_JP) return NB_EINVAL;
     if (n == 0) return NB_OK;
     const int32_t* didx = nullptr;
     const int rc = resolve_idx(ctx, idx, n, ctx->L.idx_tmp, &didx);
@@ -387,7 +399,7 @@ int nb_get_state(nb_ctx* ctx, int field, const int32_t* idx, int64_t n, double* 
 
 int nb_set_state(nb_ctx* ctx, int field, const int32_t* idx, int64_t n, const double* in)
 {
-    if (!ctx || !in || n < 0 || n > ctx->N || field < NB_M || field > NB_DT) return NB_EINVAL;
+    if (!ctx || !in || n < 0 || n > ctx->N || field < NB_M || (field > NB_DT && field != NB_A4 && field != NB_A5)) return NB_EINVAL;
     if (n == 0) return NB_OK;
     const int32_t* didx = nullptr;
     const int rc = resolve_idx(ctx, idx, n, ctx->L.idx_tmp, &didx);

@@ -23,9 +23,9 @@ namespace {
 // ---------------------------------------------------------------------------------------------
 // One pair.  53 FP64-pipe instructions (32 DFMA + 11 DMUL + 10 DADD) + 1 MUFU.RSQ64H.
 // ---------------------------------------------------------------------------------------------
-struct Sums { double ax, ay, az, jx, jy, jz, sx, sy, sz, p; };
+struct Sums { double ax, ay, az, jx, jy, jz, sx, sy, sz, p, cx, cy, cz; };   // cx..cz: crackle, 8th order only
 
-struct IPart { double x, y, z, vx, vy, vz, ax, ay, az; };
+struct IPart { double x, y, z, vx, vy, vz, ax, ay, az, jx, jy, jz; };        // jx..jz: predicted jerk, 8th order only
 
 // fp64 reciprocal-square-root seed: MUFU.RSQ64H works on the high word only (about 20 good bits).
 __device__ __forceinline__ double rsqrt_seed(double s)
@@ -332,26 +332,82 @@ __device__ __forceinline__ void pair2_o4(const IPart& pi, const JRec (&J)[2], co
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// 8th-order variant (R22): crackle added.  With T3 = 3 dv.da + dx.dj and
+// gamma = T3/s + alpha (3 beta - 4 alpha^2):  crackle term = q (dj - 9 alpha w - 9 beta u - 3 gamma dx).
+// 84 FP64-pipe instructions per pair + 1 MUFU.RSQ64H; one pair at a time (ptxas schedules it; 2 x 12 differences would
+// not fit the register budget).
+// ---------------------------------------------------------------------------------------------
+template <bool EPS0, bool MASK = true>
+__device__ __forceinline__ void pair_o8(const IPart& pi, const double4 p0, const double4 p1, const double2 p2, const double4 p3,
+                                        const double eps2, const bool self, Sums& S)
+{
+    const double dx = p0.x - pi.x, dy = p0.y - pi.y, dz = p0.z - pi.z;
+    const double dvx = p1.x - pi.vx, dvy = p1.y - pi.vy, dvz = p1.z - pi.vz;
+    const double dax = p1.w - pi.ax, day = p2.x - pi.ay, daz = p2.y - pi.az;
+    const double djx = p3.x - pi.jx, djy = p3.y - pi.jy, djz = p3.z - pi.jz;
+    double s = F(dx, dx, F(dy, dy, F(dz, dz, eps2)));
+    if (EPS0 && MASK) s = self ? 1.0 : s;
+    const double y0 = rsqrt_seed(s);
+    const double e = F(-s, M(y0, y0), 1.0);
+    const double y = F(M(y0, e), F(e, 0.375, 0.5), y0);
+    const double rv = F(dx, dvx, F(dy, dvy, M(dz, dvz)));
+    double B = M(dvz, dvz);
+    B = F(dz, daz, B); B = F(dvy, dvy, B); B = F(dy, day, B); B = F(dvx, dvx, B); B = F(dx, dax, B);
+    const double va = F(dvx, dax, F(dvy, day, M(dvz, daz)));
+    const double xj = F(dx, djx, F(dy, djy, M(dz, djz)));
+    const double T3 = F(va, 3.0, xj);
+    const double yy = M(y, y);
+    const double z = M(yy, -3.0);
+    const double mr = M(y, p0.w);
+    const double q = M(yy, mr);
+    const double alpha = M(yy, rv);
+    const double c1 = M(z, rv);                          // -3 alpha
+    const double c3 = F(c1, alpha, M(z, B));             // -3 beta
+    const double c2 = twice(c1);                         // -6 alpha
+    const double g3 = F(alpha, F(c3, 3.0, M(M(alpha, alpha), 12.0)), M(z, T3));   // -3 gamma = z T3 + alpha (-9 beta + 12 alpha^2)
+    const double c9a = M(c1, 3.0), c9b = M(c3, 3.0);     // -9 alpha, -9 beta
+    const double ux = F(c1, dx, dvx), uy = F(c1, dy, dvy), uz = F(c1, dz, dvz);
+    double wx = F(c3, dx, dax), wy = F(c3, dy, day), wz = F(c3, dz, daz);
+    wx = F(c2, ux, wx); wy = F(c2, uy, wy); wz = F(c2, uz, wz);
+    double kx = F(g3, dx, djx), ky = F(g3, dy, djy), kz = F(g3, dz, djz);
+    kx = F(c9b, ux, kx); ky = F(c9b, uy, ky); kz = F(c9b, uz, kz);
+    kx = F(c9a, wx, kx); ky = F(c9a, wy, ky); kz = F(c9a, wz, kz);
+    S.ax = F(q, dx, S.ax); S.ay = F(q, dy, S.ay); S.az = F(q, dz, S.az);
+    S.jx = F(q, ux, S.jx); S.jy = F(q, uy, S.jy); S.jz = F(q, uz, S.jz);
+    S.sx = F(q, wx, S.sx); S.sy = F(q, wy, S.sy); S.sz = F(q, wz, S.sz);
+    S.cx = F(q, kx, S.cx); S.cy = F(q, ky, S.cy); S.cz = F(q, kz, S.cz);
+    S.p += (MASK && self) ? 0.0 : mr;
+}
+
+template <int ORDER>
 __device__ __forceinline__ IPart load_ipart(const ForceArgs& A, int i)
 {
     const double4 a = A.pj0[i], b = A.pj1[i];
     const double2 c = A.pj2[i];
-    return IPart{a.x, a.y, a.z, b.x, b.y, b.z, b.w, c.x, c.y};
+    IPart p{a.x, a.y, a.z, b.x, b.y, b.z, b.w, c.x, c.y, 0.0, 0.0, 0.0};
+    if (ORDER == 8) { const double4 d = A.pj3[i]; p.jx = d.x; p.jy = d.y; p.jz = d.z; }
+    return p;
 }
 
+// partial planes are [plane][NC][ld] with NC = 10 (a, jerk, snap, pot), 13 at the 8th order (+ crackle)
+template <int ORDER>
 __device__ __forceinline__ void store_sums(const ForceArgs& A, int slice, int k, bool valid, const Sums& S)
 {
+    constexpr int NC = ORDER == 8 ? 13 : 10;
     if (A.n_planes > 1) {
-        double* P = A.partial + (size_t)slice * 10 * A.ld + k;      // plane (slice, c) is contiguous in k
+        double* P = A.partial + (size_t)slice * NC * A.ld + k;      // plane (slice, c) is contiguous in k
         const size_t ld = A.ld;
         P[0] = S.ax; P[ld] = S.ay; P[2 * ld] = S.az;
         P[3 * ld] = S.jx; P[4 * ld] = S.jy; P[5 * ld] = S.jz;
         P[6 * ld] = S.sx; P[7 * ld] = S.sy; P[8 * ld] = S.sz; P[9 * ld] = S.p;
+        if (ORDER == 8) { P[10 * ld] = S.cx; P[11 * ld] = S.cy; P[12 * ld] = S.cz; }
     } else if (valid) {
         A.out_a[3 * k] = S.ax; A.out_a[3 * k + 1] = S.ay; A.out_a[3 * k + 2] = S.az;
         A.out_j[3 * k] = S.jx; A.out_j[3 * k + 1] = S.jy; A.out_j[3 * k + 2] = S.jz;
         A.out_s[3 * k] = S.sx; A.out_s[3 * k + 1] = S.sy; A.out_s[3 * k + 2] = S.sz;
         A.out_p[k] = -S.p;
+        if (ORDER == 8) { A.out_c[3 * k] = S.cx; A.out_c[3 * k + 1] = S.cy; A.out_c[3 * k + 2] = S.cz; }
     }
 }
 
@@ -423,6 +479,7 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
     __shared__ alignas(128) double4 s0[LI_STAGES][LI_TJ];
     __shared__ alignas(128) double4 s1[LI_STAGES][LI_TJ];
     __shared__ alignas(128) double2 s2[LI_STAGES][LI_TJ];
+    __shared__ alignas(128) double4 s3[LI_STAGES][ORDER == 8 ? LI_TJ : 1];   // predicted jerk, 8th order only
     __shared__ alignas(8) unsigned long long full[LI_STAGES];
     __shared__ int next_item;
 
@@ -439,10 +496,11 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
     auto stage_tile = [&](int tile, int st) {
         const uint32_t bar = smem_u32(&full[st]);
         const size_t j0 = (size_t)tile * LI_TJ;
-        mbar_expect_tx(bar, LI_TJ * 80);
+        mbar_expect_tx(bar, LI_TJ * (ORDER == 8 ? 112 : 80));
         bulk_g2s(smem_u32(&s0[st][0]), A.pj0 + j0, LI_TJ * 32, bar);
         bulk_g2s(smem_u32(&s1[st][0]), A.pj1 + j0, LI_TJ * 32, bar);
         bulk_g2s(smem_u32(&s2[st][0]), A.pj2 + j0, LI_TJ * 16, bar);
+        if (ORDER == 8) bulk_g2s(smem_u32(&s3[st][0]), A.pj3 + j0, LI_TJ * 32, bar);
     };
 
     uint32_t uses = 0;   // j-tiles this CTA has consumed so far: stage = uses % STAGES, parity = (uses / STAGES) & 1
@@ -469,8 +527,8 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
             valid[q] = k < A.n_act;
             const int kk = valid[q] ? k : 0;
             ii[q] = A.idx ? A.idx[kk] : kk;
-            pi[q] = load_ipart(A, ii[q]);
-            acc[q] = Sums{0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+            pi[q] = load_ipart<ORDER>(A, ii[q]);
+            acc[q] = Sums{0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
         }
 
         for (int t = 0; t < nt; ++t) {
@@ -485,7 +543,23 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
             for (int q = 0; q < LI_I; ++q) own |= (unsigned)(ii[q] - jbase) < (unsigned)TJW;
             const double4 *t0p = &s0[st][wg * TJW], *t1p = &s1[st][wg * TJW];
             const double2* t2p = &s2[st][wg * TJW];
-            if (__any_sync(0xffffffffu, own)) {
+            if (ORDER == 8) {
+                const double4* t3p = &s3[st][ORDER == 8 ? wg * TJW : 0];
+                if (__any_sync(0xffffffffu, own)) {
+#pragma unroll 2
+                    for (int jj = 0; jj < TJW; ++jj) {
+#pragma unroll
+                        for (int q = 0; q < LI_I; ++q)
+                            pair_o8<EPS0, true>(pi[q], t0p[jj], t1p[jj], t2p[jj], t3p[jj], A.eps2, jbase + jj == ii[q], acc[q]);
+                    }
+                } else {
+#pragma unroll 2
+                    for (int jj = 0; jj < TJW; ++jj) {
+#pragma unroll
+                        for (int q = 0; q < LI_I; ++q) pair_o8<EPS0, false>(pi[q], t0p[jj], t1p[jj], t2p[jj], t3p[jj], A.eps2, false, acc[q]);
+                    }
+                }
+            } else if (__any_sync(0xffffffffu, own)) {
 #pragma unroll 1
                 for (int jj = 0; jj < TJW; jj += 2) {
                     const JRec J[2] = {{t0p[jj], t1p[jj], t2p[jj]}, {t0p[jj + 1], t1p[jj + 1], t2p[jj + 1]}};
@@ -514,7 +588,7 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
         uses += nt;
 
 #pragma unroll
-        for (int q = 0; q < LI_I; ++q) store_sums(A, slice * W + wg, unit * UNIT + q * LI_THREADS + til, valid[q], acc[q]);
+        for (int q = 0; q < LI_I; ++q) store_sums<ORDER>(A, slice * W + wg, unit * UNIT + q * LI_THREADS + til, valid[q], acc[q]);
     }
     if (tid == 0) queue_retire(A.queue, gridDim.x);
 }
@@ -530,7 +604,7 @@ __device__ __forceinline__ double warp_sum(double v)
 }
 
 template <bool EPS0, int ORDER>
-__global__ void __launch_bounds__(LJ_THREADS, LJ_CTAS_PER_SM) force_lj_kernel(const ForceArgs A_)
+__global__ void __launch_bounds__(LJ_THREADS, ORDER == 8 ? 1 : LJ_CTAS_PER_SM) force_lj_kernel(const ForceArgs A_)
 {
     ForceArgs A = A_;
     if (!take_devplan(A, 1)) return;
@@ -554,20 +628,25 @@ __global__ void __launch_bounds__(LJ_THREADS, LJ_CTAS_PER_SM) force_lj_kernel(co
             valid[q] = k < A.n_act;
             const int kk = valid[q] ? k : 0;
             ii[q] = A.idx ? A.idx[kk] : kk;
-            pi[q] = load_ipart(A, ii[q]);
-            acc[q] = Sums{0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+            pi[q] = load_ipart<ORDER>(A, ii[q]);
+            acc[q] = Sums{0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
         }
 
         int j = t0 * LJ_TJ + lane;
         double4 n0 = A.pj0[j], n1 = A.pj1[j];
         double2 n2 = A.pj2[j];
+        double4 n3 = ORDER == 8 ? A.pj3[j] : make_double4(0, 0, 0, 0);
         for (int t = 0; t < nt; ++t) {
-            const double4 p0 = n0, p1 = n1;
+            const double4 p0 = n0, p1 = n1, p3 = n3;
             const double2 p2 = n2;
-            if (t + 1 < nt) { n0 = A.pj0[j + LJ_TJ]; n1 = A.pj1[j + LJ_TJ]; n2 = A.pj2[j + LJ_TJ]; }   // prefetch
+            if (t + 1 < nt) {                                                                            // prefetch
+                n0 = A.pj0[j + LJ_TJ]; n1 = A.pj1[j + LJ_TJ]; n2 = A.pj2[j + LJ_TJ];
+                if (ORDER == 8) n3 = A.pj3[j + LJ_TJ];
+            }
 #pragma unroll
             for (int q = 0; q < LJ_I; ++q) {
                 if (ORDER == 4) pair_o4<EPS0>(pi[q], p0, p1, A.eps2, j == ii[q], acc[q]);
+                else if (ORDER == 8) pair_o8<EPS0>(pi[q], p0, p1, p2, p3, A.eps2, j == ii[q], acc[q]);
                 else pair<EPS0>(pi[q], p0, p1, p2, A.eps2, j == ii[q], acc[q]);
             }
             j += LJ_TJ;
@@ -580,7 +659,8 @@ __global__ void __launch_bounds__(LJ_THREADS, LJ_CTAS_PER_SM) force_lj_kernel(co
             S.jx = warp_sum(S.jx); S.jy = warp_sum(S.jy); S.jz = warp_sum(S.jz);
             S.sx = warp_sum(S.sx); S.sy = warp_sum(S.sy); S.sz = warp_sum(S.sz);
             S.p = warp_sum(S.p);
-            if (lane == 0) store_sums(A, slice, unit * LJ_I + q, valid[q], S);
+            if (ORDER == 8) { S.cx = warp_sum(S.cx); S.cy = warp_sum(S.cy); S.cz = warp_sum(S.cz); }
+            if (lane == 0) store_sums<ORDER>(A, slice, unit * LJ_I + q, valid[q], S);
         }
     }
     if (lane == 0) queue_retire(A.queue, gridDim.x * LJ_WARPS);
@@ -592,9 +672,10 @@ __global__ void __launch_bounds__(LJ_THREADS, LJ_CTAS_PER_SM) force_lj_kernel(co
 // tree in shared memory.  The order depends only on (S, T): bitwise reproducible.  T = 1 is the plain loop over
 // slices (large active sets, few slices: the loads of neighbouring threads coalesce over k).
 // ---------------------------------------------------------------------------------------------
+template <int NC>
 __global__ void __launch_bounds__(RED_THREADS) reduce_partials_kernel(const ForceArgs A_, int T)
 {
-    __shared__ double sm[10][RED_THREADS];
+    __shared__ double sm[NC][RED_THREADS];
     ForceArgs A = A_;
     if (A.dp) {                                            // device-planned: any kernel shape, T from the plan
         if (A.dp->stop) return;
@@ -605,26 +686,26 @@ __global__ void __launch_bounds__(RED_THREADS) reduce_partials_kernel(const Forc
     const int kl = threadIdx.x % R, lane = threadIdx.x / R;
     for (int k0 = blockIdx.x * R; k0 < A.n_act; k0 += gridDim.x * R) {      // uniform over the block
         const int k = k0 + kl;
-        double r[10];
+        double r[NC];
 #pragma unroll
-        for (int c = 0; c < 10; ++c) r[c] = 0.0;
+        for (int c = 0; c < NC; ++c) r[c] = 0.0;
         if (k < A.n_act) {
-            const size_t plane = (size_t)10 * A.ld;
+            const size_t plane = (size_t)NC * A.ld;
             const double* P = A.partial + (size_t)lane * plane + k;
             for (int s = lane; s < A.n_planes; s += T, P += (size_t)T * plane) {
 #pragma unroll
-                for (int c = 0; c < 10; ++c) r[c] += P[(size_t)c * A.ld];
+                for (int c = 0; c < NC; ++c) r[c] += P[(size_t)c * A.ld];
             }
         }
         for (int off = T >> 1; off > 0; off >>= 1) {
             if (lane >= off && lane < 2 * off) {
 #pragma unroll
-                for (int c = 0; c < 10; ++c) sm[c][threadIdx.x] = r[c];
+                for (int c = 0; c < NC; ++c) sm[c][threadIdx.x] = r[c];
             }
             __syncthreads();
             if (lane < off) {
 #pragma unroll
-                for (int c = 0; c < 10; ++c) r[c] += sm[c][threadIdx.x + off * R];
+                for (int c = 0; c < NC; ++c) r[c] += sm[c][threadIdx.x + off * R];
             }
             __syncthreads();
         }
@@ -633,6 +714,7 @@ __global__ void __launch_bounds__(RED_THREADS) reduce_partials_kernel(const Forc
         A.out_j[3 * k] = r[3]; A.out_j[3 * k + 1] = r[4]; A.out_j[3 * k + 2] = r[5];
         A.out_s[3 * k] = r[6]; A.out_s[3 * k + 1] = r[7]; A.out_s[3 * k + 2] = r[8];
         A.out_p[k] = -r[9];
+        if (NC == 13) { A.out_c[3 * k] = r[10]; A.out_c[3 * k + 1] = r[11]; A.out_c[3 * k + 2] = r[12]; }
     }
 }
 
@@ -641,8 +723,9 @@ __global__ void __launch_bounds__(RED_THREADS) reduce_partials_kernel(const Forc
 // kernel instantiation for (eps == 0, order)
 #define NB_DISPATCH(CALL)                                               \
     do {                                                                \
-        if (order == 4) { if (eps_is_zero) { CALL(true, 4); } else { CALL(false, 4); } } \
-        else            { if (eps_is_zero) { CALL(true, 6); } else { CALL(false, 6); } } \
+        if (order == 4)      { if (eps_is_zero) { CALL(true, 4); } else { CALL(false, 4); } } \
+        else if (order == 8) { if (eps_is_zero) { CALL(true, 8); } else { CALL(false, 8); } } \
+        else                 { if (eps_is_zero) { CALL(true, 6); } else { CALL(false, 6); } } \
     } while (0)
 
 cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps_is_zero, int order, cudaStream_t st, int* launches)
@@ -662,7 +745,8 @@ cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps
     if (args.n_planes > 1) {
         const int T = nb_reduce_threads(args.n_act, args.n_planes);
         const int R = RED_THREADS / T;
-        reduce_partials_kernel<<<(args.n_act + R - 1) / R, RED_THREADS, 0, st>>>(args, T);
+        if (order == 8) reduce_partials_kernel<13><<<(args.n_act + R - 1) / R, RED_THREADS, 0, st>>>(args, T);
+        else reduce_partials_kernel<10><<<(args.n_act + R - 1) / R, RED_THREADS, 0, st>>>(args, T);
         ++*launches;
         e = cudaGetLastError();
     }
@@ -680,7 +764,8 @@ cudaError_t nb_launch_force_devplan(const ForceArgs& args_, bool eps_is_zero, in
     force_li_kernel<E, 1, O><<<g_li, LI_THREADS, 0, st>>>(args)
     NB_DISPATCH(ALL3);
 #undef ALL3
-    reduce_partials_kernel<<<n_sm * 4, RED_THREADS, 0, st>>>(args, 1);
+    if (order == 8) reduce_partials_kernel<13><<<n_sm * 4, RED_THREADS, 0, st>>>(args, 1);
+    else reduce_partials_kernel<10><<<n_sm * 4, RED_THREADS, 0, st>>>(args, 1);
     *launches += 4;
     return cudaGetLastError();
 }

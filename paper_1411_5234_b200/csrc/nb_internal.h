@@ -56,6 +56,7 @@ struct DevPlan;   // nb_plan.h
 
 struct ForceArgs {
     const double4* pj0; const double4* pj1; const double2* pj2;   // predicted records (padded)
+    const double4* pj3;      // predicted jerk (8th order only)
     const int32_t* idx;      // active indices or nullptr (i = k)
     int n_act;
     int n_units;             // i-tiles (LI) or warp i-groups (LJ)
@@ -70,6 +71,7 @@ struct ForceArgs {
     const DevPlan* dp;       // non-null: the launch was planned on the device (nb_run_blocks); overrides the plan fields above
     int* queue;              // work queue: [0] next item, [1] finished CTAs (both 0 between launches)
     double* out_a; double* out_j; double* out_s; double* out_p;   // [n_act][3] x3, [n_act]
+    double* out_c;           // crackle [n_act][3] (8th order only)
 };
 
 // nb_force.cu
@@ -79,7 +81,13 @@ cudaError_t nb_launch_force_devplan(const ForceArgs& args, bool eps_is_zero, int
 void nb_force_occupancy(int* li_ctas_per_sm, int* lj_ctas_per_sm);
 
 // nb_step.cu
-struct StateArrays { double4 *st0, *st1, *st2, *st3, *st4; double* dt; double4 *pj0, *pj1; double2* pj2; int order; /* 4 or 6 */ };
+struct StateArrays {
+    double4 *st0, *st1, *st2, *st3, *st4; double* dt; double4 *pj0, *pj1; double2* pj2;
+    double4 *st5, *st6;   // 8th order: st5 = (a4x, a4y, a4z, a5x), st6 = (a5y, a5z, -, -), a4 = d4a/dt4, a5 = d5a/dt5
+    double4* pj3;         // 8th order: predicted jerk (jxp, jyp, jzp, -)
+    const double* fc;     // 8th order: crackle of the last evaluation, row k <-> active_idx[k]
+    int order;            // 4, 6 or 8
+};
 cudaError_t nb_launch_init_state(const StateArrays& s, int64_t N, int64_t Npad, const double* m, const double* x, const double* v, cudaStream_t st);
 cudaError_t nb_launch_predict(const StateArrays& s, int64_t N, double t, bool own_time, cudaStream_t st);
 cudaError_t nb_launch_startup(const StateArrays& s, int64_t N, const double* fa, const double* fj, const double* fs, int pass,

@@ -15,6 +15,7 @@ __device__ __forceinline__ void write_pad_record(const StateArrays& s, int64_t i
     s.pj0[i] = make_double4(3e33, 3e33, 3e33, 0.0);
     s.pj1[i] = make_double4(0.0, 0.0, 0.0, 0.0);
     s.pj2[i] = make_double2(0.0, 0.0);
+    s.pj3[i] = make_double4(0.0, 0.0, 0.0, 0.0);
 }
 
 // ------------------------------------------------------------------ init: AoS inputs -> packed state
@@ -33,7 +34,7 @@ __global__ void init_state_kernel(StateArrays s, int64_t N, int64_t Npad, const 
         s.dt[i] = 1e300;
         write_pad_record(s, i);
     }
-    s.st2[i] = zero; s.st3[i] = zero; s.st4[i] = zero;
+    s.st2[i] = zero; s.st3[i] = zero; s.st4[i] = zero; s.st5[i] = zero; s.st6[i] = zero;
 }
 
 // ------------------------------------------------------------------ a1: predictor (reading R6)
@@ -52,7 +53,20 @@ __global__ void __launch_bounds__(TPB) predict_kernel(StateArrays s, int64_t N, 
     const double x[3] = {p.x, p.y, p.z}, v[3] = {q.x, q.y, q.z}, a[3] = {r.x, r.y, r.z};
     const double j[3] = {r.w, u.x, u.y}, sn[3] = {u.z, u.w, w.x}, c[3] = {w.y, w.z, w.w};
     double xp[3], vp[3], ap[3];
-    if (s.order == 4) {                                    // 4th-order variant (R21): x to the jerk term, v to D^2/2 jerk
+    if (s.order == 8) {                                    // 8th-order variant (R22): two more terms, and the predicted jerk
+        const double4 g = s.st5[i], hq = s.st6[i];
+        const double a4[3] = {g.x, g.y, g.z}, a5[3] = {g.w, hq.x, hq.y};
+        const double D6 = D * (1.0 / 6.0), D7 = D * (1.0 / 7.0);
+        double jp[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            xp[k] = fma(D, fma(D2, fma(D3, fma(D4, fma(D5, fma(D6, fma(D7, a5[k], a4[k]), c[k]), sn[k]), j[k]), a[k]), v[k]), x[k]);
+            vp[k] = fma(D, fma(D2, fma(D3, fma(D4, fma(D5, fma(D6, a5[k], a4[k]), c[k]), sn[k]), j[k]), a[k]), v[k]);
+            ap[k] = fma(D, fma(D2, fma(D3, fma(D4, fma(D5, a5[k], a4[k]), c[k]), sn[k]), j[k]), a[k]);
+            jp[k] = fma(D, fma(D2, fma(D3, fma(D4, a5[k], a4[k]), c[k]), sn[k]), j[k]);
+        }
+        s.pj3[i] = make_double4(jp[0], jp[1], jp[2], 0.0);
+    } else if (s.order == 4) {                                    // 4th-order variant (R21): x to the jerk term, v to D^2/2 jerk
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
             xp[k] = fma(D, fma(D2, fma(D3, j[k], a[k]), v[k]), x[k]);
@@ -104,7 +118,8 @@ __global__ void startup_kernel(StateArrays s, int64_t N, const double* fa, const
     const double sx = o4 ? 0.0 : fs[3 * i], sy = o4 ? 0.0 : fs[3 * i + 1], sz = o4 ? 0.0 : fs[3 * i + 2];
     s.st2[i] = make_double4(ax, ay, az, jx);
     s.st3[i] = make_double4(jy, jz, sx, sy);
-    s.st4[i] = make_double4(sz, 0.0, 0.0, 0.0);
+    const bool c8 = s.order == 8 && pass == 3;              // 8th order: the third pass (a and jerk known) gives crackle
+    s.st4[i] = make_double4(sz, c8 ? s.fc[3 * i] : 0.0, c8 ? s.fc[3 * i + 1] : 0.0, c8 ? s.fc[3 * i + 2] : 0.0);
     const double r = eta_s * norm3(ax, ay, az) / norm3(jx, jy, jz);
     int k;
     if (!(r < INFINITY)) k = k_max;
@@ -125,6 +140,54 @@ __device__ __forceinline__ void corrector_one(const StateArrays& s, const int32_
     const double hh = 0.5 * h;
     const double x0[3] = {p.x, p.y, p.z}, v0[3] = {q.x, q.y, q.z};
     const double a0[3] = {r.x, r.y, r.z}, j0[3] = {r.w, u.x, u.y}, s0[3] = {u.z, u.w, w.x};
+    if (s.order == 8) {
+        // 8th-order variant (R22): septic Hermite quadrature; d4a/dt4 .. d7a/dt7 at the end of the step from the interpolant
+        const double c0[3] = {w.y, w.z, w.w};
+        double a1[3], j1[3], s1[3], c1[3], x1[3], v1[3], d4[3], d5[3], d6[3], d7[3];
+        const double h2 = h * h, h3 = h2 * h, h4 = h3 * h;
+        const double ihh = 1.0 / hh, ihh2 = ihh * ihh, ihh4 = ihh2 * ihh2;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            a1[c] = fa[3 * k + c]; j1[c] = fj[3 * k + c]; s1[c] = fs[3 * k + c]; c1[c] = s.fc[3 * k + c];
+            v1[c] = v0[c] + hh * (a1[c] + a0[c]) - h2 * (3.0 / 28.0) * (j1[c] - j0[c]) + h3 * (1.0 / 84.0) * (s1[c] + s0[c])
+                    - h4 * (1.0 / 1680.0) * (c1[c] - c0[c]);
+            x1[c] = x0[c] + hh * (v1[c] + v0[c]) - h2 * (3.0 / 28.0) * (a1[c] - a0[c]) + h3 * (1.0 / 84.0) * (j1[c] + j0[c])
+                    - h4 * (1.0 / 1680.0) * (s1[c] - s0[c]);
+            const double Am = a1[c] - a0[c];
+            const double Jp = hh * (j1[c] + j0[c]), Jm = hh * (j1[c] - j0[c]);
+            const double Sp = hh * hh * (s1[c] + s0[c]), Sm = hh * hh * (s1[c] - s0[c]);
+            const double Cp = hh * hh * hh * (c1[c] + c0[c]), Cm = hh * hh * hh * (c1[c] - c0[c]);
+            d4[c] = (0.5 * (-105.0 * Am + 105.0 * Jp + 15.0 * Jm - 45.0 * Sm - 15.0 * Sp) + 5.0 * Cp + 3.0 * Cm) * ihh4;
+            d5[c] = (-315.0 * Am + 315.0 * Jp + 0.5 * (45.0 * Jm - 255.0 * Sm - 45.0 * Sp + 45.0 * Cp + 15.0 * Cm)) * (ihh4 * ihh);
+            d6[c] = (0.5 * (-1575.0 * Am + 1575.0 * Jp + 45.0 * Jm - 45.0 * Sp + 105.0 * Cp + 15.0 * Cm) - 315.0 * Sm) * (ihh4 * ihh2);
+            d7[c] = (0.5 * (-1575.0 * Am + 1575.0 * Jp + 105.0 * Cp) - 315.0 * Sm) * (ihh4 * ihh2 * ihh);
+        }
+        s.st0[i] = make_double4(x1[0], x1[1], x1[2], p.w);
+        s.st1[i] = make_double4(v1[0], v1[1], v1[2], t_new);
+        s.st2[i] = make_double4(a1[0], a1[1], a1[2], j1[0]);
+        s.st3[i] = make_double4(j1[1], j1[2], s1[0], s1[1]);
+        s.st4[i] = make_double4(s1[2], c1[0], c1[1], c1[2]);
+        s.st5[i] = make_double4(d4[0], d4[1], d4[2], d5[0]);
+        s.st6[i] = make_double4(d5[1], d5[2], 0.0, 0.0);
+        if (dt_shared > 0.0) { s.dt[i] = dt_shared; return; }
+        // dt_crit = eta (A1/A6)^(1/5); level = floor(log2 dt_crit) = floor(ilogb(dt_crit^5)/5) (eta3 carries eta^5 for this order)
+        const double n0 = norm3(a1[0], a1[1], a1[2]), n1 = norm3(j1[0], j1[1], j1[2]), n2 = norm3(s1[0], s1[1], s1[2]);
+        const double n5 = norm3(d5[0], d5[1], d5[2]), n6 = norm3(d6[0], d6[1], d6[2]), n7 = norm3(d7[0], d7[1], d7[2]);
+        const double r5 = eta3 * (sqrt(fma(n0, n2, n1 * n1)) / sqrt(fma(n5, n7, n6 * n6)));
+        int k_crit;
+        if (!(r5 < INFINITY)) k_crit = k_max;
+        else if (!(r5 > 0.0)) k_crit = k_min;
+        else { const int e5 = ilog2_pos(r5); k_crit = clampi(e5 >= 0 ? e5 / 5 : -((-e5 + 4) / 5), k_min, k_max); }
+        const int k_old = ilog2_pos(dt_old);
+        int k_new = k_old;
+        if (k_crit < k_old) k_new = k_crit;
+        else if (k_crit > k_old && k_old < k_max) {
+            const double mm = scalbn(t_new, -(k_old + 1));
+            if (mm == rint(mm)) k_new = k_old + 1;
+        }
+        s.dt[i] = scalbn(1.0, k_new);
+        return;
+    }
     if (s.order == 4) {
         // 4th-order variant (R21): cubic Hermite quadrature; d2a/dt2 at the end of the step and d3a/dt3 from the interpolant
         double a1[3], j1[3], x1[3], v1[3], d2[3], d3[3];
@@ -246,6 +309,9 @@ __global__ void get_kernel(StateArrays s, int field, const int32_t* idx, int64_t
         case NB_XP: { double4 p = s.pj0[i]; a = p.x; b = p.y; c = p.z; } break;
         case NB_VP: { double4 p = s.pj1[i]; a = p.x; b = p.y; c = p.z; } break;
         case NB_AP: { double4 p = s.pj1[i]; double2 q = s.pj2[i]; a = p.w; b = q.x; c = q.y; } break;
+        case NB_A4: { double4 p = s.st5[i]; a = p.x; b = p.y; c = p.z; } break;
+        case NB_A5: { double4 p = s.st5[i], q = s.st6[i]; a = p.w; b = q.x; c = q.y; } break;
+        case NB_JP: { double4 p = s.pj3[i]; a = p.x; b = p.y; c = p.z; } break;
     }
     if (field_width(field) == 1) out[k] = a;
     else { out[3 * k] = a; out[3 * k + 1] = b; out[3 * k + 2] = c; }
@@ -268,6 +334,8 @@ __global__ void set_kernel(StateArrays s, int field, const int32_t* idx, int64_t
         case NB_J: s.st2[i].w = a; s.st3[i].x = b; s.st3[i].y = c; break;
         case NB_S: s.st3[i].z = a; s.st3[i].w = b; s.st4[i].x = c; break;
         case NB_C: s.st4[i].y = a; s.st4[i].z = b; s.st4[i].w = c; break;
+        case NB_A4: s.st5[i].x = a; s.st5[i].y = b; s.st5[i].z = c; break;
+        case NB_A5: s.st5[i].w = a; s.st6[i].x = b; s.st6[i].y = c; break;
     }
 }
 
@@ -514,8 +582,8 @@ cudaError_t nb_launch_corrector(const StateArrays& s, const int32_t* idx, int64_
                                 const double* fa, const double* fj, const double* fs, double eta, int k_min, int k_max,
                                 cudaStream_t st)
 {
-    corrector_kernel<<<nblocks(n_act), TPB, 0, st>>>(s, idx, n_act, dt_shared, t_new, fa, fj, fs, s.order == 4 ? eta : eta * eta * eta, k_min, k_max,
-                                                     nullptr, nullptr);
+    corrector_kernel<<<nblocks(n_act), TPB, 0, st>>>(s, idx, n_act, dt_shared, t_new, fa, fj, fs, s.order == 4 ? eta : s.order == 8 ? eta * eta * eta * eta * eta : eta * eta * eta,
+                                                     k_min, k_max, nullptr, nullptr);
     return cudaGetLastError();
 }
 
@@ -569,7 +637,8 @@ cudaError_t nb_launch_devstep_head(const StateArrays& s, int64_t N, int64_t Npad
 cudaError_t nb_launch_devstep_tail(const StateArrays& s, int n_sm, const int32_t* active, void* scratch, DevPlan* dp, const double* fa,
                                    const double* fj, const double* fs, double eta, int k_min, int k_max, cudaStream_t st, int* launches)
 {
-    corrector_kernel<<<n_sm * 8, TPB, 0, st>>>(s, active, 0, 0.0, 0.0, fa, fj, fs, s.order == 4 ? eta : eta * eta * eta, k_min, k_max, dp,
+    corrector_kernel<<<n_sm * 8, TPB, 0, st>>>(s, active, 0, 0.0, 0.0, fa, fj, fs,
+                                               s.order == 4 ? eta : s.order == 8 ? eta * eta * eta * eta * eta : eta * eta * eta, k_min, k_max, dp,
                                                (unsigned long long*)scratch);
     *launches += 1;
     return cudaGetLastError();

@@ -479,5 +479,83 @@ def test_order4_force_steps_and_block_steps(B, oracle):
 
 def test_order_is_validated(B):
     m, x, v = W.plummer(64, 1)
-    with pytest.raises(B.NBError):
-        B.System(m, x, v, 1e-3, order=8)
+    for bad in (2, 5, 10):
+        with pytest.raises(B.NBError):
+            B.System(m, x, v, 1e-3, order=bad)
+
+
+# ------------------------------------------------------------------ 8th-order variant (nb_config.order = 8; R22)
+def test_order8_force_steps_and_block_steps(B, oracle):
+    N, eps = 1500, 1e-3
+    m, x, v = W.plummer(N, 8008, "kroupa")
+    g = B.System(m, x, v, eps, order=8)
+    o = oracle.OracleSystem(m, x, v, eps, order=8)
+    # three-pass startup: a, jerk, snap, crackle; a4 = a5 = 0; same levels
+    for f, ref in (("A", o.a), ("J", o.j), ("S", o.s), ("C", o.c)):
+        assert relvec(g.nb_get_state(f), ref).max() <= TOL, f
+    assert not g.nb_get_state("A4").any() and not g.nb_get_state("A5").any()
+    assert np.array_equal(g.nb_get_state("DT"), o.dt)
+    dt = 2.0 ** -8
+    rng = np.random.default_rng(88)
+    for step in range(1, 5):
+        g.nb_predict(step * dt); o.predict(step * dt)
+        # after the first step a4, a5 enter the predictor; they are 4th / 5th differences over the step, so a force
+        # difference delta is amplified by ~105/hh^4, 315/hh^5 (hh = dt/2) whatever the implementation: with D = dt the
+        # predicted jerk inherits ~200 delta |a| / hh, the predicted acceleration ~100 delta |a|
+        tols = (1e-12, 1e-12, 1e-12, 1e-12) if step == 1 else (1e-12, 1e-11, 1e-9, None)
+        for (f, ref), tol in zip((("XP", o.xp), ("VP", o.vp), ("AP", o.ap), ("JP", o.jp)), tols):
+            if tol is not None:
+                assert relvec(g.nb_get_state(f), ref).max() <= tol, (f, step)
+            else:
+                bound = 1e-11 * 200 * (np.linalg.norm(o.a, axis=-1) + dt * np.linalg.norm(o.j, axis=-1)) / (dt / 2)
+                assert np.all(np.linalg.norm(g.nb_get_state(f) - ref, axis=-1) <= bound), (f, step)
+        if step == 3:                                    # all three kernel shapes on identical records
+            mm = g.nb_get_state("M")
+            rec = [g.nb_get_state(f) for f in ("XP", "VP", "AP", "JP")]
+            for n_act in (1, 7, 16, 17, 64, 96, 97, 300):
+                idx = rng.choice(N, n_act, replace=False).astype(np.int32)
+                ga, gj, gs, gp = g.nb_force(idx)
+                gc = g.nb_force_crackle(n_act)
+                oa, oj, os_, oc, op = oracle.hermite6.force8(mm, *rec, eps, idx)
+                assert_force_parity((ga, gj, gs, gp), (oa, oj, os_, op))
+                assert relvec(gc, oc).max() <= TOL, ("crackle", n_act, relvec(gc, oc).max())
+        ga, gj, gs, gp = g.nb_force()
+        gc = g.nb_force_crackle(N)
+        oa, oj, os_, op, oc = o.force()
+        assert_force_parity((ga, gj, gs, gp), (oa, oj, os_, op), 1e-9)     # states differ at round-off after a step
+        assert relvec(gc, oc).max() <= 1e-8
+        g.nb_corrector(None, dt); o.corrector(None, dt)
+    for f, ref, tol in (("X", o.x, 1e-13), ("V", o.v, 1e-12), ("A", o.a, 1e-9), ("C", o.c, 1e-8)):
+        assert relvec(g.nb_get_state(f), ref).max() <= tol, f
+    # a4, a5 are fourth / fifth differences over the step: a relative force difference delta is amplified by ~105/hh^4, 315/hh^5
+    nrm = lambda q: np.linalg.norm(q, axis=-1)
+    hh, delta = dt / 2, 1e-9
+    scale = nrm(o.a) + hh * nrm(o.j) + hh ** 2 * nrm(o.s) + hh ** 3 * nrm(o.c)
+    assert np.all(nrm(g.nb_get_state("A4") - o.a4) <= delta * 400 * scale / hh ** 4)
+    assert np.all(nrm(g.nb_get_state("A5") - o.a5) <= delta * 1200 * scale / hh ** 5)
+    Kg, Wg = g.nb_energy(); Ko, Wo = o.energy()
+    assert abs((Kg + Wg) - (Ko + Wo)) / abs(Ko + Wo) < 1e-10
+    g.nb_free()
+    # block steps: same schedule on both sides, then nb_run_blocks bit-identical to the separate calls
+    N = 384
+    m, x, v = W.plummer(N, 8009, "kroupa")
+    g, g2 = B.System(m, x, v, eps, order=8), B.System(m, x, v, eps, order=8)
+    o = oracle.OracleSystem(m, x, v, eps, order=8)
+    steps = 0
+    while True:
+        tg, ng, actg = g.nb_next_block()
+        to, acto = o.next_block()
+        assert tg == to and np.array_equal(actg, acto)
+        if to > 2.0 ** -5:
+            break
+        g.nb_predict(tg); g.nb_force(actg, outputs=False); g.nb_corrector(actg, 0.0)
+        o.predict(to); o.force(acto); o.corrector(acto, 0.0)
+        assert np.array_equal(g.nb_get_state("DT"), o.dt)
+        steps += 1
+    assert steps > 20
+    assert relvec(g.nb_get_state("X"), o.x).max() <= 1e-12
+    s2, t2, _ = g2.nb_run_blocks(2.0 ** -5)
+    assert s2 == steps and t2 == 2.0 ** -5
+    for f in ("X", "V", "A", "J", "S", "C", "A4", "A5", "T", "DT"):
+        assert np.array_equal(g.nb_get_state(f), g2.nb_get_state(f)), f
+    g.nb_free(); g2.nb_free()
