@@ -20,7 +20,9 @@
  * mpmath brute force + differentiation on N = 2, 3, Newton's third law, finite differences
  * along the Taylor trajectory, polynomial exactness of predictor/corrector, Kepler orbit
  * 6th-order convergence, time-step criterion on the circular binary, energy conservation,
- * Plummer mean field.  Unpinned: the VALUES of eta, eta_s (parameters).
+ * Plummer mean field; for the 4th- and 8th-order variants (R21, R22) their own polynomial-exactness,
+ * Kepler-convergence, criterion and (8th) 50-digit crackle pins.  Unpinned: the VALUES of eta, eta_s
+ * (parameters).
  */
 #include <math.h>
 #include <stdint.h>
