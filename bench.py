@@ -262,7 +262,7 @@ def run_ours(args, cfg_dict):
     pipe_probe = B.nb_probe_dfma_sources(sm_max_mhz, local)   # cycles per DFMA: 2 / 3 / 3-with-reuse register sources
     f_ms = float(np.mean(force_ms))
     achieved = FLOP_EXEC * inter_per_step / (f_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "force_li_kernel<false, 1> (+ reduce_partials_kernel)", "achieved": achieved,
+    roofline = {"bound": "alu", "kernel": "force_li_kernel<false, 1, 6> (+ reduce_partials_kernel<10>)", "achieved": achieved,
                 "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
                 "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max_mhz:.0f} MHz (DESIGN.md)",
                 "peak_measured_dfma": peak_measured, "frac_of_measured_dfma": achieved / peak_measured,

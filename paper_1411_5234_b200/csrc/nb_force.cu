@@ -1,15 +1,18 @@
 // nb_force.cu — the pairwise evaluation: acceleration, jerk, snap and
 // potential of eq. (1)-(2) and their time derivatives (R3), for
 // the active particles against all N predicted j-records.  fp64 on the FP64 ALU pipe; tensor cores
-// are not used (no dense contraction).  Two kernel shapes, both writing per-slice partial sums
-// that a third kernel adds in slice order (the "Bfactor" j-split of PAPER.md:59-65, made
-// deterministic):
-//   force_li_kernel  lanes-over-i: a thread owns LI_I active particles in registers; the CTA
+// are not used (no dense contraction).  Kernel shapes, all writing per-slice partial sums that a
+// reduction kernel adds in a fixed order (the "Bfactor" j-split of PAPER.md:59-65, made deterministic):
+//   force_li_kernel<EPS0, W, ORDER>  lanes-over-i: a thread owns one active particle in registers; the CTA
 //                    streams j-tiles into shared memory with 1-D TMA bulk copies (UBLKCP) signalled
 //                    on mbarriers, double-buffered; every lane reads the same j-record (broadcast LDS).
-//   force_lj_kernel  lanes-over-j: a warp owns LJ_I active particles (same in every lane); its 32
-//                    lanes read 32 different j-records straight from global memory (coalesced) and
-//                    the ten sums per particle are combined with a warp-shuffle butterfly.
+//                    W = 1: i-tiles of 128 particles.  W = 4 (17..96 active): i-tiles of 32, the four warps
+//                    take different parts of each j-tile.
+//   force_lj_kernel<EPS0, ORDER>  lanes-over-j (<= 16 active): a warp owns one active particle (same in every
+//                    lane); its 32 lanes read 32 different j-records straight from global memory (coalesced)
+//                    and the sums are combined with a warp-shuffle butterfly.
+// ORDER = 6 is the scheme of the north star (a, jerk, snap, pot); 4 (a, jerk, pot) and 8 (+ crackle) are the other
+// Hermite orders the paper names (R21, R22).
 // Work items (i-unit, j-slice) are handed out by an atomic queue, not by a static stride: warps of
 // co-resident CTAs do NOT get equal shares of the FP64 pipe (measured: of three CTAs with equal work on
 // one SM the first finished after 40 % of the time the last one needed), so a static partition ends in a
@@ -21,7 +24,8 @@
 namespace {
 
 // ---------------------------------------------------------------------------------------------
-// One pair.  53 FP64-pipe instructions (32 DFMA + 11 DMUL + 10 DADD) + 1 MUFU.RSQ64H.
+// One pair, 6th order.  53 FP64-pipe instructions (32 DFMA + 11 DMUL + 10 DADD) + 1 MUFU.RSQ64H.  Used by the
+// lanes-over-j kernel; the lanes-over-i kernel uses pair2 below.
 // ---------------------------------------------------------------------------------------------
 struct Sums { double ax, ay, az, jx, jy, jz, sx, sy, sz, p, cx, cy, cz; };   // cx..cz: crackle, 8th order only
 
