@@ -559,3 +559,36 @@ def test_order8_force_steps_and_block_steps(B, oracle):
     for f in ("X", "V", "A", "J", "S", "C", "A4", "A5", "T", "DT"):
         assert np.array_equal(g.nb_get_state(f), g2.nb_get_state(f)), f
     g.nb_free(); g2.nb_free()
+
+
+@pytest.mark.parametrize("order", [4, 8])
+@pytest.mark.parametrize("N,eps", [(2, 0.0), (257, 0.0), (1, 1e-3), (300, 1e-2)])
+def test_other_orders_edge_sizes(B, oracle, order, N, eps):
+    """Degenerate and ragged sizes at the 4th and 8th order: N = 1 (no pairs: all sums 0), N = 2 unsoftened, a ragged
+    N with eps = 0 (index-masked self pair), a permuted full list, an empty active set."""
+    m, x, v = W.plummer(max(N, 2), 900 + N + order, "kroupa")
+    m, x, v = m[:N].copy(), x[:N].copy(), v[:N].copy()
+    g = B.System(m, x, v, eps, order=order)
+    g.nb_predict(2.0 ** -10)
+    assert g.nb_force(np.zeros(0, dtype=np.int32))[0].shape == (0, 3)        # n_act = 0 is a no-op
+    rng = np.random.default_rng(N)
+    perm = rng.permutation(N).astype(np.int32)
+    ga, gj, gs, gp = g.nb_force(perm)
+    mm = g.nb_get_state("M")
+    rec = [g.nb_get_state(f) for f in ("XP", "VP", "AP")]
+    if N == 1:
+        assert not ga.any() and not gj.any() and not gs.any() and not gp.any()
+        g.nb_free()
+        return
+    if order == 8:
+        gc = g.nb_force_crackle(N)
+        oa, oj, os_, oc, op = oracle.hermite6.force8(mm, *rec, g.nb_get_state("JP"), eps, perm)
+        assert_force_parity((ga, gj, gs, gp), (oa, oj, os_, op))
+        assert relvec(gc, oc).max() <= TOL
+    else:
+        oa, oj, _, op = oracle.hermite6.force(mm, *rec, eps, perm)
+        assert relvec(ga, oa).max() <= TOL and relvec(gj, oj).max() <= TOL and np.abs(gp / op - 1).max() <= TOL
+        assert not gs.any()
+    g.nb_corrector(perm, 2.0 ** -10)
+    assert np.all(g.nb_get_state("T") == 2.0 ** -10) and np.isfinite(g.nb_get_state("X")).all()
+    g.nb_free()
