@@ -14,7 +14,8 @@
 
 constexpr int NB_PAD = 256;          // particle arrays are padded to a multiple of this
 
-// Both force kernels keep ONE active particle per thread (lanes-over-i) or per warp (lanes-over-j).  The
+// The force kernels keep one active particle per thread (lanes-over-i) or two per warp (lanes-over-j: every j-record
+// loaded from L2 serves both, measured 20 % faster for 8-16 active particles at N = 2^20, 128 registers).  The
 // lanes-over-i kernel evaluates two j-records at a time with a fixed instruction order (pair2, nb_force.cu): 112
 // registers, 16 warps (4 per scheduler) per SM as 4 CTAs of 128 threads; CTA shapes that leave the four
 // schedulers with unequal warp counts (5 x 96, 3 x 160) measured 15-27 % slower.
@@ -45,9 +46,15 @@ constexpr int LI_W = LI_THREADS / 32;        // small active sets: the CTA's war
 // lanes-over-j kernel: each warp owns LJ_I active particles, lanes take different j
 constexpr int LJ_THREADS = 256;
 constexpr int LJ_WARPS = LJ_THREADS / 32;
-constexpr int LJ_I = 1;
+#ifndef NB_LJ_I
+#define NB_LJ_I 2
+#endif
+#ifndef NB_LJ_CTAS_PER_SM
+#define NB_LJ_CTAS_PER_SM 2
+#endif
+constexpr int LJ_I = NB_LJ_I;
 constexpr int LJ_TJ = 32;                    // j-records per warp iteration
-constexpr int LJ_CTAS_PER_SM = 3;
+constexpr int LJ_CTAS_PER_SM = NB_LJ_CTAS_PER_SM;
 constexpr int64_t LJ_MAX_ACT = 16;           // n_act <= this -> lanes-over-j
 constexpr int RED_THREADS = 256;             // threads per block of the partial-sum reduction
 constexpr int64_t LIW_MAX_ACT = 96;          // n_act <= this -> lanes-over-i with 32-particle units (above, a 128-lane i-tile is >= 75 % full)

@@ -52,7 +52,7 @@ def test_plan_invariants(B, N):
             p = B.nb_plan_force(N, n_act, n_sm)
             Npad = (N + 255) // 256 * 256
             assert p.kernel == (1 if n_act <= 16 else 2 if n_act <= 96 else 0)
-            assert p.sub == (4 if p.kernel == 2 else 1) and p.unit == (1 if p.kernel == 1 else 128 // p.sub)
+            assert p.sub == (4 if p.kernel == 2 else 1) and p.unit == (2 if p.kernel == 1 else 128 // p.sub)
             unit, n_tiles = p.unit, Npad // p.tile
             assert unit >= 1 and Npad % p.tile == 0 and p.n_units == (n_act + unit - 1) // unit
             assert 1 <= p.ctas_per_sm <= 32 and p.grid <= n_sm * p.ctas_per_sm
@@ -61,7 +61,7 @@ def test_plan_invariants(B, N):
             assert S * st >= n_tiles and (S - 1) * st < n_tiles            # slices cover all j-tiles, none empty
             assert S * p.sub * p.n_units * unit <= 8 * Npad + (1 << 19)    # partial-sum buffer capacity
             # small active sets are split so that the device is filled
-            resident = n_sm * p.ctas_per_sm * (8 if p.kernel == 1 else 1)
+            resident = n_sm * p.ctas_per_sm * (8 if p.kernel == 1 else 1)       # lanes-over-j: 8 warps per CTA
             if p.n_units < resident and n_tiles >= 16 * resident:
                 assert p.n_units * S >= 0.5 * resident
 
