@@ -592,3 +592,25 @@ def test_other_orders_edge_sizes(B, oracle, order, N, eps):
     g.nb_corrector(perm, 2.0 ** -10)
     assert np.all(g.nb_get_state("T") == 2.0 ** -10) and np.isfinite(g.nb_get_state("X")).all()
     g.nb_free()
+
+
+def test_max_split_and_probes(B, oracle):
+    """nb_set_max_split(1) (the "Bfactor off" arm of the Fig. 1 sweep) changes the launch, not the result beyond the
+    summation order; the operand-source probes return the pipe model's 2 / 3 / 2-3 cycles."""
+    N, eps = 5000, 1e-3
+    m, x, v = W.plummer(N, 606)
+    g = B.System(m, x, v, eps)
+    g.nb_predict(2.0 ** -9)
+    for n_act in (3, 40, 700, N):
+        idx = None if n_act == N else np.random.default_rng(n_act).choice(N, n_act, replace=False).astype(np.int32)
+        g.nb_set_max_split(0); split = g.nb_force(idx)
+        g.nb_set_max_split(1); nosplit = g.nb_force(idx)
+        ref = oracle_on_gpu_records(oracle, g, eps, idx)
+        assert_force_parity(split, ref); assert_force_parity(nosplit, ref)
+    g.nb_set_max_split(0)
+    with pytest.raises(B.NBError):
+        g.nb_set_max_split(-1)
+    g.nb_free()
+    cyc = B.nb_probe_dfma_sources(1965.0)
+    assert 1.9 < cyc["two_sources"] < 2.4 and 2.8 < cyc["three_sources"] < 3.5
+    assert cyc["two_sources"] <= cyc["three_sources_one_reused"] <= cyc["three_sources"]
