@@ -1,7 +1,7 @@
 """BASELINE.json configs[2]: the block-time-step run (N = 262144 Plummer sphere, Kroupa-like masses, eps = 1e-4,
 levels 2^-3 .. 2^-20 by the Aarseth criterion, 1/8 time unit), advanced with nb_run_blocks.
 
-    python -m paper_1411_5234_b200.config3 [--N 262144] [--t-end 0.125] [--order 6] [--profile-steps 1500]
+    python -m paper_1411_5234_b200.config3 [--N 262144] [--t-end 0.125] [--order 6] [--eta 0] [--profile-steps 1500]
 
 Prints the run's totals (block steps, interactions, wall time, energy drift) and, from a second stretch driven one
 step at a time, the device time per block step by active-set size.  PAPER.md:58 (block time steps)
@@ -24,13 +24,14 @@ def main():
     ap.add_argument("--t-end", type=float, default=0.125)
     ap.add_argument("--order", type=int, default=6)
     ap.add_argument("--profile-steps", type=int, default=1500)
+    ap.add_argument("--eta", type=float, default=0.0, help="accuracy parameter of the time-step criterion (0: the order's default)")
     a = ap.parse_args()
     import torch
     c, m, x, v = W.config_inputs(3, N=a.N)
     N = m.shape[0]
     dev = "cuda:0"
     g = B.System(torch.tensor(m, device=dev), torch.tensor(x, device=dev), torch.tensor(v, device=dev), c.eps,
-                 host=False, device=0, order=a.order)
+                 host=False, device=0, order=a.order, eta=a.eta)
     K0, W0 = g.nb_energy()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
@@ -39,7 +40,7 @@ def main():
     el = time.perf_counter() - t0
     K1, W1 = g.nb_energy()
     inter = sum_act * (N - 1)
-    print(f"N = {N}, order {a.order}, eps = {c.eps}: {steps} block steps to t = {t_last}, {sum_act / N:.1f} steps per particle, "
+    print(f"N = {N}, order {a.order}, eta = {a.eta or 'default'}, eps = {c.eps}: {steps} block steps to t = {t_last}, {sum_act / N:.1f} steps per particle, "
           f"{inter:.4e} interactions in {el:.3f} s = {inter / el:.4e} interactions/s; dE/E = {(K1 + W1) / (K0 + W0) - 1:.3e}")
     if a.profile_steps <= 0:
         return
