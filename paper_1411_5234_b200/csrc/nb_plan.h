@@ -54,16 +54,24 @@ NB_HD PlanShape nb_plan_shape(int64_t Npad, int64_t n_act, int n_sm, int64_t max
 
 // Cost of splitting into S slices, in units of one j-tile of work on one work slot (a negative value: S leaves a
 // slice empty and is not a candidate).  Work items (unit, slice) are pulled from a queue by `resident` workers (CTAs
-// or warps); an item costs slice_tiles + fixed.  Up to four rounds the last round is counted whole; beyond that the
-// queue balances the workers up to a tail of about one item.
+// or warps); an item costs slice_tiles + fixed.
+// Lanes-over-i with 128-particle tiles (kernel 0): co-resident CTAs do not get equal shares of the FP64 pipe, so a
+// single round of equal items ends with the slow CTA of every SM running alone (measured 0.78 of the issue bound
+// against 0.86 with ten rounds): one round counts 1.5, more rounds items / resident + 0.9 for the tail.
+// The other shapes (tiny active sets, latency-bound): up to four rounds the last round is counted whole; beyond that
+// the queue balances the workers up to a tail of about 0.7 items.
 NB_HD double nb_split_cost(const PlanShape& p, int64_t S, int64_t* slice_tiles)
 {
     const int64_t st = (p.n_tiles + S - 1) / S;
     *slice_tiles = st;
     if ((p.n_tiles + st - 1) / st != S) return -1.0;
     const int64_t items = p.n_units * S;
-    const double rounds = items <= 4 * p.resident ? (double)((items + p.resident - 1) / p.resident)
-                                                  : (double)items / (double)p.resident + 0.7;
+    double rounds;
+    if (p.kernel == 0)
+        rounds = items <= p.resident ? 1.5 : (double)items / (double)p.resident + 0.9;
+    else
+        rounds = items <= 4 * p.resident ? (double)((items + p.resident - 1) / p.resident)
+                                         : (double)items / (double)p.resident + 0.7;
     return rounds * (double)(st + p.fixed);
 }
 
