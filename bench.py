@@ -258,8 +258,9 @@ def run_ours(args, cfg_dict):
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
     sm_max_mhz = float(peaks.get("sm_max_mhz") or (clocks or {}).get("sm_max_mhz") or 1965.0)
     peak_nominal = n_sm * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12       # TFLOP/s, all-FMA
-    peak_measured, _ = B.nb_probe_fp64_peak(1.0, local)
-    pipe_probe = B.nb_probe_dfma_sources(sm_max_mhz, local)   # cycles per DFMA: 2 / 3 / 3-with-reuse register sources
+    from paper_1411_5234_b200 import probes as P          # libnbprobe.so: measurement aids, not part of libnb.so
+    peak_measured, _ = P.fp64_peak(1.0, local)
+    pipe_probe = P.dfma_sources(sm_max_mhz, local)            # cycles per DFMA: 2 / 3 / 3-with-reuse register sources
     f_ms = float(np.mean(force_ms))
     achieved = FLOP_EXEC * inter_per_step / (f_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "force_li_kernel<false, 1, 6> (+ reduce_partials_kernel<10>)", "achieved": achieved,

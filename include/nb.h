@@ -39,7 +39,8 @@ typedef struct nb_ctx nb_ctx; /* opaque: one particle system on one GPU */
 
 typedef enum {
     NB_OK = 0,
-    NB_EINVAL = -1, /* bad argument: N < 1, eps < 0, NULL where not allowed, n_act out of range, bad level range */
+    NB_EINVAL = -1, /* bad argument: N < 1, eps < 0, NULL where not allowed, n_act out of range, bad level range; with index
+                       checking on (nb_config.check_indices): an index outside [0, N) or a duplicate in an index list */
     NB_ENOMEM = -2, /* workspace missing, misaligned (< 256 B) or smaller than nb_workspace_bytes(N) */
     NB_ESTATE = -3, /* call order: nb_force without nb_predict since the last state change, nb_corrector without nb_force */
     NB_ECUDA = -4   /* a CUDA runtime call or kernel failed; nb_last_error(ctx) holds the CUDA message */
@@ -60,7 +61,14 @@ typedef struct {
                                quadrature and the criterion dt = eta A1/A2;
                                8 = the 8th-order variant (reading R22): nb_force also evaluates crackle = d3a/dt3 (read it with
                                nb_force_crackle), the predictor runs to d5a/dt5 and predicts the jerk, nb_corrector is the
-                               septic Hermite quadrature, criterion dt = eta (A1/A6)^(1/5), eta -> 0.75, three startup passes. */
+                               septic Hermite quadrature, criterion dt = eta (A1/A6)^(1/5), eta -> 0.75, two startup passes. */
+    int check_indices;      /* index lists passed to nb_force / nb_corrector / nb_get_state / nb_set_state (the
+                               m <= N active particles) are verified on the device before use: every index in [0, N), and no
+                               duplicates (nb_get_state allows duplicates).  A bad list returns NB_EINVAL and nothing is
+                               launched on it.  The check reads one flag back, so it synchronises the stream.
+                               0 = default: on for host-pointer contexts (those calls synchronise anyway), off for
+                               device-pointer contexts (calls stay asynchronous; indices are then the caller's contract);
+                               1 = always on; -1 = always off. */
 } nb_config;
 
 /* Selectors of nb_get_state / nb_set_state.  Width = doubles per particle. */
@@ -197,23 +205,11 @@ int nb_set_state(nb_ctx* ctx, int field, const int32_t* idx, int64_t n, const do
 int nb_energy(nb_ctx* ctx, double* kinetic, double* potential);
 
 /*
- * nb_probe_fp64_peak — measurement aid: runs a register-resident chain of independent FP64 FMAs on
- * every SM for about `seconds` and returns the sustained rate in TFLOP/s (FMA = 2 flop).  This is the
- * measured denominator of the "fraction of FP64 peak" that bench.py reports.  workspace: >= 64 KiB
- * of device memory.
+ * nb_check_indices — verify an index list (h/d) the way nb_config.check_indices does, on demand: NB_OK if all n
+ * indices are in [0, N) and (unique != 0) pairwise different, NB_EINVAL otherwise (also for n > N: no call takes a
+ * longer list).  Synchronises the stream.  n == 0 is NB_OK.  (the active subset, m <= N.)
  */
-int nb_probe_fp64_peak(int device, void* stream, void* workspace, size_t workspace_bytes,
-                       double seconds, double* tflops, int* n_sm);
-
-/*
- * nb_probe_dfma_sources — measurement aid: cycles one warp-wide DFMA holds the FP64 pipe of an SM
- * sub-partition, from a stream of independent DFMAs whose sources are (kind 0) one register and two
- * constants, (kind 1) three different registers, (kind 2) three registers of which one is shared by
- * the whole run, so that the operand-reuse cache can supply it.  sm_mhz: the SM clock to convert with.
- * These are the numbers behind the pipe model of DESIGN.md section 6.  workspace: >= 64 KiB, device.
- */
-int nb_probe_dfma_sources(int device, void* stream, void* workspace, size_t workspace_bytes, int kind,
-                          double sm_mhz, double* cycles);
+int nb_check_indices(nb_ctx* ctx, const int32_t* idx, int64_t n, int unique);
 
 /* Kernel launches issued by this context so far (what bench.py reports as gpu_launches). */
 int64_t nb_launch_count(const nb_ctx* ctx);

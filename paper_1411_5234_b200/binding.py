@@ -21,14 +21,15 @@ _WIDTH = {0: 1, 7: 1, 8: 1}
 ACTIVE_INTERNAL = C.c_void_p(1)
 
 EXPORTS = ["nb_workspace_bytes", "nb_plan_force", "nb_set_max_split", "nb_init", "nb_predict", "nb_force", "nb_force_crackle", "nb_corrector",
-           "nb_next_block", "nb_run_blocks", "nb_get_state", "nb_set_state", "nb_energy", "nb_probe_fp64_peak", "nb_probe_dfma_sources",
+           "nb_next_block", "nb_run_blocks", "nb_get_state", "nb_set_state", "nb_energy", "nb_check_indices",
            "nb_launch_count", "nb_last_force_ms", "nb_strerror", "nb_last_error", "nb_free"]
 
 
 class nb_config(C.Structure):
     _fields_ = [("device", C.c_int), ("stream", C.c_void_p), ("workspace", C.c_void_p),
                 ("workspace_bytes", C.c_size_t), ("ptrs_on_device", C.c_int),
-                ("eta", C.c_double), ("eta_s", C.c_double), ("k_min", C.c_int), ("k_max", C.c_int), ("order", C.c_int)]
+                ("eta", C.c_double), ("eta_s", C.c_double), ("k_min", C.c_int), ("k_max", C.c_int), ("order", C.c_int),
+                ("check_indices", C.c_int)]
 
 
 class nb_plan(C.Structure):
@@ -69,10 +70,7 @@ def lib() -> C.CDLL:
     L.nb_get_state.argtypes = [vp, C.c_int, vp, i64, vp]; L.nb_get_state.restype = C.c_int
     L.nb_set_state.argtypes = [vp, C.c_int, vp, i64, vp]; L.nb_set_state.restype = C.c_int
     L.nb_energy.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl)]; L.nb_energy.restype = C.c_int
-    L.nb_probe_fp64_peak.argtypes = [C.c_int, vp, vp, C.c_size_t, dbl, C.POINTER(dbl), C.POINTER(C.c_int)]
-    L.nb_probe_fp64_peak.restype = C.c_int
-    L.nb_probe_dfma_sources.argtypes = [C.c_int, vp, vp, C.c_size_t, C.c_int, dbl, C.POINTER(dbl)]
-    L.nb_probe_dfma_sources.restype = C.c_int
+    L.nb_check_indices.argtypes = [vp, vp, i64, C.c_int]; L.nb_check_indices.restype = C.c_int
     L.nb_launch_count.argtypes = [vp]; L.nb_launch_count.restype = i64
     L.nb_last_force_ms.argtypes = [vp]; L.nb_last_force_ms.restype = dbl
     L.nb_strerror.argtypes = [C.c_int]; L.nb_strerror.restype = C.c_char_p
@@ -114,7 +112,8 @@ class System:
     host=False: array arguments are torch CUDA tensors (DEVICE pointers; calls are asynchronous).
     """
 
-    def __init__(self, m, x, v, eps, host=True, device=0, eta=0.0, eta_s=0.0, k_min=0, k_max=0, stream=None, order=0):
+    def __init__(self, m, x, v, eps, host=True, device=0, eta=0.0, eta_s=0.0, k_min=0, k_max=0, stream=None, order=0,
+                 check_indices=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1411_5234_b200 needs a CUDA device; there is no CPU fallback")
@@ -130,7 +129,7 @@ class System:
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=f"cuda:{device}")
         base = (self.workspace.data_ptr() + 255) // 256 * 256
         self.cfg = nb_config(device, C.c_void_p(self.stream.cuda_stream), C.c_void_p(base), nbytes,
-                             0 if host else 1, eta, eta_s, k_min, k_max, order)
+                             0 if host else 1, eta, eta_s, k_min, k_max, order, check_indices)
         m, x, v = self._in(m, (self.N,)), self._in(x, (self.N, 3)), self._in(v, (self.N, 3))
         self._check(self.L.nb_init(C.byref(self.ctx), self.N, _ptr(m), _ptr(x), _ptr(v), float(eps), C.byref(self.cfg)))
 
@@ -238,6 +237,11 @@ class System:
         self._check(self.L.nb_energy(self.ctx, C.byref(k), C.byref(w)))
         return k.value, w.value
 
+    def nb_check_indices(self, idx, unique=True):
+        """NB_OK (0) or NB_EINVAL (-1): the status itself, not an exception."""
+        idx = self._in(idx, dtype=np.int32)
+        return self.L.nb_check_indices(self.ctx, _ptr(idx), int(idx.shape[0]), 1 if unique else 0)
+
     def nb_launch_count(self):
         return self.L.nb_launch_count(self.ctx)
 
@@ -254,34 +258,3 @@ class System:
             self.nb_free()
         except Exception:
             pass
-
-
-def nb_probe_fp64_peak(seconds=1.0, device=0):
-    """Sustained FP64 FMA rate of the device in TFLOP/s (FMA = 2 flop) and its SM count."""
-    import torch
-    torch.cuda.set_device(device)
-    ws = torch.empty(65536 + 256, dtype=torch.uint8, device=f"cuda:{device}")
-    base = (ws.data_ptr() + 255) // 256 * 256
-    tf, nsm = C.c_double(), C.c_int()
-    rc = lib().nb_probe_fp64_peak(device, C.c_void_p(torch.cuda.current_stream(device).cuda_stream), C.c_void_p(base), 65536,
-                                  float(seconds), C.byref(tf), C.byref(nsm))
-    if rc != NB_OK:
-        raise NBError(rc, lib().nb_strerror(rc).decode())
-    return tf.value, nsm.value
-
-
-def nb_probe_dfma_sources(sm_mhz, device=0):
-    """Cycles per warp-wide DFMA and SM sub-partition for 2-source, 3-source and 3-source-with-reuse streams."""
-    import torch
-    torch.cuda.set_device(device)
-    ws = torch.empty(65536 + 256, dtype=torch.uint8, device=f"cuda:{device}")
-    base = (ws.data_ptr() + 255) // 256 * 256
-    out = {}
-    for kind, name in enumerate(("two_sources", "three_sources", "three_sources_one_reused")):
-        cyc = C.c_double()
-        rc = lib().nb_probe_dfma_sources(device, C.c_void_p(torch.cuda.current_stream(device).cuda_stream), C.c_void_p(base), 65536,
-                                         kind, float(sm_mhz), C.byref(cyc))
-        if rc != NB_OK:
-            raise NBError(rc, lib().nb_strerror(rc).decode())
-        out[name] = cyc.value
-    return out

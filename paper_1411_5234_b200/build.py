@@ -1,9 +1,10 @@
-"""Build libnb.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
+"""Build libnb.so (the product) and libnbprobe.so (measurement aids) in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
     python -m paper_1411_5234_b200.build [--force]
 """
 from __future__ import annotations
 
+import glob
 import os
 import subprocess
 import sys
@@ -12,8 +13,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnb.so")
+PROBE_LIB = os.path.join(HERE, "libnbprobe.so")          # measurement aids (csrc/nb_probe.h), loaded by bench.py only
 SOURCES = ["nb_api.cu", "nb_force.cu", "nb_step.cu"]
-HEADERS = [os.path.join(CSRC, "nb_internal.h"), os.path.join(ROOT, "include", "nb.h")]
+PROBE_SOURCES = ["nb_probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I" + os.path.join(ROOT, "include")]
 
@@ -25,12 +27,19 @@ def _nvcc() -> str:
     return "nvcc"
 
 
+def _headers():
+    return glob.glob(os.path.join(CSRC, "*.h")) + glob.glob(os.path.join(ROOT, "include", "*.h"))
+
+
 def stale() -> bool:
-    if not os.path.exists(LIB):
-        return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES] + HEADERS
-    return any(os.path.getmtime(d) > t for d in deps)
+    """True if a library is missing or older than any source or header (every csrc/*.h and include/*.h counts)."""
+    for lib, sources in ((LIB, SOURCES), (PROBE_LIB, PROBE_SOURCES)):
+        if not os.path.exists(lib):
+            return True
+        t = os.path.getmtime(lib)
+        if any(os.path.getmtime(d) > t for d in [os.path.join(CSRC, s) for s in sources] + _headers()):
+            return True
+    return False
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -38,20 +47,21 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
-    objs = []
-    procs = []
-    for s in SOURCES:
+    procs, objs = [], {}
+    for s in SOURCES + PROBE_SOURCES:
         o = os.path.join(objdir, s.replace(".cu", ".o"))
         cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, s), "-o", o]
         procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
-        objs.append(o)
+        objs[s] = o
     for cmd, p in procs:
         out, _ = p.communicate()
         if verbose or p.returncode != 0:
             sys.stderr.write(out)
         if p.returncode != 0:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
-    subprocess.run([_nvcc(), "-shared", "-o", LIB] + objs + ["-gencode", "arch=compute_100a,code=sm_100a"], check=True)
+    arch = ["-gencode", "arch=compute_100a,code=sm_100a"]
+    subprocess.run([_nvcc(), "-shared", "-o", LIB] + [objs[s] for s in SOURCES] + arch, check=True)
+    subprocess.run([_nvcc(), "-shared", "-o", PROBE_LIB] + [objs[s] for s in PROBE_SOURCES] + arch, check=True)
     return LIB
 
 

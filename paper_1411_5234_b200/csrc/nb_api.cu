@@ -2,6 +2,8 @@
 // checks.  No arithmetic of the method lives here; every step runs in the kernels of nb_force.cu
 // and nb_step.cu.
 #include <algorithm>
+#include <cfloat>
+#include <climits>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -33,6 +35,7 @@ struct Layout {
     int32_t *idx_user, *idx_sched, *idx_tmp;
     double* stage;                      // staging for host <-> device transfers, 10 doubles per particle
     char* scratch;
+    uint32_t* idx_bitmap;               // one bit per particle + one flag word: index-list verification (nb_config.check_indices)
     int* queue;                         // work queue of the force kernels (2 counters)
     DevPlan* devplan;                   // plan and counters of the device-planned block steps (nb_run_blocks)
     size_t bytes;
@@ -49,6 +52,7 @@ struct Layout {
         idx_user = c.take<int32_t>(Npad); idx_sched = c.take<int32_t>(Npad); idx_tmp = c.take<int32_t>(Npad);
         stage = c.take<double>(10 * Npad);
         scratch = c.take<char>(scratch_bytes(Npad));
+        idx_bitmap = c.take<uint32_t>(Npad / 32 + 64);      // [Npad/32] bits, then the flag word
         queue = c.take<int>(64);
         devplan = c.take<DevPlan>(1);
         bytes = c.off;
@@ -61,6 +65,7 @@ struct nb_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
     bool on_device = false;
+    bool check_idx = false;        // verify user index lists before use (nb_config.check_indices)
     int64_t N = 0, Npad = 0;
     double eps = 0, eta = 0.45, eta_s = 0.01;
     int k_min = -20, k_max = -3;
@@ -88,12 +93,33 @@ int fail_cuda(nb_ctx* c, cudaError_t e, const char* where)
 }
 #define CU(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail_cuda(ctx, e_, where); } while (0)
 
+// Every entry point that touches the device runs with the context's device current and puts the caller's device back
+// on return: a process that holds contexts on several GPUs (or whose framework switched devices) stays correct.
+struct DeviceGuard {
+    int prev = -1;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int device)
+    {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != device) err = cudaSetDevice(device);
+        else if (err == cudaSuccess) prev = -1;             // nothing to restore
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+#define ON_DEVICE(ctx) DeviceGuard guard_((ctx)->device); if (guard_.err != cudaSuccess) return fail_cuda(ctx, guard_.err, "cudaSetDevice")
+
+// The kernels see eps^2 only.  For 0 < eps < ~1.5e-154 it underflows to 0 or a denormal (flushed by the ftz rsqrt seed),
+// so such an eps is treated as what it computes as: eps = 0, self pair masked by index.
+inline bool eps2_is_zero(double eps) { return !(eps * eps >= DBL_MIN); }
+
 // the fields of ForceArgs that do not depend on the plan
 ForceArgs base_force_args(const nb_ctx* ctx)
 {
     ForceArgs A{};
     A.pj0 = ctx->L.s.pj0; A.pj1 = ctx->L.s.pj1; A.pj2 = ctx->L.s.pj2; A.pj3 = ctx->L.s.pj3;
-    A.eps2 = ctx->eps * ctx->eps;
+    A.eps2 = eps2_is_zero(ctx->eps) ? 0.0 : ctx->eps * ctx->eps;
     A.partial = ctx->L.partial;
     A.queue = ctx->L.queue;                                 // zeroed by nb_init, left at 0 by every launch
     A.out_a = ctx->L.fa; A.out_j = ctx->L.fj; A.out_s = ctx->L.fs; A.out_p = ctx->L.fp; A.out_c = ctx->L.fc;
@@ -117,7 +143,7 @@ int build_step_graph(nb_ctx* ctx)
         A.n_tiles = 0;                                      // set per kernel below
         A.dp = ctx->L.devplan;
         e = nb_launch_devstep_head(ctx->L.s, ctx->N, ctx->Npad, ctx->n_sm, ctx->L.idx_sched, ctx->L.scratch, ctx->L.devplan, cs, &launches);
-        if (e == cudaSuccess) e = nb_launch_force_devplan(A, ctx->eps == 0.0, ctx->order, ctx->n_sm, (int)ctx->Npad, cs, &launches);
+        if (e == cudaSuccess) e = nb_launch_force_devplan(A, eps2_is_zero(ctx->eps), ctx->order, ctx->n_sm, (int)ctx->Npad, cs, &launches);
         if (e == cudaSuccess)
             e = nb_launch_devstep_tail(ctx->L.s, ctx->n_sm, ctx->L.idx_sched, ctx->L.scratch, ctx->L.devplan, ctx->L.fa, ctx->L.fj, ctx->L.fs,
                                        ctx->eta, ctx->k_min, ctx->k_max, cs, &launches);
@@ -131,8 +157,23 @@ int build_step_graph(nb_ctx* ctx)
     return launches == STEP_GRAPH_KERNELS ? NB_OK : NB_ECUDA;
 }
 
-// device pointer to n_act indices: uploads a host list into `buf`, or passes a device list through
-int resolve_idx(nb_ctx* ctx, const int32_t* idx, int64_t n, int32_t* buf, const int32_t** out)
+// Verify a DEVICE index list: all in [0, N) and, if `unique`, pairwise different.  One kernel marks a bitmap and raises
+// a flag, the flag is read back (the stream is synchronised).  NB_EINVAL on a bad list.
+int verify_idx(nb_ctx* ctx, const int32_t* didx, int64_t n, bool unique)
+{
+    uint32_t* flag = ctx->L.idx_bitmap + ctx->Npad / 32;
+    CU(cudaMemsetAsync(ctx->L.idx_bitmap, 0, (ctx->Npad / 32 + 1) * sizeof(uint32_t), ctx->stream), "index check");
+    CU(nb_launch_check_idx(didx, n, ctx->N, ctx->L.idx_bitmap, flag, unique, ctx->stream), "index check");
+    ctx->launches += 1;
+    uint32_t bad = 0;
+    CU(cudaMemcpyAsync(&bad, flag, sizeof bad, cudaMemcpyDeviceToHost, ctx->stream), "index check");
+    CU(cudaStreamSynchronize(ctx->stream), "index check");
+    return bad ? NB_EINVAL : NB_OK;
+}
+
+// device pointer to n_act indices: uploads a host list into `buf`, or passes a device list through; with index checking
+// on, a user list is verified before anything reads through it
+int resolve_idx(nb_ctx* ctx, const int32_t* idx, int64_t n, int32_t* buf, const int32_t** out, bool unique = true)
 {
     if (idx == nullptr) { *out = nullptr; return NB_OK; }
     if (idx == NB_ACTIVE_INTERNAL) {
@@ -140,10 +181,12 @@ int resolve_idx(nb_ctx* ctx, const int32_t* idx, int64_t n, int32_t* buf, const 
         *out = ctx->L.idx_sched;
         return NB_OK;
     }
-    if (ctx->on_device) { *out = idx; return NB_OK; }
-    CU(cudaMemcpyAsync(buf, idx, n * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream), "upload active_idx");
-    *out = buf;
-    return NB_OK;
+    if (ctx->on_device) *out = idx;
+    else {
+        CU(cudaMemcpyAsync(buf, idx, n * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream), "upload active_idx");
+        *out = buf;
+    }
+    return ctx->check_idx && n > 0 ? verify_idx(ctx, *out, n, unique) : NB_OK;
 }
 
 int copy_out(nb_ctx* ctx, double* dst, const double* src, size_t count)
@@ -154,17 +197,9 @@ int copy_out(nb_ctx* ctx, double* dst, const double* src, size_t count)
     return NB_OK;
 }
 
-}  // namespace
-
-extern "C" {
-
-size_t nb_workspace_bytes(int64_t N)
-{
-    if (N < 1) return 0;
-    return Layout(nullptr, pad_n(N)).bytes;
-}
-
-static int plan_force(int64_t N, int64_t n_act, int n_sm, int64_t max_split, nb_plan* plan)
+// The evaluation itself: plan, launch, results left in the context (fa, fj, fs, fp, fc).  didx: DEVICE indices or
+// nullptr (all N).  No copies, no synchronisation: nb_force, nb_init's startup and nb_energy share it.
+int plan_force(int64_t N, int64_t n_act, int n_sm, int64_t max_split, nb_plan* plan)
 {
     if (!plan || N < 1 || n_act < 1 || n_act > N || n_sm < 1 || N > (int64_t(1) << 30) || max_split < 0) return NB_EINVAL;
     const PlanShape sh = nb_plan_shape(pad_n(N), n_act, n_sm, max_split);
@@ -176,11 +211,48 @@ static int plan_force(int64_t N, int64_t n_act, int n_sm, int64_t max_split, nb_
     p.kernel = sh.kernel; p.unit = sh.unit; p.tile = sh.tile; p.sub = sh.sub; p.ctas_per_sm = sh.ctas_per_sm;
     p.n_units = (int)sh.n_units; p.n_split = (int)S; p.slice_tiles = (int)st;
     const int64_t items = sh.n_units * S;
+    // everything the kernels index with int: work items, rows of a partial plane, planes
+    if (items > INT_MAX || sh.n_units * sh.unit > INT_MAX || S * sh.sub > INT_MAX) return NB_EINVAL;
     p.waves = (double)items / (double)sh.resident;
     p.grid = sh.kernel == 1 ? (int)std::min<int64_t>((items + LJ_WARPS - 1) / LJ_WARPS, (int64_t)n_sm * LJ_CTAS_PER_SM)
                             : (int)std::min<int64_t>(items, sh.resident);
     *plan = p;
     return NB_OK;
+}
+
+int force_internal(nb_ctx* ctx, const int32_t* didx, int64_t n_act)
+{
+    nb_plan plan;
+    const int rc = plan_force(ctx->N, n_act, ctx->n_sm, ctx->max_split, &plan);
+    if (rc != NB_OK) return rc;
+
+    ForceArgs A = base_force_args(ctx);
+    A.idx = didx;
+    A.n_act = (int)n_act;
+    A.n_units = plan.n_units; A.n_split = plan.n_split; A.slice_tiles = plan.slice_tiles;
+    A.n_tiles = (int)(ctx->Npad / plan.tile);
+    A.n_items = plan.n_units * plan.n_split;
+    A.n_planes = plan.n_split * plan.sub;
+    A.ld = plan.n_units * plan.unit;
+
+    int launches = 0;
+    CU(cudaEventRecord(ctx->ev0, ctx->stream), "event record");
+    CU(nb_launch_force(plan, A, eps2_is_zero(ctx->eps), ctx->order, ctx->stream, &launches), "force kernel");
+    CU(cudaEventRecord(ctx->ev1, ctx->stream), "event record");
+    ctx->ev_valid = true;
+    ctx->launches += launches;
+    ctx->forced_n = n_act;
+    return NB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t nb_workspace_bytes(int64_t N)
+{
+    if (N < 1) return 0;
+    return Layout(nullptr, pad_n(N)).bytes;
 }
 
 int nb_plan_force(int64_t N, int64_t n_act, int n_sm, nb_plan* plan) { return plan_force(N, n_act, n_sm, 0, plan); }
@@ -209,6 +281,7 @@ int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const dou
     ctx->device = cfg->device;
     ctx->stream = (cudaStream_t)cfg->stream;
     ctx->on_device = cfg->ptrs_on_device != 0;
+    ctx->check_idx = cfg->check_indices > 0 || (cfg->check_indices == 0 && !ctx->on_device);
     ctx->N = N; ctx->Npad = Npad; ctx->eps = eps;
     ctx->order = cfg->order == 0 ? 6 : cfg->order;
     ctx->eta = cfg->eta > 0 ? cfg->eta : (ctx->order == 4 ? 0.14 : ctx->order == 8 ? 0.75 : 0.45);
@@ -217,7 +290,7 @@ int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const dou
     ctx->L = Layout(cfg->workspace, Npad);
     ctx->L.s.order = ctx->order;
 
-    CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+    ON_DEVICE(ctx);
     CU(cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, ctx->device), "device attribute");
     CU(cudaEventCreate(&ctx->ev0), "event");
     CU(cudaEventCreate(&ctx->ev1), "event");
@@ -235,12 +308,13 @@ int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const dou
     CU(nb_launch_init_state(ctx->L.s, N, Npad, dm, dx, dv, ctx->stream), "init_state");
     ctx->launches += 1;
 
-    // startup (reading R8): two all-active evaluations at t = 0
-    for (int pass = 1; pass <= (ctx->order == 4 ? 1 : ctx->order == 8 ? 3 : 2); ++pass) {
+    // startup (reading R8): two all-active evaluations at t = 0 (one at the 4th order).  The 8th order needs no third:
+    // a and jerk are complete after pass 1, so pass 2 - whose records carry them - yields snap AND crackle (R22).
+    for (int pass = 1; pass <= (ctx->order == 4 ? 1 : 2); ++pass) {
         CU(nb_launch_predict(ctx->L.s, N, 0.0, true, ctx->stream), "predict");
         ctx->launches += 1;
         ctx->predicted = true; ctx->t_pred = 0.0;
-        const int rc = nb_force(ctx, nullptr, N, nullptr, nullptr, nullptr, nullptr);
+        const int rc = force_internal(ctx, nullptr, N);
         if (rc != NB_OK) return rc;
         CU(nb_launch_startup(ctx->L.s, N, ctx->L.fa, ctx->L.fj, ctx->L.fs, pass, ctx->eta_s, k_min, k_max, ctx->stream), "startup");
         ctx->launches += 1;
@@ -253,6 +327,7 @@ int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const dou
 int nb_predict(nb_ctx* ctx, double t)
 {
     if (!ctx || !std::isfinite(t)) return NB_EINVAL;
+    ON_DEVICE(ctx);
     CU(nb_launch_predict(ctx->L.s, ctx->N, t, false, ctx->stream), "predict");
     ctx->launches += 1;
     ctx->t_pred = t; ctx->predicted = true; ctx->forced_n = -1;
@@ -265,31 +340,12 @@ int nb_force(nb_ctx* ctx, const int32_t* active_idx, int64_t n_act, double* a, d
     if (active_idx == nullptr && n_act != 0 && n_act != ctx->N) return NB_EINVAL;
     if (!ctx->predicted) return NB_ESTATE;
     if (n_act == 0) { ctx->forced_n = 0; return NB_OK; }
+    ON_DEVICE(ctx);
 
     const int32_t* didx = nullptr;
     int rc = resolve_idx(ctx, active_idx, n_act, ctx->L.idx_user, &didx);
     if (rc != NB_OK) return rc;
-
-    nb_plan plan;
-    rc = plan_force(ctx->N, n_act, ctx->n_sm, ctx->max_split, &plan);
-    if (rc != NB_OK) return rc;
-
-    ForceArgs A = base_force_args(ctx);
-    A.idx = didx;
-    A.n_act = (int)n_act;
-    A.n_units = plan.n_units; A.n_split = plan.n_split; A.slice_tiles = plan.slice_tiles;
-    A.n_tiles = (int)(ctx->Npad / plan.tile);
-    A.n_items = plan.n_units * plan.n_split;
-    A.n_planes = plan.n_split * plan.sub;
-    A.ld = plan.n_units * plan.unit;
-
-    int launches = 0;
-    CU(cudaEventRecord(ctx->ev0, ctx->stream), "event record");
-    CU(nb_launch_force(plan, A, ctx->eps == 0.0, ctx->order, ctx->stream, &launches), "force kernel");
-    CU(cudaEventRecord(ctx->ev1, ctx->stream), "event record");
-    ctx->ev_valid = true;
-    ctx->launches += launches;
-    ctx->forced_n = n_act;
+    if ((rc = force_internal(ctx, didx, n_act)) != NB_OK) return rc;
 
     if ((rc = copy_out(ctx, a, ctx->L.fa, 3 * n_act)) != NB_OK) return rc;
     if ((rc = copy_out(ctx, jerk, ctx->L.fj, 3 * n_act)) != NB_OK) return rc;
@@ -303,6 +359,7 @@ int nb_force_crackle(nb_ctx* ctx, double* crackle)
 {
     if (!ctx || !crackle) return NB_EINVAL;
     if (ctx->order != 8 || ctx->forced_n < 0) return NB_ESTATE;
+    ON_DEVICE(ctx);
     const int rc = copy_out(ctx, crackle, ctx->L.fc, 3 * (size_t)ctx->forced_n);
     if (rc != NB_OK) return rc;
     if (!ctx->on_device) CU(cudaStreamSynchronize(ctx->stream), "nb_force_crackle");
@@ -314,6 +371,7 @@ int nb_corrector(nb_ctx* ctx, const int32_t* active_idx, int64_t n_act, double d
     if (!ctx || n_act < 0 || n_act > ctx->N || !(dt == dt)) return NB_EINVAL;
     if (active_idx == nullptr && n_act != 0 && n_act != ctx->N) return NB_EINVAL;
     if (ctx->forced_n < 0 || ctx->forced_n != n_act) return NB_ESTATE;
+    ON_DEVICE(ctx);
     if (n_act > 0) {
         const int32_t* didx = nullptr;
         const int rc = resolve_idx(ctx, active_idx, n_act, ctx->L.idx_user, &didx);
@@ -330,6 +388,7 @@ int nb_corrector(nb_ctx* ctx, const int32_t* active_idx, int64_t n_act, double d
 int nb_next_block(nb_ctx* ctx, double* t_next, int32_t* active_idx, int64_t* n_act)
 {
     if (!ctx || !t_next || !n_act) return NB_EINVAL;
+    ON_DEVICE(ctx);
     int launches = 0;
     CU(nb_launch_next_block(ctx->L.s, ctx->N, ctx->L.idx_sched, ctx->L.scratch, ctx->stream, &launches), "scheduler");
     ctx->launches += launches;
@@ -348,6 +407,7 @@ int nb_next_block(nb_ctx* ctx, double* t_next, int32_t* active_idx, int64_t* n_a
 int nb_run_blocks(nb_ctx* ctx, double t_end, int64_t max_steps, int64_t* steps_done, double* t_last, int64_t* sum_n_act)
 {
     if (!ctx || !(t_end == t_end) || max_steps < 0) return NB_EINVAL;
+    ON_DEVICE(ctx);
     if (!ctx->step_graph) {
         const int rc = build_step_graph(ctx);
         if (rc != NB_OK) return rc;
@@ -383,8 +443,9 @@ int nb_get_state(nb_ctx* ctx, int field, const int32_t* idx, int64_t n, double* 
 {
     if (!ctx || !out || n < 0 || n > ctx->N || field < NB_M || field > NB_JP) return NB_EINVAL;
     if (n == 0) return NB_OK;
+    ON_DEVICE(ctx);
     const int32_t* didx = nullptr;
-    const int rc = resolve_idx(ctx, idx, n, ctx->L.idx_tmp, &didx);
+    const int rc = resolve_idx(ctx, idx, n, ctx->L.idx_tmp, &didx, /*unique=*/false);
     if (rc != NB_OK) return rc;
     const size_t count = (size_t)n * field_width_host(field);
     double* dst = ctx->on_device ? out : ctx->L.stage;
@@ -401,6 +462,7 @@ int nb_set_state(nb_ctx* ctx, int field, const int32_t* idx, int64_t n, const do
 {
     if (!ctx || !in || n < 0 || n > ctx->N || field < NB_M || (field > NB_DT && field != NB_A4 && field != NB_A5)) return NB_EINVAL;
     if (n == 0) return NB_OK;
+    ON_DEVICE(ctx);
     const int32_t* didx = nullptr;
     const int rc = resolve_idx(ctx, idx, n, ctx->L.idx_tmp, &didx);
     if (rc != NB_OK) return rc;
@@ -420,13 +482,11 @@ int nb_set_state(nb_ctx* ctx, int field, const int32_t* idx, int64_t n, const do
 int nb_energy(nb_ctx* ctx, double* kinetic, double* potential)
 {
     if (!ctx || !kinetic || !potential) return NB_EINVAL;
+    ON_DEVICE(ctx);
     CU(nb_launch_predict(ctx->L.s, ctx->N, 0.0, true, ctx->stream), "predict");
     ctx->launches += 1;
     ctx->predicted = true;
-    const bool od = ctx->on_device;
-    ctx->on_device = true;                                  // no copies, no sync inside nb_force
-    const int rc = nb_force(ctx, nullptr, ctx->N, nullptr, nullptr, nullptr, nullptr);
-    ctx->on_device = od;
+    const int rc = force_internal(ctx, nullptr, ctx->N);
     if (rc != NB_OK) return rc;
     int launches = 0;
     CU(nb_launch_energy(ctx->L.s, ctx->N, ctx->L.fp, (double*)ctx->L.scratch + 16, ctx->stream, &launches), "energy");
@@ -439,63 +499,18 @@ int nb_energy(nb_ctx* ctx, double* kinetic, double* potential)
     return NB_OK;
 }
 
-int nb_probe_fp64_peak(int device, void* stream, void* workspace, size_t workspace_bytes, double seconds, double* tflops, int* n_sm_out)
+int nb_check_indices(nb_ctx* ctx, const int32_t* idx, int64_t n, int unique)
 {
-    if (!workspace || workspace_bytes < 65536 || !tflops || !(seconds > 0)) return NB_EINVAL;
-    cudaStream_t st = (cudaStream_t)stream;
-    int n_sm = 0;
-    if (cudaSetDevice(device) != cudaSuccess) return NB_ECUDA;
-    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return NB_ECUDA;
-    cudaEvent_t e0, e1;
-    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return NB_ECUDA;
-    const double flop_per_iter = (double)n_sm * 4 * 256 * 16 * 8 * 2;
-    int iters = 20000;
-    float ms = 0;
-    double best = 0;
-    int rc = NB_OK;
-    // calibrate, then run back-to-back launches of ~0.25 s until `seconds` have elapsed
-    for (int round = 0; round < 2 && rc == NB_OK; ++round) {
-        double elapsed = 0;
-        do {
-            cudaEventRecord(e0, st);
-            if (nb_launch_fp64_probe((double*)workspace, n_sm, iters, st) != cudaSuccess) { rc = NB_ECUDA; break; }
-            cudaEventRecord(e1, st);
-            if (cudaEventSynchronize(e1) != cudaSuccess || cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) { rc = NB_ECUDA; break; }
-            elapsed += ms * 1e-3;
-            if (round == 1) best = flop_per_iter * iters / (ms * 1e-3) * 1e-12;   // the LAST launch: sustained, not burst
-        } while (round == 1 && elapsed < seconds);
-        if (round == 0 && ms > 0) iters = std::max(1000, (int)(iters * 250.0 / ms));
+    if (!ctx || n < 0 || (n > 0 && !idx) || idx == NB_ACTIVE_INTERNAL) return NB_EINVAL;
+    if (n == 0) return NB_OK;
+    if (n > ctx->N) return NB_EINVAL;                       // no call of this library takes a longer list
+    ON_DEVICE(ctx);
+    const int32_t* didx = idx;
+    if (!ctx->on_device) {
+        CU(cudaMemcpyAsync(ctx->L.idx_tmp, idx, n * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream), "upload indices");
+        didx = ctx->L.idx_tmp;
     }
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    if (rc != NB_OK) return rc;
-    *tflops = best;
-    if (n_sm_out) *n_sm_out = n_sm;
-    return NB_OK;
-}
-
-int nb_probe_dfma_sources(int device, void* stream, void* workspace, size_t workspace_bytes, int kind, double sm_mhz, double* cycles)
-{
-    if (!workspace || workspace_bytes < 65536 || !cycles || kind < 0 || kind > 2 || !(sm_mhz > 0)) return NB_EINVAL;
-    cudaStream_t st = (cudaStream_t)stream;
-    int n_sm = 0;
-    if (cudaSetDevice(device) != cudaSuccess) return NB_ECUDA;
-    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return NB_ECUDA;
-    cudaEvent_t e0, e1;
-    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return NB_ECUDA;
-    const int iters = 40000;
-    float ms = 0;
-    int rc = NB_OK;
-    for (int round = 0; round < 2 && rc == NB_OK; ++round) {       // the first launch warms up
-        cudaEventRecord(e0, st);
-        if (nb_launch_dfma_source_probe((double*)workspace, n_sm, kind, iters, st) != cudaSuccess) rc = NB_ECUDA;
-        cudaEventRecord(e1, st);
-        if (cudaEventSynchronize(e1) != cudaSuccess || cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) rc = NB_ECUDA;
-    }
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    if (rc != NB_OK) return rc;
-    // 3 x 8 warps per SM = 6 per sub-partition, 64 DFMAs per iteration each
-    *cycles = (double)ms * 1e-3 * sm_mhz * 1e6 / (6.0 * 64.0 * iters);
-    return NB_OK;
+    return verify_idx(ctx, didx, n, unique != 0);
 }
 
 int64_t nb_launch_count(const nb_ctx* ctx) { return ctx ? ctx->launches : 0; }
@@ -503,6 +518,7 @@ int64_t nb_launch_count(const nb_ctx* ctx) { return ctx ? ctx->launches : 0; }
 double nb_last_force_ms(nb_ctx* ctx)
 {
     if (!ctx || !ctx->ev_valid) return -1.0;
+    DeviceGuard guard(ctx->device);
     float ms = 0;
     if (cudaEventSynchronize(ctx->ev1) != cudaSuccess) return -1.0;
     if (cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1) != cudaSuccess) return -1.0;
@@ -526,6 +542,7 @@ const char* nb_last_error(const nb_ctx* ctx) { return ctx ? ctx->err : ""; }
 void nb_free(nb_ctx* ctx)
 {
     if (!ctx) return;
+    DeviceGuard guard(ctx->device);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     if (ctx->step_graph) cudaGraphExecDestroy(ctx->step_graph);

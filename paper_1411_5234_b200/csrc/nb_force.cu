@@ -131,11 +131,7 @@ __device__ __forceinline__ void pair2(const IPart& pi, const JRec (&J)[2], const
 {
     // PIN(v): a branch that is never taken (v > 0) but that ptxas cannot see through.  The sums are live on its
     // taken side, so the run of DFMAs that updates them cannot be moved across it: each pair's run stays in one piece.
-#ifndef NB_NO_PIN
 #define PIN(v) if (__double2hiint(v) < 0) return;
-#else
-#define PIN(v)
-#endif
     double dx[2], dy[2], dz[2], dvx[2], dvy[2], dvz[2], dax[2], day[2], daz[2];
     double s[2], rv[2], rv2[2], B[2], y0[2], t[2], e[2], h[2], y[2], yy[2], mr[2], z[2], q[2], c1[2], c2[2], c3[2];
     // differences, with B = dv.dv (operands are duplicates: two-cycle DFMAs) threaded through them

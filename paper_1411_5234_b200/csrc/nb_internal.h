@@ -15,46 +15,23 @@
 constexpr int NB_PAD = 256;          // particle arrays are padded to a multiple of this
 
 // The force kernels keep one active particle per thread (lanes-over-i) or two per warp (lanes-over-j: every j-record
-// loaded from L2 serves both, measured 20 % faster for 8-16 active particles at N = 2^20, 128 registers).  The
-// lanes-over-i kernel evaluates two j-records at a time with a fixed instruction order (pair2, nb_force.cu): 112
-// registers, 16 warps (4 per scheduler) per SM as 4 CTAs of 128 threads; CTA shapes that leave the four
-// schedulers with unequal warp counts (5 x 96, 3 x 160) measured 15-27 % slower (DESIGN.md 6).
-// The NB_* macros are build-time tunables (defaults = the measured best); -DNB_...=v overrides one for experiments.
-#ifndef NB_LI_THREADS
-#define NB_LI_THREADS 128
-#endif
-#ifndef NB_LI_I
-#define NB_LI_I 1
-#endif
-#ifndef NB_LI_TJ
-#define NB_LI_TJ 128
-#endif
-#ifndef NB_LI_STAGES
-#define NB_LI_STAGES 2
-#endif
-#ifndef NB_LI_CTAS_PER_SM
-#define NB_LI_CTAS_PER_SM 4
-#endif
-// lanes-over-i kernel: each thread owns LI_I active particles, a CTA streams j-tiles through smem
-constexpr int LI_THREADS = NB_LI_THREADS;
-constexpr int LI_I = NB_LI_I;
+// loaded serves both).  The lanes-over-i kernel evaluates two j-records at a time with a fixed instruction order (pair2,
+// nb_force.cu): 114 registers, 16 warps (4 per scheduler) per SM as 4 CTAs of 128 threads; CTA shapes that leave the four
+// schedulers with unequal warp counts (5 x 96, 3 x 160) measured 15-27 % slower (DESIGN.md 6, 11).
+// lanes-over-i kernel: each thread owns one active particle, a CTA streams j-tiles through smem
+constexpr int LI_THREADS = 128;
+constexpr int LI_I = 1;
 constexpr int LI_UNIT = LI_THREADS * LI_I;   // active particles per i-tile
-constexpr int LI_TJ = NB_LI_TJ;              // j-records per smem stage (80 B each), even
-constexpr int LI_STAGES = NB_LI_STAGES;
-constexpr int LI_CTAS_PER_SM = NB_LI_CTAS_PER_SM;
+constexpr int LI_TJ = 128;                   // j-records per smem stage (80 B each), even
+constexpr int LI_STAGES = 2;
+constexpr int LI_CTAS_PER_SM = 4;
 constexpr int LI_W = LI_THREADS / 32;        // small active sets: the CTA's warps share 32 particles and split each j-tile
 // lanes-over-j kernel: each warp owns LJ_I active particles, lanes take different j
 constexpr int LJ_THREADS = 256;
 constexpr int LJ_WARPS = LJ_THREADS / 32;
-#ifndef NB_LJ_I
-#define NB_LJ_I 2
-#endif
-#ifndef NB_LJ_CTAS_PER_SM
-#define NB_LJ_CTAS_PER_SM 2
-#endif
-constexpr int LJ_I = NB_LJ_I;
+constexpr int LJ_I = 2;
 constexpr int LJ_TJ = 32;                    // j-records per warp iteration
-constexpr int LJ_CTAS_PER_SM = NB_LJ_CTAS_PER_SM;
+constexpr int LJ_CTAS_PER_SM = 2;
 constexpr int64_t LJ_MAX_ACT = 16;           // n_act <= this -> lanes-over-j
 constexpr int RED_THREADS = 256;             // threads per block of the partial-sum reduction
 constexpr int64_t LIW_MAX_ACT = 96;          // n_act <= this -> lanes-over-i with 32-particle units (above, a 128-lane i-tile is >= 75 % full)
@@ -74,7 +51,7 @@ struct ForceArgs {
     int n_items;             // n_units * n_split
     int ld;                  // rows of the partial buffer per (slice, component) plane
     double eps2;
-    double* partial;         // [S][10][ld] when S > 1
+    double* partial;         // [planes][NC][ld] when planes > 1; NC = 10 components (a, jerk, snap, pot), 13 at the 8th order
     const DevPlan* dp;       // non-null: the launch was planned on the device (nb_run_blocks); overrides the plan fields above
     int* queue;              // work queue: [0] next item, [1] finished CTAs (both 0 between launches)
     double* out_a; double* out_j; double* out_s; double* out_p;   // [n_act][3] x3, [n_act]
@@ -112,6 +89,4 @@ cudaError_t nb_launch_devstep_head(const StateArrays& s, int64_t N, int64_t Npad
 cudaError_t nb_launch_devstep_tail(const StateArrays& s, int n_sm, const int32_t* active, void* scratch, DevPlan* dp, const double* fa,
                                    const double* fj, const double* fs, double eta, int k_min, int k_max, cudaStream_t st, int* launches);
 cudaError_t nb_launch_energy(const StateArrays& s, int64_t N, const double* pot, double* scratch, cudaStream_t st, int* launches);
-cudaError_t nb_launch_fp64_probe(double* out, int n_sm, int iters, cudaStream_t st);
-// 3 CTAs x 256 threads per SM, 64 DFMAs per thread and iteration; kind: see nb_step.cu
-cudaError_t nb_launch_dfma_source_probe(double* out, int n_sm, int kind, int iters, cudaStream_t st);
+cudaError_t nb_launch_check_idx(const int32_t* idx, int64_t n, int64_t N, uint32_t* bitmap, uint32_t* flag, bool unique, cudaStream_t st);

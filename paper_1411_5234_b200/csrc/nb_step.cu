@@ -100,7 +100,7 @@ __device__ __forceinline__ double norm3(double a, double b, double c) { return s
 
 // ------------------------------------------------------------------ a0: startup (reading R8)
 // pass 1: store a, jerk from the first evaluation (snap of that evaluation is discarded).
-// pass 2: store a, jerk, snap; crackle = 0; dt = eta_s |a|/|jerk| floored to a power of two.
+// pass 2: store a, jerk, snap; crackle = 0 (8th order: the evaluated crackle); dt = eta_s |a|/|jerk| floored to a power of two.
 __global__ void startup_kernel(StateArrays s, int64_t N, const double* fa, const double* fj, const double* fs, int pass,
                                double eta_s, int k_min, int k_max)
 {
@@ -118,7 +118,7 @@ __global__ void startup_kernel(StateArrays s, int64_t N, const double* fa, const
     const double sx = o4 ? 0.0 : fs[3 * i], sy = o4 ? 0.0 : fs[3 * i + 1], sz = o4 ? 0.0 : fs[3 * i + 2];
     s.st2[i] = make_double4(ax, ay, az, jx);
     s.st3[i] = make_double4(jy, jz, sx, sy);
-    const bool c8 = s.order == 8 && pass == 3;              // 8th order: the third pass (a and jerk known) gives crackle
+    const bool c8 = s.order == 8;                           // 8th order: pass 2's records carry a AND jerk, so it gives crackle too
     s.st4[i] = make_double4(sz, c8 ? s.fc[3 * i] : 0.0, c8 ? s.fc[3 * i + 1] : 0.0, c8 ? s.fc[3 * i + 2] : 0.0);
     const double r = eta_s * norm3(ax, ay, az) / norm3(jx, jy, jz);
     int k;
@@ -500,62 +500,24 @@ __global__ void __launch_bounds__(TPB) energy_final_kernel(const double* part, i
     if (threadIdx.x == 0) { out[0] = sk[0]; out[1] = sw[0]; }
 }
 
-// ------------------------------------------------------------------ FP64 peak probe
-// 8 independent FMA chains per thread, 256 threads x 4 CTAs per SM: nothing but DFMA in the loop.
-__global__ void __launch_bounds__(256) fp64_probe_kernel(double* out, int iters)
+// ------------------------------------------------------------------ index-list verification (nb_config.check_indices)
+// flag bit 0: an index outside [0, N); bit 1: a duplicate (bitmap: one bit per particle, zeroed by the caller).
+__global__ void __launch_bounds__(TPB) check_idx_kernel(const int32_t* idx, int64_t n, int64_t N, uint32_t* bitmap, uint32_t* flag, bool unique)
 {
-    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
-    const double m = 0.999999, c = 1e-7;
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int u = 0; u < 16; ++u) {
-            a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
-            a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
-        }
-    }
-    const double r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
-    if (r == 12345.678) out[blockIdx.x] = r;     // never true; keeps the chains alive
-}
-
-// Operand-source probes: 8 independent chains, 64 DFMAs per loop iteration, in three flavours.
-//   0: acc = acc * m + c, m and c loop constants       -> two cycles per DFMA (the pipe's rate)
-//   1: acc_k = b_k * d_k + acc_k, three register pairs  -> three cycles
-//   2: acc_k = q * d_k + acc_k, q shared by the run     -> two cycles where the operand-reuse cache supplies q
-#define PROBE_FMA(d, a, b, c) asm volatile("fma.rn.f64 %0, %1, %2, %3;" : "=d"(d) : "d"(a), "d"(b), "d"(c))
-template <int KIND>
-__global__ void __launch_bounds__(256) dfma_source_probe_kernel(double* out, int iters, double seed)
-{
-    double a[8], b[8], d[8];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) {
-        a[k] = threadIdx.x + k; b[k] = seed * (k + 1) + threadIdx.x * 1e-9; d[k] = seed * 0.1 * (k + 2) + threadIdx.x * 1e-9;
-    }
-    const double q = seed + threadIdx.x * 1e-9;
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int u = 0; u < 8; ++u) {
-#pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                if (KIND == 0) PROBE_FMA(a[k], a[k], 0.999999, 1e-7);
-                if (KIND == 1) PROBE_FMA(a[k], b[k], d[k], a[k]);
-                if (KIND == 2) PROBE_FMA(a[k], q, d[k], a[k]);
-            }
-        }
-    }
-    double r = 0;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) r += a[k];
-    if (r == 12345.678) out[blockIdx.x] = r;     // never true; keeps the chains alive
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const int32_t i = idx[k];
+    if (i < 0 || (int64_t)i >= N) { atomicOr(flag, 1u); return; }
+    if (!unique) return;
+    const uint32_t bit = 1u << (i & 31);
+    if (atomicOr(bitmap + (i >> 5), bit) & bit) atomicOr(flag, 2u);
 }
 
 }  // namespace
 
-cudaError_t nb_launch_dfma_source_probe(double* out, int n_sm, int kind, int iters, cudaStream_t st)
+cudaError_t nb_launch_check_idx(const int32_t* idx, int64_t n, int64_t N, uint32_t* bitmap, uint32_t* flag, bool unique, cudaStream_t st)
 {
-    const double seed = 1e-3;
-    if (kind == 0) dfma_source_probe_kernel<0><<<n_sm * 3, 256, 0, st>>>(out, iters, seed);
-    else if (kind == 1) dfma_source_probe_kernel<1><<<n_sm * 3, 256, 0, st>>>(out, iters, seed);
-    else dfma_source_probe_kernel<2><<<n_sm * 3, 256, 0, st>>>(out, iters, seed);
+    check_idx_kernel<<<nblocks(n), TPB, 0, st>>>(idx, n, N, bitmap, flag, unique);
     return cudaGetLastError();
 }
 
@@ -650,11 +612,5 @@ cudaError_t nb_launch_energy(const StateArrays& s, int64_t N, const double* pot,
     energy_partial_kernel<<<nb, TPB, 0, st>>>(s, N, pot, scratch + 2);
     energy_final_kernel<<<1, TPB, 0, st>>>(scratch + 2, nb, scratch);
     *launches += 2;
-    return cudaGetLastError();
-}
-
-cudaError_t nb_launch_fp64_probe(double* out, int n_sm, int iters, cudaStream_t st)
-{
-    fp64_probe_kernel<<<n_sm * 4, 256, 0, st>>>(out, iters);
     return cudaGetLastError();
 }

@@ -27,11 +27,34 @@ def test_library_exports_every_declared_symbol(B):
     L = B.lib()
     for name in declared:
         assert hasattr(L, name), name
+    # the product library holds the method's calls and their helpers only: measurement aids live in libnbprobe.so
+    assert not [n for n in declared if "probe" in n]
+
+
+def test_probe_library_is_separate_and_exports_its_header(B):
+    from paper_1411_5234_b200 import probes
+    hdr = open(os.path.join(ROOT, "paper_1411_5234_b200", "csrc", "nb_probe.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = sorted(set(re.findall(r"\b(nbp_[a-z0-9_]+)\s*\(", hdr)))
+    assert declared == sorted(probes.EXPORTS)
+    L = probes.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+    assert L.nbp_fp64_peak(0, None, None, 0, 1.0, None, None) == -1            # argument validation needs no GPU
+    for name in declared:
+        assert not hasattr(B.lib(), name), name                                 # ... and none of it is in libnb.so
+
+
+def test_build_staleness_tracks_every_header(B):
+    from paper_1411_5234_b200 import build
+    hs = {os.path.basename(h) for h in build._headers()}
+    assert {"nb.h", "nb_internal.h", "nb_plan.h", "nb_probe.h"} <= hs
+    assert not build.stale()
 
 
 def test_struct_layouts_match_header(B):
-    # nb_config: int, void*, void*, size_t, int, double, double, int, int  (natural alignment)
-    assert C.sizeof(B.nb_config) == 72 and B.nb_config.order.offset == 64
+    # nb_config: int, void*, void*, size_t, int, double, double, int, int, int, int  (natural alignment)
+    assert C.sizeof(B.nb_config) == 72 and B.nb_config.order.offset == 64 and B.nb_config.check_indices.offset == 68
     assert B.nb_config.workspace.offset == 16 and B.nb_config.eta.offset == 40 and B.nb_config.k_max.offset == 60
     assert C.sizeof(B.nb_plan) == 48 and B.nb_plan.waves.offset == 40
 
@@ -80,16 +103,17 @@ def test_argument_validation_without_gpu(B):
     L = B.lib()
     ctx = C.c_void_p()
     m = np.ones(4); x = np.zeros((4, 3)); v = np.zeros((4, 3))
-    cfg = B.nb_config(0, None, None, 0, 0, 0, 0, 0, 0)
+    cfg = B.nb_config(0, None, None, 0, 0, 0, 0, 0, 0, 0, 0)
     pm, px, pv = B._ptr(m), B._ptr(x), B._ptr(v)
     assert L.nb_init(C.byref(ctx), 4, pm, px, pv, 1e-3, C.byref(cfg)) == B.NB_ENOMEM       # no workspace
     assert L.nb_init(C.byref(ctx), 0, pm, px, pv, 1e-3, C.byref(cfg)) == B.NB_EINVAL
     assert L.nb_init(C.byref(ctx), 4, None, px, pv, 1e-3, C.byref(cfg)) == B.NB_EINVAL
     assert L.nb_init(C.byref(ctx), 4, pm, px, pv, float("nan"), C.byref(cfg)) == B.NB_EINVAL
-    bad = B.nb_config(0, None, None, 0, 0, 0, 0, -3, -20)                                   # k_min > k_max
+    bad = B.nb_config(0, None, None, 0, 0, 0, 0, -3, -20, 0, 0)                                   # k_min > k_max
     assert L.nb_init(C.byref(ctx), 4, pm, px, pv, 1e-3, C.byref(bad)) == B.NB_EINVAL
     assert L.nb_predict(None, 0.0) == B.NB_EINVAL
     assert L.nb_force(None, None, 0, None, None, None, None) == B.NB_EINVAL
+    assert L.nb_check_indices(None, None, 0, 1) == B.NB_EINVAL
     assert L.nb_launch_count(None) == 0
     assert L.nb_strerror(B.NB_ESTATE).decode().startswith("call order")
     assert L.nb_strerror(12345).decode() == "unknown status"

@@ -48,6 +48,28 @@ def test_p1_circular_binary_closed_form_and_startup(oracle):
         np.testing.assert_allclose(sysm.s[1], -sn, atol=1e-16)
 
 
+def test_startup_levels_closed_form_on_circular_binary(oracle):
+    """O5 (oracle_startup_levels, reading R8/R11): on the circular binary |jerk| = omega |a| exactly, so the startup step is
+    dt0 = 2^floor(log2(eta_s / omega)) clamped to [2^k_min, 2^k_max].  eta_s values chosen so that eta_s/omega and
+    eta_s*omega (|a| and |jerk| swapped) fall on different sides of a power of two, plus both clamps."""
+    for eps, d in ((0.0, 1.0), (0.1, 1.0), (0.0, 0.25), (0.1, 0.5)):
+        s = d * d + eps * eps
+        omega = np.sqrt(1.0 / s ** 1.5)                     # M = 1: omega^2 = M / (d^2 + eps^2)^(3/2)
+        m = np.array([0.5, 0.5])
+        x = np.array([[0.5 * d, 0, 0], [-0.5 * d, 0, 0]])
+        v = np.array([[0, 0.5 * d * omega, 0], [0, -0.5 * d * omega, 0]])
+        for eta_s in (0.01, 2.0 ** -6 * 0.999 * omega, 2.0 ** -6 * 1.001 * omega, 2.0 ** -9 * 1.3, 0.3):
+            o = oracle.OracleSystem(m, x, v, eps, eta_s=eta_s)
+            k = int(np.floor(np.log2(eta_s / omega)))
+            assert np.all(o.dt == 2.0 ** min(max(k, -20), -3)), (eps, d, eta_s, o.dt, k)
+        # the two values around 2^-6 really straddle the power of two
+        assert np.floor(np.log2(2.0 ** -6 * 0.999)) == -7 and np.floor(np.log2(2.0 ** -6 * 1.001)) == -6
+        # clamps
+        assert np.all(oracle.OracleSystem(m, x, v, eps, eta_s=1e-9).dt == 2.0 ** -20)
+        assert np.all(oracle.OracleSystem(m, x, v, eps, eta_s=50.0).dt == 2.0 ** -3)
+        assert np.all(oracle.OracleSystem(m, x, v, eps, eta_s=0.01, k_min=-5, k_max=-4).dt == 2.0 ** -5)
+
+
 # ---------------------------------------------------------------- P9: 50-digit brute force + differentiation
 @pytest.mark.parametrize("N,eps,seed", [(2, 0.0, 1), (3, 0.05, 2), (3, 0.0, 3), (4, 0.3, 4)])
 def test_p9_tiny_systems_against_mpmath(oracle, N, eps, seed):
@@ -400,6 +422,10 @@ def test_o4_criterion_closed_form_and_block_steps(oracle):
             break
         o.predict(tn); o.force(act); o.corrector(act, 0.0)
         n += 1
+        # block rule (R12): every particle's time is a multiple of its power-of-two step, levels stay in range
+        assert np.all(np.mod(o.t, o.dt) == 0.0)
+        lv = np.log2(o.dt)
+        assert np.all(lv == np.round(lv)) and lv.min() >= -20 and lv.max() <= -3
     assert np.all(o.t == 0.125) and n > 10
     assert abs(sum(o.energy()) / E0 - 1) < 1e-5
 
@@ -526,5 +552,9 @@ def test_o8_criterion_closed_form_and_block_steps(oracle):
             break
         o.predict(tn); o.force(act); o.corrector(act, 0.0)
         n += 1
+        # block rule (R12): every particle's time is a multiple of its power-of-two step, levels stay in range
+        assert np.all(np.mod(o.t, o.dt) == 0.0)
+        lv = np.log2(o.dt)
+        assert np.all(lv == np.round(lv)) and lv.min() >= -20 and lv.max() <= -3
     assert np.all(o.t == 0.125) and n > 10
     assert abs(sum(o.energy()) / E0 - 1) < 1e-6
