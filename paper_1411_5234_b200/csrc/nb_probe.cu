@@ -90,9 +90,11 @@ __global__ void __launch_bounds__(256) mixed_rate_kernel(double* out, int iters,
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
                 if (KIND == 0) P_FFMA(fa[k], fb[k], fd[k], fa[k]);                       // FFMA, three register sources
-                if (KIND == 1) P_D2F(fa[k], db[k]);                                      // F2F.F32.F64
-                if (KIND == 2) P_F2D(da[k], fb[k]);                                      // F2F.F64.F32
-                if (KIND == 3) { double t; P_F2D(t, fb[k]); P_DADD(da[k], da[k], t); }    // DP accumulation of an SP term
+                // ptxas removes conversions whose results are dead, so the conversion streams are dependent chains
+                // (8 independent chains per thread, like the FMA streams): double -> float -> double -> ...
+                if (KIND == 1) { P_D2F(fa[k], da[k]); P_F2D(da[k], fa[k]); }             // one F2F.F32.F64 + one F2F.F64.F32
+                if (KIND == 2) { P_D2F(fa[k], da[k]); P_F2D(da[k], fa[k]); P_DADD(da[k], da[k], db[k]); }   // ... + one DADD
+                if (KIND == 3) { double t; P_F2D(t, fb[k]); P_DADD(da[k], da[k], t); P_FADD(fb[k], fb[k], fd[k]); }   // DP accumulation of a changing SP term
                 if (KIND == 4) {                                                         // float-float accumulation (two-sum)
                     float s, bb, t1, t2, t3;
                     P_FADD(s, fa[k], fb[k]); P_FSUB(bb, s, fa[k]); P_FSUB(t1, s, bb); P_FSUB(t2, fa[k], t1); P_FSUB(t3, fb[k], bb);

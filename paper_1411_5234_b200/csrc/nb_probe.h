@@ -24,13 +24,15 @@ int nbp_dfma_sources(int device, void* stream, void* workspace, size_t workspace
 
 /* Cycles per warp-wide instruction and SM sub-partition of the streams a mixed-precision pair evaluation would be
  * made of ("DP for reciprocal distances and accumulation, SP elsewhere"):
- *   kind 0  FFMA, three register sources            kind 1  F2F.F32.F64 (double -> float)
- *   kind 2  F2F.F64.F32 (float -> double)           kind 3  DADD of a converted float: F2F.F64.F32 + DADD per element
+ *   kind 0  FFMA, three register sources
+ *   kind 1  conversion round trip double -> float -> double (one F2F.F32.F64 + one F2F.F64.F32 per element)
+ *   kind 2  the same round trip + one DADD per element
+ *   kind 3  DP accumulation of an SP term: F2F.F64.F32 + DADD + one FADD (that changes the term) per element
  *   kind 4  float-float accumulation (two-sum, 6 FADD-class ops per element, no conversion)
  *   kind 5  DFMA (2-source) and FFMA interleaved 1:1 - do the FP32 and FP64 pipes issue side by side?
  *   kind 6  FFMA with one source shared by the run (operand-reuse cache)
  *   kind 7  FFMA with one register and two immediates
- * `cycles` = sub-partition cycles per warp instruction of the named kind (kind 3, 4: per accumulated element;
+ * `cycles` = sub-partition cycles per warp instruction of the named kind (kinds 1-4: per element;
  * kind 5: per DFMA+FFMA pair). */
 int nbp_mixed_rates(int device, void* stream, void* workspace, size_t workspace_bytes, int kind, double sm_mhz, double* cycles);
 
