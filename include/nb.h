@@ -92,19 +92,21 @@ typedef enum {
 
 /* How nb_force maps an evaluation onto the GPU (reading R15; "Bfactor"). */
 typedef struct {
-    int kernel;       /* 0 = lanes-over-i (each thread owns I active particles, j-tiles broadcast from shared memory)
-                         1 = lanes-over-j (each warp owns I active particles, its lanes take different j)
-                         2 = lanes-over-i with 32-particle units: the CTA's warps share the particles and split each j-tile */
-    int n_units;      /* i-tiles (kernel 0) or i-groups per warp (kernel 1) */
-    int n_split;      /* S: number of j-slices each unit is split into ("Bfactor") */
+    int kernel;       /* 0 = CTA tiles: a CTA of 128 threads owns 128 active particles, j-tiles broadcast from shared memory
+                         1 = warp units: every warp owns a unit of p = 32, 16, ... 1 active particles and streams its own
+                             j-slice; its lanes are split p ways over particles and 32/p ways over j-records (p = 32:
+                             lanes over i; p = 1: lanes over j).  n_act = 32 a + r is decomposed into a units of 32 and
+                             the binary digits of r, so no lane idles */
+    int n_units;      /* i-tiles (kernel 0) or warp units (kernel 1) */
+    int n_split;      /* S: number of j-slices each unit is split into ("Bfactor") = partial sums per particle */
     int slice_tiles;  /* j-tiles per slice (the last slice may hold fewer) */
     int grid;         /* CTAs launched */
-    int unit;         /* active particles per unit (kernel 0: threads per CTA x I; kernel 1: I) */
-    int tile;         /* j-records per j-tile (kernel 0: one shared-memory stage; kernel 1: one warp iteration) */
+    int unit;         /* active particles per full unit (kernel 0: 128; kernel 1: 32) */
+    int tile;         /* j-records per j-tile (kernel 0: one shared-memory stage of the CTA, 128; kernel 1: of a warp, 64) */
     int ctas_per_sm;  /* resident CTAs per multiprocessor the plan assumes */
-    int sub;          /* parts each j-tile is split into inside a CTA (kernel 2: warps per CTA; else 1); a unit
-                         writes n_split * sub partial sums */
-    double waves;     /* work items / resident CTAs (or warps) on the device */
+    int predict_in_force; /* 1: in a device-planned block step (nb_run_blocks) with this n_act the force kernel predicts the
+                         j-records it reads from the state itself and the predictor's pass over all N is skipped */
+    double waves;     /* work items / resident workers (CTAs or warps) on the device */
 } nb_plan;
 
 /* Bytes of device workspace a context for N particles needs.  Pure; 0 if N < 1. */
@@ -184,9 +186,11 @@ int nb_next_block(nb_ctx* ctx, double* t_next, int32_t* active_idx, int64_t* n_a
  * repeats { nb_next_block; stop if t_next > t_end; nb_predict(t_next); nb_force(internal list);
  * nb_corrector(internal list, per-particle dt) } at most max_steps times.  Every decision of a step -
  * t_next, the active list, n_act, the j-split of the force launch (reading R15; "determined
- * step by step") - is taken on the device, and one step is one replay of a CUDA graph; the host enqueues
- * batches of replays and reads the counters after each batch.  The arithmetic and its order are those of
- * the separate calls: states agree bit for bit.
+ * step by step") - is taken on the device, and one step is one replay of a CUDA graph of four kernels
+ * (scheduler, predictor, force, reduction + corrector); for small active sets the force kernel predicts the
+ * j-records it reads and the predictor's pass is skipped.  The host enqueues batches of replays and reads
+ * the counters after each batch.  The arithmetic and its order are those of the separate calls: states
+ * agree bit for bit.  The predicted records (NB_XP ...) are not defined afterwards.
  * steps_done, t_last (time of the last completed step; -1 if none), sum_n_act (sum of n_act over the
  * steps: interactions = sum_n_act * (N - 1)): HOST pointers, any may be NULL.  Synchronises the stream.
  */

@@ -34,7 +34,7 @@ class nb_config(C.Structure):
 
 class nb_plan(C.Structure):
     _fields_ = [("kernel", C.c_int), ("n_units", C.c_int), ("n_split", C.c_int), ("slice_tiles", C.c_int),
-                ("grid", C.c_int), ("unit", C.c_int), ("tile", C.c_int), ("ctas_per_sm", C.c_int), ("sub", C.c_int),
+                ("grid", C.c_int), ("unit", C.c_int), ("tile", C.c_int), ("ctas_per_sm", C.c_int), ("predict_in_force", C.c_int),
                 ("waves", C.c_double)]
 
 

@@ -44,8 +44,9 @@ struct Layout {
         Carve c(base);
         s.st0 = c.take<double4>(Npad); s.st1 = c.take<double4>(Npad); s.st2 = c.take<double4>(Npad);
         s.st3 = c.take<double4>(Npad); s.st4 = c.take<double4>(Npad); s.dt = c.take<double>(Npad);
-        s.pj0 = c.take<double4>(Npad); s.pj1 = c.take<double4>(Npad); s.pj2 = c.take<double2>(Npad);
-        s.st5 = c.take<double4>(Npad); s.st6 = c.take<double4>(Npad); s.pj3 = c.take<double4>(Npad);
+        s.tn = c.take<double>(Npad);
+        s.rec = c.take<double2>(Npad * REC_Q_MAX);          // 80-B records (112 B at the 8th order)
+        s.st5 = c.take<double4>(Npad); s.st6 = c.take<double4>(Npad);
         fa = c.take<double>(3 * Npad); fj = c.take<double>(3 * Npad); fs = c.take<double>(3 * Npad); fp = c.take<double>(Npad);
         fc = c.take<double>(3 * Npad); s.fc = fc; s.order = 6;
         partial = c.take<double>(13 * partial_rows(Npad));   // 10 components, 13 at the 8th order
@@ -118,7 +119,9 @@ inline bool eps2_is_zero(double eps) { return !(eps * eps >= DBL_MIN); }
 ForceArgs base_force_args(const nb_ctx* ctx)
 {
     ForceArgs A{};
-    A.pj0 = ctx->L.s.pj0; A.pj1 = ctx->L.s.pj1; A.pj2 = ctx->L.s.pj2; A.pj3 = ctx->L.s.pj3;
+    const StateArrays& s = ctx->L.s;
+    A.rec = s.rec;
+    A.st0 = s.st0; A.st1 = s.st1; A.st2 = s.st2; A.st3 = s.st3; A.st4 = s.st4; A.st5 = s.st5; A.st6 = s.st6;
     A.eps2 = eps2_is_zero(ctx->eps) ? 0.0 : ctx->eps * ctx->eps;
     A.partial = ctx->L.partial;
     A.queue = ctx->L.queue;                                 // zeroed by nb_init, left at 0 by every launch
@@ -126,9 +129,10 @@ ForceArgs base_force_args(const nb_ctx* ctx)
     return A;
 }
 
-// One block step with every decision taken on the device, captured once as a CUDA graph: scheduler (+ plan of the
-// force launch) -> predictor -> the three force kernel shapes (two of them return at once) -> reduction -> corrector.
-constexpr int STEP_GRAPH_KERNELS = 9;
+// One block step with every decision taken on the device, captured once as a CUDA graph of FOUR kernels: scheduler (+ plan
+// of the force launch) -> predictor (returns at once when the force kernel predicts for itself) -> force (either shape,
+// from the plan) -> partial-sum reduction + corrector.
+constexpr int STEP_GRAPH_KERNELS = 4;
 
 int build_step_graph(nb_ctx* ctx)
 {
@@ -140,13 +144,12 @@ int build_step_graph(nb_ctx* ctx)
     if (e == cudaSuccess) {
         ForceArgs A = base_force_args(ctx);
         A.idx = ctx->L.idx_sched;
-        A.n_tiles = 0;                                      // set per kernel below
         A.dp = ctx->L.devplan;
-        e = nb_launch_devstep_head(ctx->L.s, ctx->N, ctx->Npad, ctx->n_sm, ctx->L.idx_sched, ctx->L.scratch, ctx->L.devplan, cs, &launches);
+        e = nb_launch_devstep_head(ctx->L.s, ctx->N, ctx->Npad, ctx->n_sm, ctx->L.idx_sched, ctx->L.idx_tmp, ctx->L.scratch, ctx->L.devplan,
+                                   cs, &launches);
         if (e == cudaSuccess) e = nb_launch_force_devplan(A, eps2_is_zero(ctx->eps), ctx->order, ctx->n_sm, (int)ctx->Npad, cs, &launches);
         if (e == cudaSuccess)
-            e = nb_launch_devstep_tail(ctx->L.s, ctx->n_sm, ctx->L.idx_sched, ctx->L.scratch, ctx->L.devplan, ctx->L.fa, ctx->L.fj, ctx->L.fs,
-                                       ctx->eta, ctx->k_min, ctx->k_max, cs, &launches);
+            e = nb_launch_devstep_tail(ctx->L.s, ctx->n_sm, ctx->L.idx_sched, A, ctx->L.devplan, ctx->eta, ctx->k_min, ctx->k_max, cs, &launches);
         const cudaError_t e2 = cudaStreamEndCapture(cs, &graph);
         if (e == cudaSuccess) e = e2;
     }
@@ -208,13 +211,14 @@ int plan_force(int64_t N, int64_t n_act, int n_sm, int64_t max_split, nb_plan* p
     int64_t st;
     nb_split_cost(sh, S, &st);
     nb_plan p{};
-    p.kernel = sh.kernel; p.unit = sh.unit; p.tile = sh.tile; p.sub = sh.sub; p.ctas_per_sm = sh.ctas_per_sm;
+    p.kernel = sh.kernel; p.unit = sh.unit; p.tile = sh.tile; p.ctas_per_sm = sh.ctas_per_sm;
     p.n_units = (int)sh.n_units; p.n_split = (int)S; p.slice_tiles = (int)st;
+    p.predict_in_force = sh.kernel == 1 && sh.n_units <= PIF_MAX_UNITS;
     const int64_t items = sh.n_units * S;
-    // everything the kernels index with int: work items, rows of a partial plane, planes
-    if (items > INT_MAX || sh.n_units * sh.unit > INT_MAX || S * sh.sub > INT_MAX) return NB_EINVAL;
+    // everything the kernels index with int: work items, rows of a partial plane
+    if (items > INT_MAX || sh.n_units * sh.unit > INT_MAX) return NB_EINVAL;
     p.waves = (double)items / (double)sh.resident;
-    p.grid = sh.kernel == 1 ? (int)std::min<int64_t>((items + LJ_WARPS - 1) / LJ_WARPS, (int64_t)n_sm * LJ_CTAS_PER_SM)
+    p.grid = sh.kernel == 1 ? (int)std::min<int64_t>((items + WU_WARPS - 1) / WU_WARPS, (int64_t)n_sm * WU_CTAS_PER_SM)
                             : (int)std::min<int64_t>(items, sh.resident);
     *plan = p;
     return NB_OK;
@@ -232,8 +236,7 @@ int force_internal(nb_ctx* ctx, const int32_t* didx, int64_t n_act)
     A.n_units = plan.n_units; A.n_split = plan.n_split; A.slice_tiles = plan.slice_tiles;
     A.n_tiles = (int)(ctx->Npad / plan.tile);
     A.n_items = plan.n_units * plan.n_split;
-    A.n_planes = plan.n_split * plan.sub;
-    A.ld = plan.n_units * plan.unit;
+    A.ld = plan.kernel == 0 ? plan.n_units * plan.unit : (int)n_act;
 
     int launches = 0;
     CU(cudaEventRecord(ctx->ev0, ctx->stream), "event record");
@@ -292,6 +295,7 @@ int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const dou
 
     ON_DEVICE(ctx);
     CU(cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, ctx->device), "device attribute");
+    CU(nb_force_setup(), "kernel attributes");
     CU(cudaEventCreate(&ctx->ev0), "event");
     CU(cudaEventCreate(&ctx->ev1), "event");
     CU(cudaMemsetAsync(ctx->L.scratch, 0, scratch_bytes(Npad), ctx->stream), "memset scratch");
@@ -390,7 +394,7 @@ int nb_next_block(nb_ctx* ctx, double* t_next, int32_t* active_idx, int64_t* n_a
     if (!ctx || !t_next || !n_act) return NB_EINVAL;
     ON_DEVICE(ctx);
     int launches = 0;
-    CU(nb_launch_next_block(ctx->L.s, ctx->N, ctx->L.idx_sched, ctx->L.scratch, ctx->stream, &launches), "scheduler");
+    CU(nb_launch_next_block(ctx->L.s, ctx->N, ctx->L.idx_sched, ctx->L.idx_tmp, ctx->L.scratch, ctx->stream, &launches), "scheduler");
     ctx->launches += launches;
     struct { double t; long long n; } res;
     CU(cudaMemcpyAsync(&res, ctx->L.scratch, sizeof res, cudaMemcpyDeviceToHost, ctx->stream), "scheduler result");
@@ -415,7 +419,6 @@ int nb_run_blocks(nb_ctx* ctx, double t_end, int64_t max_steps, int64_t* steps_d
     DevPlan h{};
     h.t_end = t_end; h.steps_left = max_steps; h.t_last = -1.0; h.max_split = ctx->max_split;
     CU(cudaMemcpyAsync(ctx->L.devplan, &h, sizeof h, cudaMemcpyHostToDevice, ctx->stream), "upload step control");
-    CU(cudaMemsetAsync(ctx->L.scratch, 0xff, 8, ctx->stream), "reset t_next");
     ctx->predicted = false; ctx->forced_n = -1; ctx->sched_n = -1;
     // The host cannot know when the device stops, so it enqueues batches of steps and looks at the counters after each;
     // steps enqueued after the stop flag is up return at once (every kernel checks it).

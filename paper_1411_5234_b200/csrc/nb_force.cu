@@ -1,16 +1,17 @@
 // nb_force.cu — the pairwise evaluation: acceleration, jerk, snap and
 // potential of eq. (1)-(2) and their time derivatives (R3), for
 // the active particles against all N predicted j-records.  fp64 on the FP64 ALU pipe; tensor cores
-// are not used (no dense contraction).  Kernel shapes, all writing per-slice partial sums that a
-// reduction kernel adds in a fixed order (the "Bfactor" j-split of PAPER.md:59-65, made deterministic):
-//   force_li_kernel<EPS0, W, ORDER>  lanes-over-i: a thread owns one active particle in registers; the CTA
-//                    streams j-tiles into shared memory with 1-D TMA bulk copies (UBLKCP) signalled
-//                    on mbarriers, double-buffered; every lane reads the same j-record (broadcast LDS).
-//                    W = 1: i-tiles of 128 particles.  W = 4 (17..96 active): i-tiles of 32, the four warps
-//                    take different parts of each j-tile.
-//   force_lj_kernel<EPS0, ORDER>  lanes-over-j (<= 16 active): a warp owns one active particle (same in every
-//                    lane); its 32 lanes read 32 different j-records straight from global memory (coalesced)
-//                    and the sums are combined with a warp-shuffle butterfly.
+// are not used (no dense contraction).  Two kernel shapes, both writing per-slice partial sums that are
+// added in a fixed order (the "Bfactor" j-split of PAPER.md:59-65, made deterministic):
+//   li_body  "CTA tiles" (n_act >= LI_MIN_ACT): a thread owns one active particle in registers; the CTA streams
+//            j-tiles of 128 records into shared memory with 1-D TMA bulk copies (UBLKCP) signalled on mbarriers,
+//            double-buffered; every lane reads the same j-record (broadcast LDS).
+//   wu_body  "warp units" (smaller active sets, the paper's Bfactor regime): every warp is its own worker with a
+//            private double-buffered ring of 64-record tiles (one bulk copy per tile).  A unit is p = 32, 16, .. 1
+//            particles: the lanes are split p ways over particles and 32/p ways over the records of a step, from
+//            lanes-over-i (p = 32) to lanes-over-j (p = 1); the 32/p lane sums of a particle are combined with a
+//            warp-shuffle butterfly.  In a device-planned block step with few units the warp PREDICTS the records of
+//            its slice from the state instead of reading them (the predictor's pass over all N is skipped).
 // ORDER = 6 is the scheme of the north star (a, jerk, snap, pot); 4 (a, jerk, pot) and 8 (+ crackle) are the other
 // Hermite orders the paper names (R21, R22).
 // Work items (i-unit, j-slice) are handed out by an atomic queue, not by a static stride: warps of
@@ -20,24 +21,15 @@
 // results stay bitwise reproducible.
 #include "nb_internal.h"
 #include "nb_plan.h"
+#include "nb_predict.h"
 
 namespace {
 
-// ---------------------------------------------------------------------------------------------
-// One pair, 6th order.  53 FP64-pipe instructions (32 DFMA + 11 DMUL + 10 DADD) + 1 MUFU.RSQ64H.  Used by the
-// lanes-over-j kernel; the lanes-over-i kernel uses pair2 below.
-// ---------------------------------------------------------------------------------------------
 struct Sums { double ax, ay, az, jx, jy, jz, sx, sy, sz, p, cx, cy, cz; };   // cx..cz: crackle, 8th order only
 
 struct IPart { double x, y, z, vx, vy, vz, ax, ay, az, jx, jy, jz; };        // jx..jz: predicted jerk, 8th order only
 
-// fp64 reciprocal-square-root seed: MUFU.RSQ64H works on the high word only (about 20 good bits).
-__device__ __forceinline__ double rsqrt_seed(double s)
-{
-    double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(s));
-    return y;
-}
+struct JRec { double x, y, z, m, vx, vy, vz, ax, ay, az, jx, jy, jz; };      // one predicted j-record in registers
 
 // fma / mul with the operand order fixed in PTX.  A DFMA that reads three different register pairs occupies
 // the FP64 pipe for 3 cycles instead of 2 unless one operand comes from the operand-reuse cache of its slot
@@ -55,52 +47,18 @@ __device__ __forceinline__ double M(double a, double b)
     asm("mul.rn.f64 %0, %1, %2;" : "=d"(d) : "d"(a), "d"(b));
     return d;
 }
+// fp64 reciprocal-square-root seed: MUFU.RSQ64H works on the high word only (about 20 good bits).
+__device__ __forceinline__ double rsqrt_seed(double s)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(s));
+    return y;
+}
 // 2 c by incrementing the exponent field (integer pipe, not the FP64 pipe).  Exact for every normal c; for
 // c = +-0 it returns +-2^-1022 instead of 0, which only ever multiplies a finite u and is added to da.
 __device__ __forceinline__ double twice(double c)
 {
     return __hiloint2double(__double2hiint(c) + 0x00100000, __double2loint(c));
-}
-
-// MASK = false: the caller knows that no lane meets its own record here (self is ignored).
-template <bool EPS0, bool MASK = true>
-__device__ __forceinline__ void pair(const IPart& pi, const double4 p0, const double4 p1, const double2 p2,
-                                     const double eps2, const bool self, Sums& S)
-{
-    const double dx = p0.x - pi.x, dy = p0.y - pi.y, dz = p0.z - pi.z;
-    const double dvx = p1.x - pi.vx, dvy = p1.y - pi.vy, dvz = p1.z - pi.vz;
-    const double dax = p1.w - pi.ax, day = p2.x - pi.ay, daz = p2.y - pi.az;
-    double s = F(dx, dx, F(dy, dy, F(dz, dz, eps2)));
-    if (EPS0 && MASK) s = self ? 1.0 : s;                // eps = 0: keep the masked self pair finite
-    // y = s^(-1/2): seed e0 ~ 2^-20, one cubic (Halley) step leaves 5/16 e0^3 < 2^-60
-    const double y0 = rsqrt_seed(s);
-    const double e = F(-s, M(y0, y0), 1.0);
-    const double y = F(M(y0, e), F(e, 0.375, 0.5), y0);
-    // rv = dx.dv and B = dv.dv + dx.da, interleaved so that dx_k is shared by consecutive FMAs
-    double rv = M(dz, dvz);
-    double B = M(dvz, dvz);
-    B = F(dz, daz, B);
-    B = F(dvy, dvy, B);
-    rv = F(dy, dvy, rv);
-    B = F(dy, day, B);
-    B = F(dvx, dvx, B);
-    rv = F(dx, dvx, rv);
-    B = F(dx, dax, B);
-    const double yy = M(y, y);                           // 1/s
-    const double z = M(yy, -3.0);
-    const double mr = M(y, p0.w);                        // m_j / sqrt(s)
-    const double q = M(yy, mr);                          // m_j s^(-3/2)
-    const double alpha = M(yy, rv);
-    const double c1 = M(z, rv);                          // -3 alpha
-    const double c3 = F(c1, alpha, M(z, B));             // -3 beta = -3 (B/s + alpha^2)
-    const double c2 = twice(c1);                         // -6 alpha
-    const double ux = F(c1, dx, dvx), uy = F(c1, dy, dvy), uz = F(c1, dz, dvz);      // dv - 3 alpha dx
-    double wx = F(c3, dx, dax), wy = F(c3, dy, day), wz = F(c3, dz, daz);            // da - 3 beta dx ...
-    wx = F(c2, ux, wx); wy = F(c2, uy, wy); wz = F(c2, uz, wz);                      // ... - 6 alpha u
-    S.ax = F(q, dx, S.ax); S.ay = F(q, dy, S.ay); S.az = F(q, dz, S.az);
-    S.jx = F(q, ux, S.jx); S.jy = F(q, uy, S.jy); S.jz = F(q, uz, S.jz);
-    S.sx = F(q, wx, S.sx); S.sy = F(q, wy, S.sy); S.sz = F(q, wz, S.sz);
-    S.p += (MASK && self) ? 0.0 : mr;                    // j != i (eq. 1); a, jerk, snap get exactly 0 from the self pair
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -124,7 +82,6 @@ __device__ __forceinline__ void pair(const IPart& pi, const double4 p0, const do
 #define VRSQ(d, a) asm volatile("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(d) : "d"(a))
 #define BOTH for (int k = 0; k < 2; ++k)
 
-struct JRec { double4 p0, p1; double2 p2; };
 
 template <bool EPS0, bool MASK>
 __device__ __forceinline__ void pair2(const IPart& pi, const JRec (&J)[2], const double eps2, const bool (&self)[2], Sums& S)
@@ -136,29 +93,29 @@ __device__ __forceinline__ void pair2(const IPart& pi, const JRec (&J)[2], const
     double s[2], rv[2], rv2[2], B[2], y0[2], t[2], e[2], h[2], y[2], yy[2], mr[2], z[2], q[2], c1[2], c2[2], c3[2];
     // differences, with B = dv.dv (operands are duplicates: two-cycle DFMAs) threaded through them
 #pragma unroll
-    BOTH VSUB(dvz[k], J[k].p1.z, pi.vz);
+    BOTH VSUB(dvz[k], J[k].vz, pi.vz);
 #pragma unroll
-    BOTH VSUB(dvy[k], J[k].p1.y, pi.vy);
+    BOTH VSUB(dvy[k], J[k].vy, pi.vy);
 #pragma unroll
-    BOTH VSUB(dvx[k], J[k].p1.x, pi.vx);
+    BOTH VSUB(dvx[k], J[k].vx, pi.vx);
 #pragma unroll
     BOTH VMUL(B[k], dvz[k], dvz[k]);
 #pragma unroll
-    BOTH VSUB(dz[k], J[k].p0.z, pi.z);
+    BOTH VSUB(dz[k], J[k].z, pi.z);
 #pragma unroll
-    BOTH VSUB(daz[k], J[k].p2.y, pi.az);
+    BOTH VSUB(daz[k], J[k].az, pi.az);
 #pragma unroll
     BOTH VFMA(B[k], dvy[k], dvy[k], B[k]);
 #pragma unroll
-    BOTH VSUB(dy[k], J[k].p0.y, pi.y);
+    BOTH VSUB(dy[k], J[k].y, pi.y);
 #pragma unroll
-    BOTH VSUB(day[k], J[k].p2.x, pi.ay);
+    BOTH VSUB(day[k], J[k].ay, pi.ay);
 #pragma unroll
     BOTH VFMA(B[k], dvx[k], dvx[k], B[k]);
 #pragma unroll
-    BOTH VSUB(dx[k], J[k].p0.x, pi.x);
+    BOTH VSUB(dx[k], J[k].x, pi.x);
 #pragma unroll
-    BOTH VSUB(dax[k], J[k].p1.w, pi.ax);
+    BOTH VSUB(dax[k], J[k].ax, pi.ax);
     // s = dx.dx + eps2, rv = dx.dv, B += dx.da: runs of three that share d_c in slot A
 #pragma unroll
     BOTH { VFMA(s[k], dz[k], dz[k], eps2); VMUL(rv[k], dz[k], dvz[k]); VFMA(B[k], dz[k], daz[k], B[k]); }
@@ -191,7 +148,7 @@ __device__ __forceinline__ void pair2(const IPart& pi, const JRec (&J)[2], const
 #pragma unroll
     BOTH VMUL(yy[k], y[k], y[k]);
 #pragma unroll
-    BOTH VMUL(mr[k], y[k], J[k].p0.w);
+    BOTH VMUL(mr[k], y[k], J[k].m);
 #pragma unroll
     BOTH VMUL(z[k], yy[k], -3.0);
 #pragma unroll
@@ -240,41 +197,20 @@ __device__ __forceinline__ void pair2(const IPart& pi, const JRec (&J)[2], const
 
 // ---------------------------------------------------------------------------------------------
 // 4th-order variant (R21): acceleration, jerk and potential only.  32 FP64-pipe instructions per
-// pair (17 DFMA + 8 DMUL + 7 DADD) + 1 MUFU.RSQ64H; the snap sums stay 0.
+// pair (17 DFMA + 8 DMUL + 7 DADD) + 1 MUFU.RSQ64H; the snap sums stay 0.  Two j-records at a time, FP64 instruction
+// order as in pair2 (the nine three-source DFMAs of a pair in one pinned run).
 // ---------------------------------------------------------------------------------------------
-template <bool EPS0, bool MASK = true>
-__device__ __forceinline__ void pair_o4(const IPart& pi, const double4 p0, const double4 p1, const double eps2, const bool self, Sums& S)
-{
-    const double dx = p0.x - pi.x, dy = p0.y - pi.y, dz = p0.z - pi.z;
-    const double dvx = p1.x - pi.vx, dvy = p1.y - pi.vy, dvz = p1.z - pi.vz;
-    double s = F(dx, dx, F(dy, dy, F(dz, dz, eps2)));
-    if (EPS0 && MASK) s = self ? 1.0 : s;
-    const double y0 = rsqrt_seed(s);
-    const double e = F(-s, M(y0, y0), 1.0);
-    const double y = F(M(y0, e), F(e, 0.375, 0.5), y0);
-    const double rv = F(dx, dvx, F(dy, dvy, M(dz, dvz)));
-    const double yy = M(y, y);
-    const double mr = M(y, p0.w);
-    const double q = M(yy, mr);
-    const double c1 = M(M(yy, -3.0), rv);                // -3 alpha
-    const double ux = F(c1, dx, dvx), uy = F(c1, dy, dvy), uz = F(c1, dz, dvz);
-    S.ax = F(q, dx, S.ax); S.ay = F(q, dy, S.ay); S.az = F(q, dz, S.az);
-    S.jx = F(q, ux, S.jx); S.jy = F(q, uy, S.jy); S.jz = F(q, uz, S.jz);
-    S.p += (MASK && self) ? 0.0 : mr;
-}
-
-// two j-records at a time, FP64 instruction order as in pair2 (the nine three-source DFMAs of a pair in one pinned run)
 template <bool EPS0, bool MASK>
 __device__ __forceinline__ void pair2_o4(const IPart& pi, const JRec (&J)[2], const double eps2, const bool (&self)[2], Sums& S)
 {
     double dx[2], dy[2], dz[2], dvx[2], dvy[2], dvz[2];
     double s[2], rv[2], y0[2], t[2], e[2], h[2], y[2], yy[2], mr[2], z[2], q[2], c1[2];
 #pragma unroll
-    BOTH { VSUB(dz[k], J[k].p0.z, pi.z); VSUB(dvz[k], J[k].p1.z, pi.vz); }
+    BOTH { VSUB(dz[k], J[k].z, pi.z); VSUB(dvz[k], J[k].vz, pi.vz); }
 #pragma unroll
-    BOTH { VSUB(dy[k], J[k].p0.y, pi.y); VSUB(dvy[k], J[k].p1.y, pi.vy); }
+    BOTH { VSUB(dy[k], J[k].y, pi.y); VSUB(dvy[k], J[k].vy, pi.vy); }
 #pragma unroll
-    BOTH { VSUB(dx[k], J[k].p0.x, pi.x); VSUB(dvx[k], J[k].p1.x, pi.vx); }
+    BOTH { VSUB(dx[k], J[k].x, pi.x); VSUB(dvx[k], J[k].vx, pi.vx); }
 #pragma unroll
     BOTH { VFMA(s[k], dz[k], dz[k], eps2); VMUL(rv[k], dz[k], dvz[k]); }
 #pragma unroll
@@ -300,7 +236,7 @@ __device__ __forceinline__ void pair2_o4(const IPart& pi, const JRec (&J)[2], co
 #pragma unroll
     BOTH VMUL(yy[k], y[k], y[k]);
 #pragma unroll
-    BOTH VMUL(mr[k], y[k], J[k].p0.w);
+    BOTH VMUL(mr[k], y[k], J[k].m);
 #pragma unroll
     BOTH VMUL(z[k], yy[k], -3.0);
 #pragma unroll
@@ -338,14 +274,13 @@ __device__ __forceinline__ void pair2_o4(const IPart& pi, const JRec (&J)[2], co
 // 84 FP64-pipe instructions per pair + 1 MUFU.RSQ64H; one pair at a time (ptxas schedules it; 2 x 12 differences would
 // not fit the register budget).
 // ---------------------------------------------------------------------------------------------
-template <bool EPS0, bool MASK = true>
-__device__ __forceinline__ void pair_o8(const IPart& pi, const double4 p0, const double4 p1, const double2 p2, const double4 p3,
-                                        const double eps2, const bool self, Sums& S)
+template <bool EPS0, bool MASK>
+__device__ __forceinline__ void pair_o8(const IPart& pi, const JRec& J, const double eps2, const bool self, Sums& S)
 {
-    const double dx = p0.x - pi.x, dy = p0.y - pi.y, dz = p0.z - pi.z;
-    const double dvx = p1.x - pi.vx, dvy = p1.y - pi.vy, dvz = p1.z - pi.vz;
-    const double dax = p1.w - pi.ax, day = p2.x - pi.ay, daz = p2.y - pi.az;
-    const double djx = p3.x - pi.jx, djy = p3.y - pi.jy, djz = p3.z - pi.jz;
+    const double dx = J.x - pi.x, dy = J.y - pi.y, dz = J.z - pi.z;
+    const double dvx = J.vx - pi.vx, dvy = J.vy - pi.vy, dvz = J.vz - pi.vz;
+    const double dax = J.ax - pi.ax, day = J.ay - pi.ay, daz = J.az - pi.az;
+    const double djx = J.jx - pi.jx, djy = J.jy - pi.jy, djz = J.jz - pi.jz;
     double s = F(dx, dx, F(dy, dy, F(dz, dz, eps2)));
     if (EPS0 && MASK) s = self ? 1.0 : s;
     const double y0 = rsqrt_seed(s);
@@ -359,7 +294,7 @@ __device__ __forceinline__ void pair_o8(const IPart& pi, const double4 p0, const
     const double T3 = F(va, 3.0, xj);
     const double yy = M(y, y);
     const double z = M(yy, -3.0);
-    const double mr = M(y, p0.w);
+    const double mr = M(y, J.m);
     const double q = M(yy, mr);
     const double alpha = M(yy, rv);
     const double c1 = M(z, rv);                          // -3 alpha
@@ -380,29 +315,47 @@ __device__ __forceinline__ void pair_o8(const IPart& pi, const double4 p0, const
     S.p += (MASK && self) ? 0.0 : mr;
 }
 
+// ---------------------------------------------------------------------------------------------
+// records: one predicted particle is Q = 5 (7 at the 8th order) double2, nb_internal.h
+// ---------------------------------------------------------------------------------------------
 template <int ORDER>
-__device__ __forceinline__ IPart load_ipart(const ForceArgs& A, int i)
+__device__ __forceinline__ JRec load_rec(const double2* r)
 {
-    const double4 a = A.pj0[i], b = A.pj1[i];
-    const double2 c = A.pj2[i];
-    IPart p{a.x, a.y, a.z, b.x, b.y, b.z, b.w, c.x, c.y, 0.0, 0.0, 0.0};
-    if (ORDER == 8) { const double4 d = A.pj3[i]; p.jx = d.x; p.jy = d.y; p.jz = d.z; }
-    return p;
+    const double2 a = r[0], b = r[1], c = r[2], d = r[3], e = r[4];
+    JRec J{a.x, a.y, b.x, b.y, c.x, c.y, d.x, d.y, e.x, e.y, 0.0, 0.0, 0.0};
+    if (ORDER == 8) { const double2 f = r[5], g = r[6]; J.jx = f.x; J.jy = f.y; J.jz = g.x; }
+    return J;
 }
 
-// partial planes are [plane][NC][ld] with NC = 10 (a, jerk, snap, pot), 13 at the 8th order (+ crackle)
+__device__ __forceinline__ IPart ipart_of(const JRec& J) { return IPart{J.x, J.y, J.z, J.vx, J.vy, J.vz, J.ax, J.ay, J.az, J.jx, J.jy, J.jz}; }
+
+// the i-particle's own predicted record: read from the record array, or predicted from the state with the predictor's
+// fma chain (bit-identical)
+template <int ORDER, bool PREDICT>
+__device__ __forceinline__ IPart load_ipart(const ForceArgs& A, int i)
+{
+    constexpr int Q = nb_rec_q(ORDER);
+    if (PREDICT) {
+        double2 r[Q];
+        nb_predict_record<ORDER>(nb_load_pstate<ORDER>(A.st0, A.st1, A.st2, A.st3, A.st4, A.st5, A.st6, i), A.t_pred, false, r);
+        return ipart_of(load_rec<ORDER>(r));
+    }
+    return ipart_of(load_rec<ORDER>(A.rec + (size_t)i * Q));
+}
+
+// partial planes are [slice][NC][ld] with NC = 10 (a, jerk, snap, pot), 13 at the 8th order (+ crackle)
 template <int ORDER>
-__device__ __forceinline__ void store_sums(const ForceArgs& A, int slice, int k, bool valid, const Sums& S)
+__device__ __forceinline__ void store_sums(const ForceArgs& A, int slice, int k, const Sums& S)
 {
     constexpr int NC = ORDER == 8 ? 13 : 10;
-    if (A.n_planes > 1) {
+    if (A.n_split > 1) {
         double* P = A.partial + (size_t)slice * NC * A.ld + k;      // plane (slice, c) is contiguous in k
         const size_t ld = A.ld;
         P[0] = S.ax; P[ld] = S.ay; P[2 * ld] = S.az;
         P[3 * ld] = S.jx; P[4 * ld] = S.jy; P[5 * ld] = S.jz;
         P[6 * ld] = S.sx; P[7 * ld] = S.sy; P[8 * ld] = S.sz; P[9 * ld] = S.p;
         if (ORDER == 8) { P[10 * ld] = S.cx; P[11 * ld] = S.cy; P[12 * ld] = S.cz; }
-    } else if (valid) {
+    } else {
         A.out_a[3 * k] = S.ax; A.out_a[3 * k + 1] = S.ay; A.out_a[3 * k + 2] = S.az;
         A.out_j[3 * k] = S.jx; A.out_j[3 * k + 1] = S.jy; A.out_j[3 * k + 2] = S.jz;
         A.out_s[3 * k] = S.sx; A.out_s[3 * k + 1] = S.sy; A.out_s[3 * k + 2] = S.sz;
@@ -440,19 +393,30 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
     } while (!done);
 }
 
-// Device-planned launch (nb_run_blocks): take the plan the scheduler left in device memory.  False: this kernel shape
-// is not the one the plan names (or the step is not taken) and the whole grid returns.
-__device__ __forceinline__ bool take_devplan(ForceArgs& A, int kernel_id)
+constexpr int N_BARS = WU_WARPS * WU_STAGES > LI_STAGES ? WU_WARPS * WU_STAGES : LI_STAGES;
+static_assert((LI_STAGES & (LI_STAGES - 1)) == 0 && (WU_STAGES & (WU_STAGES - 1)) == 0, "stage counts must be powers of two");
+static_assert(LI_TJ % 2 == 0 && WU_TJ == 64, "pair2 takes two j-records at a time; a warp predicts a tile as lane, lane + 32");
+
+__device__ __forceinline__ void init_barriers(unsigned long long* bars)
 {
-    if (!A.dp) return true;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < N_BARS; ++s) mbar_init(smem_u32(&bars[s]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+}
+
+// Device-planned launch (nb_run_blocks): take the plan the scheduler left in device memory.  False: the step is not taken.
+__device__ __forceinline__ bool take_devplan(ForceArgs& A)
+{
     const DevPlan* d = A.dp;
-    if (d->stop || d->kernel != kernel_id) return false;
+    if (d->stop) return false;
     A.n_act = d->n_act; A.n_units = d->n_units; A.n_split = d->n_split; A.slice_tiles = d->slice_tiles;
-    A.n_items = d->n_items; A.ld = d->ld; A.n_planes = d->n_planes;
+    A.n_items = d->n_items; A.ld = d->ld; A.predict = d->predict; A.t_pred = d->t_next;
     return true;
 }
 
-// The CTA (or warp) that finds the queue empty last puts both counters back to 0 for the next launch.
+// The worker that finds the queue empty last puts both counters back to 0 for the next launch.
 __device__ __forceinline__ void queue_retire(int* queue, int n_workers)
 {
     __threadfence();
@@ -460,47 +424,21 @@ __device__ __forceinline__ void queue_retire(int* queue, int n_workers)
 }
 
 // ---------------------------------------------------------------------------------------------
-// lanes-over-i
+// CTA tiles: a work item is (i-tile of 128 particles, j-slice)
 // ---------------------------------------------------------------------------------------------
-static_assert((LI_STAGES & (LI_STAGES - 1)) == 0, "LI_STAGES must be a power of two");
-static_assert(LI_TJ % 2 == 0, "pair2 takes two j-records at a time");
-
-// W = 1: a work item is (i-tile of LI_THREADS particles, j-slice).  W = 4 (17..96 active particles): the CTA's four
-// warps hold the SAME 32 particles and each takes its own quarter of every j-tile, so an item is (32 particles,
-// j-slice) and writes four partial planes (slice * 4 + warp) that the reduction adds like any other slices.
-template <bool EPS0, int W, int ORDER>
-__global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(const ForceArgs A_)
+template <bool EPS0, int ORDER>
+__device__ __forceinline__ void li_body(const ForceArgs& A, double2* smem, unsigned long long* full)
 {
-    ForceArgs A = A_;
-    if (!take_devplan(A, W == 1 ? 0 : 2)) return;
-    constexpr int UNIT = LI_UNIT / W;                      // active particles per work item
-    constexpr int TJW = LI_TJ / W;                         // records of each j-tile one warp group takes
-    static_assert(W == 1 || (LI_I == 1 && UNIT == 32 && TJW % 2 == 0), "W > 1: one warp per group");
-    __shared__ alignas(128) double4 s0[LI_STAGES][LI_TJ];
-    __shared__ alignas(128) double4 s1[LI_STAGES][LI_TJ];
-    __shared__ alignas(128) double2 s2[LI_STAGES][LI_TJ];
-    __shared__ alignas(128) double4 s3[LI_STAGES][ORDER == 8 ? LI_TJ : 1];   // predicted jerk, 8th order only
-    __shared__ alignas(8) unsigned long long full[LI_STAGES];
+    constexpr int Q = nb_rec_q(ORDER);
+    constexpr uint32_t TILE_BYTES = LI_TJ * Q * 16;
     __shared__ int next_item;
-
     const int tid = threadIdx.x;
-    const int wg = W == 1 ? 0 : tid / UNIT;                // warp group: which part of each j-tile
-    const int til = W == 1 ? tid : tid % UNIT;             // lane within the i-tile
-    if (tid == 0) {
-        for (int s = 0; s < LI_STAGES; ++s) mbar_init(smem_u32(&full[s]), 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
 
-    // one elected thread stages j-tile `tile` into stage `st`: three bulk copies, one barrier
+    // one elected thread stages j-tile `tile` into stage `st`: one bulk copy, one barrier
     auto stage_tile = [&](int tile, int st) {
         const uint32_t bar = smem_u32(&full[st]);
-        const size_t j0 = (size_t)tile * LI_TJ;
-        mbar_expect_tx(bar, LI_TJ * (ORDER == 8 ? 112 : 80));
-        bulk_g2s(smem_u32(&s0[st][0]), A.pj0 + j0, LI_TJ * 32, bar);
-        bulk_g2s(smem_u32(&s1[st][0]), A.pj1 + j0, LI_TJ * 32, bar);
-        bulk_g2s(smem_u32(&s2[st][0]), A.pj2 + j0, LI_TJ * 16, bar);
-        if (ORDER == 8) bulk_g2s(smem_u32(&s3[st][0]), A.pj3 + j0, LI_TJ * 32, bar);
+        mbar_expect_tx(bar, TILE_BYTES);
+        bulk_g2s(smem_u32(smem + (size_t)st * LI_TJ * Q), A.rec + (size_t)tile * LI_TJ * Q, TILE_BYTES, bar);
     };
 
     uint32_t uses = 0;   // j-tiles this CTA has consumed so far: stage = uses % STAGES, parity = (uses / STAGES) & 1
@@ -517,153 +455,217 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
         if (tid == 0)
             for (int f = 0; f < LI_STAGES && f < nt; ++f) stage_tile(t0 + f, (uses + f) & (LI_STAGES - 1));
 
-        int ii[LI_I];
-        bool valid[LI_I];
-        IPart pi[LI_I];
-        Sums acc[LI_I];
-#pragma unroll
-        for (int q = 0; q < LI_I; ++q) {
-            const int k = unit * UNIT + q * LI_THREADS + til;
-            valid[q] = k < A.n_act;
-            const int kk = valid[q] ? k : 0;
-            ii[q] = A.idx ? A.idx[kk] : kk;
-            pi[q] = load_ipart<ORDER>(A, ii[q]);
-            acc[q] = Sums{0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
-        }
+        const int k = unit * LI_UNIT + tid;
+        const bool valid = k < A.n_act;
+        const int kk = valid ? k : 0;
+        const int ii = A.idx ? A.idx[kk] : kk;
+        const IPart pi = load_ipart<ORDER, false>(A, ii);
+        Sums acc{0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
 
         for (int t = 0; t < nt; ++t) {
             const uint32_t u = uses + t;
             const int st = u & (LI_STAGES - 1);
             mbar_wait(smem_u32(&full[st]), (u / LI_STAGES) & 1);
-            const int jbase = (t0 + t) * LI_TJ + wg * TJW;
+            const int jbase = (t0 + t) * LI_TJ;
             // the self pair (reading R4) lies in one j-tile per particle: only a warp that has one of its own
             // particles in this tile runs the loop that masks by index
-            bool own = false;
-#pragma unroll
-            for (int q = 0; q < LI_I; ++q) own |= (unsigned)(ii[q] - jbase) < (unsigned)TJW;
-            const double4 *t0p = &s0[st][wg * TJW], *t1p = &s1[st][wg * TJW];
-            const double2* t2p = &s2[st][wg * TJW];
+            const bool own = (unsigned)(ii - jbase) < (unsigned)LI_TJ;
+            const double2* tp = smem + (size_t)st * LI_TJ * Q;
             if (ORDER == 8) {
-                const double4* t3p = &s3[st][ORDER == 8 ? wg * TJW : 0];
                 if (__any_sync(0xffffffffu, own)) {
 #pragma unroll 2
-                    for (int jj = 0; jj < TJW; ++jj) {
-#pragma unroll
-                        for (int q = 0; q < LI_I; ++q)
-                            pair_o8<EPS0, true>(pi[q], t0p[jj], t1p[jj], t2p[jj], t3p[jj], A.eps2, jbase + jj == ii[q], acc[q]);
-                    }
+                    for (int jj = 0; jj < LI_TJ; ++jj) pair_o8<EPS0, true>(pi, load_rec<ORDER>(tp + jj * Q), A.eps2, jbase + jj == ii, acc);
                 } else {
 #pragma unroll 2
-                    for (int jj = 0; jj < TJW; ++jj) {
-#pragma unroll
-                        for (int q = 0; q < LI_I; ++q) pair_o8<EPS0, false>(pi[q], t0p[jj], t1p[jj], t2p[jj], t3p[jj], A.eps2, false, acc[q]);
-                    }
+                    for (int jj = 0; jj < LI_TJ; ++jj) pair_o8<EPS0, false>(pi, load_rec<ORDER>(tp + jj * Q), A.eps2, false, acc);
                 }
             } else if (__any_sync(0xffffffffu, own)) {
 #pragma unroll 1
-                for (int jj = 0; jj < TJW; jj += 2) {
-                    const JRec J[2] = {{t0p[jj], t1p[jj], t2p[jj]}, {t0p[jj + 1], t1p[jj + 1], t2p[jj + 1]}};
-#pragma unroll
-                    for (int q = 0; q < LI_I; ++q) {
-                        const bool self[2] = {jbase + jj == ii[q], jbase + jj + 1 == ii[q]};
-                        if (ORDER == 4) pair2_o4<EPS0, true>(pi[q], J, A.eps2, self, acc[q]);
-                        else pair2<EPS0, true>(pi[q], J, A.eps2, self, acc[q]);
-                    }
+                for (int jj = 0; jj < LI_TJ; jj += 2) {
+                    const JRec J[2] = {load_rec<ORDER>(tp + jj * Q), load_rec<ORDER>(tp + (jj + 1) * Q)};
+                    const bool self[2] = {jbase + jj == ii, jbase + jj + 1 == ii};
+                    if (ORDER == 4) pair2_o4<EPS0, true>(pi, J, A.eps2, self, acc);
+                    else pair2<EPS0, true>(pi, J, A.eps2, self, acc);
                 }
             } else {
 #pragma unroll 1
-                for (int jj = 0; jj < TJW; jj += 2) {
-                    const JRec J[2] = {{t0p[jj], t1p[jj], t2p[jj]}, {t0p[jj + 1], t1p[jj + 1], t2p[jj + 1]}};
+                for (int jj = 0; jj < LI_TJ; jj += 2) {
+                    const JRec J[2] = {load_rec<ORDER>(tp + jj * Q), load_rec<ORDER>(tp + (jj + 1) * Q)};
                     const bool self[2] = {false, false};
-#pragma unroll
-                    for (int q = 0; q < LI_I; ++q) {
-                        if (ORDER == 4) pair2_o4<EPS0, false>(pi[q], J, A.eps2, self, acc[q]);
-                        else pair2<EPS0, false>(pi[q], J, A.eps2, self, acc[q]);
-                    }
+                    if (ORDER == 4) pair2_o4<EPS0, false>(pi, J, A.eps2, self, acc);
+                    else pair2<EPS0, false>(pi, J, A.eps2, self, acc);
                 }
             }
             __syncthreads();                                   // every warp is done with stage st
             if (tid == 0 && t + LI_STAGES < nt) stage_tile(t0 + t + LI_STAGES, st);
         }
         uses += nt;
-
-#pragma unroll
-        for (int q = 0; q < LI_I; ++q) store_sums<ORDER>(A, slice * W + wg, unit * UNIT + q * LI_THREADS + til, valid[q], acc[q]);
+        if (valid || A.n_split > 1) store_sums<ORDER>(A, slice, k, acc);
     }
     if (tid == 0) queue_retire(A.queue, gridDim.x);
 }
 
 // ---------------------------------------------------------------------------------------------
-// lanes-over-j
+// warp units: a work item is (unit of p particles, j-slice), one warp per item
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ double warp_sum(double v)
+template <bool EPS0, int ORDER, bool PREDICT>
+__device__ __forceinline__ void wu_body(const ForceArgs& A, double2* smem, unsigned long long* full_all)
 {
+    constexpr int Q = nb_rec_q(ORDER);
+    constexpr uint32_t TILE_BYTES = WU_TJ * Q * 16;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double2* ring = smem + (size_t)warp * WU_STAGES * WU_TJ * Q;        // this warp's private stages
+    unsigned long long* full = full_all + warp * WU_STAGES;
+
+    auto stage_tile = [&](int tile, int st) {                          // lane 0 only
+        const uint32_t bar = smem_u32(&full[st]);
+        mbar_expect_tx(bar, TILE_BYTES);
+        bulk_g2s(smem_u32(ring + (size_t)st * WU_TJ * Q), A.rec + (size_t)tile * WU_TJ * Q, TILE_BYTES, bar);
+    };
+
+    const int n_workers = gridDim.x * WU_WARPS;
+    const bool queued = A.n_items > n_workers;              // at most one item per warp: no queue traffic at all
+    uint32_t uses = 0;
+    for (int round = 0;; ++round) {
+        int item;
+        if (queued) {
+            item = 0;
+            if (lane == 0) item = atomicAdd(A.queue, 1);
+            item = __shfl_sync(0xffffffffu, item, 0);
+        } else {
+            item = round == 0 ? (int)(blockIdx.x * WU_WARPS + warp) : A.n_items;
+        }
+        if (item >= A.n_items) break;
+        const int unit = item % A.n_units, slice = item / A.n_units;
+        const int t0 = slice * A.slice_tiles;
+        const int nt = min(A.slice_tiles, A.n_tiles - t0);
+        if (!PREDICT && lane == 0)
+            for (int f = 0; f < WU_STAGES && f < nt; ++f) stage_tile(t0 + f, (uses + f) & (WU_STAGES - 1));
+
+        // lanes: p ways over the unit's particles, LJ = 32 / p ways over the records of a step
+        int k0, p, nvalid;
+        nb_wu_unit(A.n_act, unit, &k0, &p, &nvalid);
+        const int LJ = 32 / p;                              // powers of two
+        const int lj = lane & (LJ - 1), part = lane >> (__ffs(LJ) - 1);
+        const bool valid = part < nvalid;
+        const int k = k0 + (valid ? part : 0);
+        const int ii = A.idx ? A.idx[k] : k;
+        const IPart pi = load_ipart<ORDER, PREDICT>(A, ii);
+        Sums acc{0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+
+        for (int t = 0; t < nt; ++t) {
+            const int jbase = (t0 + t) * WU_TJ;
+            const double2* tp;
+            if (PREDICT) {
+                // the warp predicts this tile's 64 records itself: lane -> records lane and lane + 32
+                tp = ring;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
+                for (int h = 0; h < 2; ++h) {
+                    const int r = lane + 32 * h;
+                    double2 rec[Q];
+                    nb_predict_record<ORDER>(nb_load_pstate<ORDER>(A.st0, A.st1, A.st2, A.st3, A.st4, A.st5, A.st6, jbase + r), A.t_pred, false, rec);
+#pragma unroll
+                    for (int q = 0; q < Q; ++q) ring[r * Q + q] = rec[q];
+                }
+                __syncwarp();
+            } else {
+                const uint32_t u = uses + t;
+                const int st = u & (WU_STAGES - 1);
+                mbar_wait(smem_u32(&full[st]), (u / WU_STAGES) & 1);
+                tp = ring + (size_t)st * WU_TJ * Q;
+            }
+            // the self pair (reading R4) lies in one j-tile per particle
+            const bool own = (unsigned)(ii - jbase) < (unsigned)WU_TJ;
+            const double2* lp = tp + lj * Q;                 // this lane's first record of the tile; a step advances LJ records
+            const int jl = jbase + lj;
+            if (ORDER == 8) {
+                if (__any_sync(0xffffffffu, own)) {
+#pragma unroll 1
+                    for (int r = 0; r < WU_TJ; r += LJ) pair_o8<EPS0, true>(pi, load_rec<ORDER>(lp + r * Q), A.eps2, jl + r == ii, acc);
+                } else {
+#pragma unroll 1
+                    for (int r = 0; r < WU_TJ; r += LJ) pair_o8<EPS0, false>(pi, load_rec<ORDER>(lp + r * Q), A.eps2, false, acc);
+                }
+            } else if (__any_sync(0xffffffffu, own)) {
+#pragma unroll 1
+                for (int r = 0; r < WU_TJ; r += 2 * LJ) {
+                    const JRec J[2] = {load_rec<ORDER>(lp + r * Q), load_rec<ORDER>(lp + (r + LJ) * Q)};
+                    const bool self[2] = {jl + r == ii, jl + r + LJ == ii};
+                    if (ORDER == 4) pair2_o4<EPS0, true>(pi, J, A.eps2, self, acc);
+                    else pair2<EPS0, true>(pi, J, A.eps2, self, acc);
+                }
+            } else {
+#pragma unroll 1
+                for (int r = 0; r < WU_TJ; r += 2 * LJ) {
+                    const JRec J[2] = {load_rec<ORDER>(lp + r * Q), load_rec<ORDER>(lp + (r + LJ) * Q)};
+                    const bool self[2] = {false, false};
+                    if (ORDER == 4) pair2_o4<EPS0, false>(pi, J, A.eps2, self, acc);
+                    else pair2<EPS0, false>(pi, J, A.eps2, self, acc);
+                }
+            }
+            __syncwarp();                                      // every lane is done with the stage
+            if (!PREDICT && lane == 0 && t + WU_STAGES < nt) stage_tile(t0 + t + WU_STAGES, (uses + t) & (WU_STAGES - 1));
+        }
+        uses += nt;
+
+        // the LJ lane sums of a particle: shuffle butterfly in a fixed order (the "warp-shuffle reduction" of the north star)
+        for (int o = LJ >> 1; o > 0; o >>= 1) {
+            acc.ax += __shfl_xor_sync(0xffffffffu, acc.ax, o); acc.ay += __shfl_xor_sync(0xffffffffu, acc.ay, o);
+            acc.az += __shfl_xor_sync(0xffffffffu, acc.az, o); acc.jx += __shfl_xor_sync(0xffffffffu, acc.jx, o);
+            acc.jy += __shfl_xor_sync(0xffffffffu, acc.jy, o); acc.jz += __shfl_xor_sync(0xffffffffu, acc.jz, o);
+            acc.p += __shfl_xor_sync(0xffffffffu, acc.p, o);
+            if (ORDER != 4) {
+                acc.sx += __shfl_xor_sync(0xffffffffu, acc.sx, o); acc.sy += __shfl_xor_sync(0xffffffffu, acc.sy, o);
+                acc.sz += __shfl_xor_sync(0xffffffffu, acc.sz, o);
+            }
+            if (ORDER == 8) {
+                acc.cx += __shfl_xor_sync(0xffffffffu, acc.cx, o); acc.cy += __shfl_xor_sync(0xffffffffu, acc.cy, o);
+                acc.cz += __shfl_xor_sync(0xffffffffu, acc.cz, o);
+            }
+        }
+        if (lj == 0 && valid) store_sums<ORDER>(A, slice, k, acc);
+    }
+    if (queued && lane == 0) queue_retire(A.queue, n_workers);
+}
+
+// ---------------------------------------------------------------------------------------------
+// kernels: one per shape for nb_force (the host planned the launch), and one that holds both shapes and takes the
+// plan from device memory (nb_run_blocks: one force launch per block step whatever the scheduler found)
+// ---------------------------------------------------------------------------------------------
+extern __shared__ __align__(128) double2 dyn_smem[];
+
+template <bool EPS0, int ORDER>
+__global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(const ForceArgs A)
+{
+    __shared__ alignas(8) unsigned long long bars[N_BARS];
+    init_barriers(bars);
+    li_body<EPS0, ORDER>(A, dyn_smem, bars);
 }
 
 template <bool EPS0, int ORDER>
-__global__ void __launch_bounds__(LJ_THREADS, ORDER == 8 ? 1 : LJ_CTAS_PER_SM) force_lj_kernel(const ForceArgs A_)
+__global__ void __launch_bounds__(WU_THREADS, WU_CTAS_PER_SM) force_wu_kernel(const ForceArgs A)
 {
+    __shared__ alignas(8) unsigned long long bars[N_BARS];
+    init_barriers(bars);
+    wu_body<EPS0, ORDER, false>(A, dyn_smem, bars);
+}
+
+static_assert(LI_THREADS == WU_THREADS && LI_CTAS_PER_SM == WU_CTAS_PER_SM, "the block-step kernel runs either shape in one launch");
+
+template <bool EPS0, int ORDER>
+__global__ void __launch_bounds__(WU_THREADS, WU_CTAS_PER_SM) force_step_kernel(const ForceArgs A_)
+{
+    __shared__ alignas(8) unsigned long long bars[N_BARS];
     ForceArgs A = A_;
-    if (!take_devplan(A, 1)) return;
-    const int lane = threadIdx.x & 31;
-    for (;;) {
-        int wi = 0;
-        if (lane == 0) wi = atomicAdd(A.queue, 1);
-        wi = __shfl_sync(0xffffffffu, wi, 0);
-        if (wi >= A.n_items) break;
-        const int unit = wi % A.n_units, slice = wi / A.n_units;
-        const int t0 = slice * A.slice_tiles;
-        const int nt = min(A.slice_tiles, A.n_tiles - t0);
-
-        int ii[LJ_I];
-        bool valid[LJ_I];
-        IPart pi[LJ_I];
-        Sums acc[LJ_I];
-#pragma unroll
-        for (int q = 0; q < LJ_I; ++q) {
-            const int k = unit * LJ_I + q;
-            valid[q] = k < A.n_act;
-            const int kk = valid[q] ? k : 0;
-            ii[q] = A.idx ? A.idx[kk] : kk;
-            pi[q] = load_ipart<ORDER>(A, ii[q]);
-            acc[q] = Sums{0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
-        }
-
-        int j = t0 * LJ_TJ + lane;
-        double4 n0 = A.pj0[j], n1 = A.pj1[j];
-        double2 n2 = A.pj2[j];
-        double4 n3 = ORDER == 8 ? A.pj3[j] : make_double4(0, 0, 0, 0);
-        for (int t = 0; t < nt; ++t) {
-            const double4 p0 = n0, p1 = n1, p3 = n3;
-            const double2 p2 = n2;
-            if (t + 1 < nt) {                                                                            // prefetch
-                n0 = A.pj0[j + LJ_TJ]; n1 = A.pj1[j + LJ_TJ]; n2 = A.pj2[j + LJ_TJ];
-                if (ORDER == 8) n3 = A.pj3[j + LJ_TJ];
-            }
-#pragma unroll
-            for (int q = 0; q < LJ_I; ++q) {
-                if (ORDER == 4) pair_o4<EPS0>(pi[q], p0, p1, A.eps2, j == ii[q], acc[q]);
-                else if (ORDER == 8) pair_o8<EPS0>(pi[q], p0, p1, p2, p3, A.eps2, j == ii[q], acc[q]);
-                else pair<EPS0>(pi[q], p0, p1, p2, A.eps2, j == ii[q], acc[q]);
-            }
-            j += LJ_TJ;
-        }
-
-#pragma unroll
-        for (int q = 0; q < LJ_I; ++q) {
-            Sums& S = acc[q];
-            S.ax = warp_sum(S.ax); S.ay = warp_sum(S.ay); S.az = warp_sum(S.az);
-            S.jx = warp_sum(S.jx); S.jy = warp_sum(S.jy); S.jz = warp_sum(S.jz);
-            S.sx = warp_sum(S.sx); S.sy = warp_sum(S.sy); S.sz = warp_sum(S.sz);
-            S.p = warp_sum(S.p);
-            if (ORDER == 8) { S.cx = warp_sum(S.cx); S.cy = warp_sum(S.cy); S.cz = warp_sum(S.cz); }
-            if (lane == 0) store_sums<ORDER>(A, slice, unit * LJ_I + q, valid[q], S);
-        }
-    }
-    if (lane == 0) queue_retire(A.queue, gridDim.x * LJ_WARPS);
+    if (!take_devplan(A)) return;
+    const int kernel = A.dp->kernel;
+    A.n_tiles = kernel == 0 ? A.n_tiles * (WU_TJ) / LI_TJ : A.n_tiles;      // the host passes Npad / WU_TJ
+    // CTAs (warps) beyond the work return before any set-up; with a queue the retire count needs every worker
+    if (kernel == 1 && A.n_items <= (int)(gridDim.x * WU_WARPS) && (int)(blockIdx.x * WU_WARPS) >= A.n_items) return;
+    init_barriers(bars);
+    if (kernel == 0) li_body<EPS0, ORDER>(A, dyn_smem, bars);
+    else if (A.predict) wu_body<EPS0, ORDER, true>(A, dyn_smem, bars);
+    else wu_body<EPS0, ORDER, false>(A, dyn_smem, bars);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -673,15 +675,9 @@ __global__ void __launch_bounds__(LJ_THREADS, ORDER == 8 ? 1 : LJ_CTAS_PER_SM) f
 // slices (large active sets, few slices: the loads of neighbouring threads coalesce over k).
 // ---------------------------------------------------------------------------------------------
 template <int NC>
-__global__ void __launch_bounds__(RED_THREADS) reduce_partials_kernel(const ForceArgs A_, int T)
+__global__ void __launch_bounds__(RED_THREADS) reduce_partials_kernel(const ForceArgs A, int T)
 {
     __shared__ double sm[NC][RED_THREADS];
-    ForceArgs A = A_;
-    if (A.dp) {                                            // device-planned: any kernel shape, T from the plan
-        if (A.dp->stop) return;
-        A.n_act = A.dp->n_act; A.ld = A.dp->ld; A.n_planes = A.dp->n_planes; T = A.dp->red_T;
-        if (A.n_planes <= 1) return;                       // the force kernel wrote the results itself
-    }
     const int R = RED_THREADS / T;                         // active particles per block and pass
     const int kl = threadIdx.x % R, lane = threadIdx.x / R;
     for (int k0 = blockIdx.x * R; k0 < A.n_act; k0 += gridDim.x * R) {      // uniform over the block
@@ -692,7 +688,7 @@ __global__ void __launch_bounds__(RED_THREADS) reduce_partials_kernel(const Forc
         if (k < A.n_act) {
             const size_t plane = (size_t)NC * A.ld;
             const double* P = A.partial + (size_t)lane * plane + k;
-            for (int s = lane; s < A.n_planes; s += T, P += (size_t)T * plane) {
+            for (int s = lane; s < A.n_split; s += T, P += (size_t)T * plane) {
 #pragma unroll
                 for (int c = 0; c < NC; ++c) r[c] += P[(size_t)c * A.ld];
             }
@@ -718,6 +714,10 @@ __global__ void __launch_bounds__(RED_THREADS) reduce_partials_kernel(const Forc
     }
 }
 
+constexpr size_t li_smem(int order) { return (size_t)LI_STAGES * LI_TJ * nb_rec_q(order) * 16; }
+constexpr size_t wu_smem(int order) { return (size_t)WU_WARPS * WU_STAGES * WU_TJ * nb_rec_q(order) * 16; }
+constexpr size_t step_smem(int order) { return li_smem(order) > wu_smem(order) ? li_smem(order) : wu_smem(order); }
+
 }  // namespace
 
 // kernel instantiation for (eps == 0, order)
@@ -728,22 +728,36 @@ __global__ void __launch_bounds__(RED_THREADS) reduce_partials_kernel(const Forc
         else                 { if (eps_is_zero) { CALL(true, 6); } else { CALL(false, 6); } } \
     } while (0)
 
+// dynamic shared memory above 48 KiB has to be allowed per kernel (warp units at the 8th order: 56 KiB)
+cudaError_t nb_force_setup()
+{
+    cudaError_t e = cudaSuccess;
+    const bool eps_is_zero_values[2] = {false, true};
+    for (int order : {4, 6, 8})
+        for (bool eps_is_zero : eps_is_zero_values) {
+#define SETUP(E, O)                                                                                                              \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(force_li_kernel<E, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)li_smem(O)); \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(force_wu_kernel<E, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wu_smem(O)); \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(force_step_kernel<E, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)step_smem(O))
+            NB_DISPATCH(SETUP);
+#undef SETUP
+        }
+    return e;
+}
+
 cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps_is_zero, int order, cudaStream_t st, int* launches)
 {
-#define LI1(E, O) force_li_kernel<E, 1, O><<<plan.grid, LI_THREADS, 0, st>>>(args)
-#define LIW(E, O) force_li_kernel<E, LI_W, O><<<plan.grid, LI_THREADS, 0, st>>>(args)
-#define LJ(E, O) force_lj_kernel<E, O><<<plan.grid, LJ_THREADS, 0, st>>>(args)
-    if (plan.kernel == 0) NB_DISPATCH(LI1);
-    else if (plan.kernel == 2) NB_DISPATCH(LIW);
-    else NB_DISPATCH(LJ);
-#undef LI1
-#undef LIW
-#undef LJ
+#define LI(E, O) force_li_kernel<E, O><<<plan.grid, LI_THREADS, li_smem(O), st>>>(args)
+#define WU(E, O) force_wu_kernel<E, O><<<plan.grid, WU_THREADS, wu_smem(O), st>>>(args)
+    if (plan.kernel == 0) NB_DISPATCH(LI);
+    else NB_DISPATCH(WU);
+#undef LI
+#undef WU
     ++*launches;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    if (args.n_planes > 1) {
-        const int T = nb_reduce_threads(args.n_act, args.n_planes);
+    if (args.n_split > 1) {
+        const int T = nb_reduce_threads(args.n_act, args.n_split);
         const int R = RED_THREADS / T;
         if (order == 8) reduce_partials_kernel<13><<<(args.n_act + R - 1) / R, RED_THREADS, 0, st>>>(args, T);
         else reduce_partials_kernel<10><<<(args.n_act + R - 1) / R, RED_THREADS, 0, st>>>(args, T);
@@ -755,23 +769,18 @@ cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps
 
 cudaError_t nb_launch_force_devplan(const ForceArgs& args_, bool eps_is_zero, int order, int n_sm, int Npad, cudaStream_t st, int* launches)
 {
-    ForceArgs args = args_, args_lj = args_;
-    args.n_tiles = Npad / LI_TJ; args_lj.n_tiles = Npad / LJ_TJ;
-    const int g_li = n_sm * LI_CTAS_PER_SM, g_lj = n_sm * LJ_CTAS_PER_SM;
-#define ALL3(E, O)                                                      \
-    force_lj_kernel<E, O><<<g_lj, LJ_THREADS, 0, st>>>(args_lj);        \
-    force_li_kernel<E, LI_W, O><<<g_li, LI_THREADS, 0, st>>>(args);     \
-    force_li_kernel<E, 1, O><<<g_li, LI_THREADS, 0, st>>>(args)
-    NB_DISPATCH(ALL3);
-#undef ALL3
-    if (order == 8) reduce_partials_kernel<13><<<n_sm * 4, RED_THREADS, 0, st>>>(args, 1);
-    else reduce_partials_kernel<10><<<n_sm * 4, RED_THREADS, 0, st>>>(args, 1);
-    *launches += 4;
+    ForceArgs args = args_;
+    args.n_tiles = Npad / WU_TJ;
+    const int grid = n_sm * WU_CTAS_PER_SM;
+#define STEP(E, O) force_step_kernel<E, O><<<grid, WU_THREADS, step_smem(O), st>>>(args)
+    NB_DISPATCH(STEP);
+#undef STEP
+    *launches += 1;
     return cudaGetLastError();
 }
 
-void nb_force_occupancy(int* li, int* lj)
+void nb_force_occupancy(int* li, int* wu)
 {
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(li, force_li_kernel<false, 1, 6>, LI_THREADS, 0);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(lj, force_lj_kernel<false, 6>, LJ_THREADS, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(li, force_li_kernel<false, 6>, LI_THREADS, li_smem(6));
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(wu, force_wu_kernel<false, 6>, WU_THREADS, wu_smem(6));
 }

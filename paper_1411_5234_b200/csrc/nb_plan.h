@@ -16,11 +16,68 @@ NB_HD int64_t nb_pad_n(int64_t N) { return (N + NB_PAD - 1) / NB_PAD * NB_PAD; }
 NB_HD int64_t nb_partial_rows(int64_t Npad) { return 8 * Npad + (int64_t(1) << 19); }   // rows of each partial-sum plane
 NB_HD int64_t nb_min64(int64_t a, int64_t b) { return a < b ? a : b; }
 NB_HD int64_t nb_max64(int64_t a, int64_t b) { return a > b ? a : b; }
+NB_HD int nb_pow2ceil(int v) { int p = 1; while (p < v) p <<= 1; return p; }
+NB_HD int nb_pow2floor(int v) { int p = 1; while (2 * p <= v) p <<= 1; return p; }
+
+// n_act at and above which the evaluation runs as CTA tiles of 128 particles (kernel 0); below, as warp units (kernel 1)
+#ifdef NB_EXP_LI_MIN_ACT   /* TEMPORARY experiment switch, removed before commit */
+constexpr int64_t LI_MIN_ACT = NB_EXP_LI_MIN_ACT;
+#else
+constexpr int64_t LI_MIN_ACT = 16384;
+#endif
+// block steps whose evaluation has at most this many warp units let the force kernel predict the j-records itself
+constexpr int PIF_MAX_UNITS = 2;
+
+// ---------------------------------------------------------------------------------------------------------------
+// Warp units (kernel 1).  n_act = 32 n_full + rem.  The first n_full units hold 32 particles each.  The remainder is
+// decomposed from its highest bit down into units of p = 16, 8, ... 1 particles, every one full, EXCEPT that a rest
+// which nearly fills the next power of two (at most a quarter of it missing) becomes one padded unit: 31 -> one unit
+// of 32 with 31 valid lanes rather than 16 + 8 + 4 + 2 + 1 (five units, each streaming all j-records).
+// unit u -> first row k0, width p (lanes are split p ways over particles, 32/p ways over the records of a step) and
+// the number of valid particles.
+// ---------------------------------------------------------------------------------------------------------------
+NB_HD void nb_wu_rest_step(int rem, int* p, int* valid)
+{
+    const int pc = nb_pow2ceil(rem);
+    if (pc - rem <= pc / 4) { *p = pc; *valid = rem; }
+    else { *p = nb_pow2floor(rem); *valid = *p; }
+}
+
+NB_HD void nb_wu_unit(int n_act, int u, int* k0, int* p, int* valid)
+{
+    const int n_full = n_act >> 5;
+    if (u < n_full) { *k0 = u << 5; *p = 32; *valid = 32; return; }
+    int rem = n_act & 31, k = n_full << 5;
+    for (int idx = u - n_full;; --idx) {
+        nb_wu_rest_step(rem, p, valid);
+        if (idx == 0) { *k0 = k; return; }
+        k += *valid; rem -= *valid;
+    }
+}
+
+// number of units; *work = sum of p / 32 (units weighted by the time a slice costs them), *w_max = the largest weight
+NB_HD int nb_wu_count(int64_t n_act, double* work, double* w_max)
+{
+    const int n_full = (int)(n_act >> 5);
+    int n = n_full, rem = (int)(n_act & 31);
+    double w = (double)n_full, wm = n_full ? 1.0 : 0.0;
+    while (rem > 0) {
+        int p, valid;
+        nb_wu_rest_step(rem, &p, &valid);
+        w += p / 32.0;
+        if (p / 32.0 > wm) wm = p / 32.0;
+        rem -= valid; ++n;
+    }
+    *work = w; *w_max = wm;
+    return n;
+}
 
 // Everything about a plan except the split S.
 struct PlanShape {
-    int kernel;        // 0 lanes-over-i, 1 lanes-over-j, 2 lanes-over-i with 32-particle units (nb.h: nb_plan.kernel)
-    int unit, tile, sub, ctas_per_sm, fixed;
+    int kernel;        // 0 CTA tiles of 128 particles, 1 warp units (nb.h: nb_plan.kernel)
+    int unit, tile, ctas_per_sm;
+    double fixed;      // cost of starting a work item, in j-tiles of a full unit
+    double work, w_max;   // kernel 1: sum and maximum of the unit weights p / 32; kernel 0: n_units, 1
     int64_t n_units, n_tiles, resident, s_max;
 };
 
@@ -29,23 +86,21 @@ NB_HD PlanShape nb_plan_shape(int64_t Npad, int64_t n_act, int n_sm, int64_t max
 {
     PlanShape p;
     const int64_t rows = nb_partial_rows(Npad);
-    if (n_act <= LJ_MAX_ACT) {
-        // lanes-over-j: a work item is (warp i-group, j-slice); resident = warps on the device
-        p.kernel = 1; p.unit = LJ_I; p.tile = LJ_TJ; p.sub = 1; p.ctas_per_sm = LJ_CTAS_PER_SM; p.fixed = 6;
-        p.n_units = (n_act + LJ_I - 1) / LJ_I;
-        p.n_tiles = Npad / LJ_TJ;
-        p.resident = (int64_t)n_sm * LJ_CTAS_PER_SM * LJ_WARPS;
-        p.s_max = nb_min64(rows / (p.n_units * LJ_I), p.n_tiles / 4);
-    } else {
-        // lanes-over-i: a work item is (i-tile, j-slice); resident = CTAs on the device.  Up to LIW_MAX_ACT active
-        // particles the i-tile is 32 particles and the CTA's warps each take a part of every j-tile (sub > 1).
-        const bool small = n_act <= LIW_MAX_ACT;
-        p.kernel = small ? 2 : 0; p.sub = small ? LI_W : 1;
-        p.unit = LI_UNIT / p.sub; p.tile = LI_TJ; p.ctas_per_sm = LI_CTAS_PER_SM; p.fixed = 2;
-        p.n_units = (n_act + p.unit - 1) / p.unit;
+    if (n_act >= LI_MIN_ACT) {
+        // CTA tiles: a work item is (i-tile of 128 particles, j-slice); resident = CTAs on the device
+        p.kernel = 0; p.unit = LI_UNIT; p.tile = LI_TJ; p.ctas_per_sm = LI_CTAS_PER_SM; p.fixed = 2.0;
+        p.n_units = (n_act + LI_UNIT - 1) / LI_UNIT;
+        p.work = (double)p.n_units; p.w_max = 1.0;
         p.n_tiles = Npad / LI_TJ;
         p.resident = (int64_t)n_sm * LI_CTAS_PER_SM;
-        p.s_max = nb_min64(nb_min64(rows / (p.n_units * p.unit * p.sub), 2048), p.n_tiles / 2);
+        p.s_max = nb_min64(nb_min64(rows / (p.n_units * LI_UNIT), 2048), p.n_tiles / 2);
+    } else {
+        // warp units: a work item is (unit, j-slice); resident = warps on the device
+        p.kernel = 1; p.unit = 32; p.tile = WU_TJ; p.ctas_per_sm = WU_CTAS_PER_SM; p.fixed = 0.5;
+        p.n_units = nb_wu_count(n_act, &p.work, &p.w_max);
+        p.n_tiles = Npad / WU_TJ;
+        p.resident = (int64_t)n_sm * WU_CTAS_PER_SM * WU_WARPS;
+        p.s_max = nb_min64(nb_min64(rows / n_act, 16384), p.n_tiles / 2);
     }
     p.s_max = nb_max64(1, nb_min64(p.s_max, p.n_tiles));
     if (max_split > 0) p.s_max = nb_min64(p.s_max, max_split);
@@ -54,25 +109,30 @@ NB_HD PlanShape nb_plan_shape(int64_t Npad, int64_t n_act, int n_sm, int64_t max
 
 // Cost of splitting into S slices, in units of one j-tile of work on one work slot (a negative value: S leaves a
 // slice empty and is not a candidate).  Work items (unit, slice) are pulled from a queue by `resident` workers (CTAs
-// or warps); an item costs slice_tiles + fixed.
-// Lanes-over-i with 128-particle tiles (kernel 0): co-resident CTAs do not get equal shares of the FP64 pipe, so a
-// single round of equal items ends with the slow CTA of every SM running alone (measured 0.78 of the issue bound
-// against 0.86 with ten rounds): one round counts 1.5, more rounds items / resident + 0.9 for the tail.
-// The other shapes (tiny active sets, latency-bound): up to four rounds the last round is counted whole; beyond that
-// the queue balances the workers up to a tail of about 0.7 items.
+// or warps); an item of a unit of weight w costs w * slice_tiles + fixed.
+// CTA tiles (kernel 0): co-resident CTAs do not get equal shares of the FP64 pipe, so a single round of equal items
+// ends with the slow CTA of every SM running alone (measured 0.78 of the issue bound against 0.86 with ten rounds):
+// one round counts 1.5, more rounds items / resident + 0.9 for the tail.
+// Warp units (kernel 1): up to one round the largest item decides; up to four rounds the last round is counted whole;
+// beyond that the queue balances the workers up to a tail of about 0.7 of the largest item.
 NB_HD double nb_split_cost(const PlanShape& p, int64_t S, int64_t* slice_tiles)
 {
     const int64_t st = (p.n_tiles + S - 1) / S;
     *slice_tiles = st;
     if ((p.n_tiles + st - 1) / st != S) return -1.0;
     const int64_t items = p.n_units * S;
-    double rounds;
-    if (p.kernel == 0)
-        rounds = items <= p.resident ? 1.5 : (double)items / (double)p.resident + 0.9;
-    else
-        rounds = items <= 4 * p.resident ? (double)((items + p.resident - 1) / p.resident)
-                                         : (double)items / (double)p.resident + 0.7;
-    return rounds * (double)(st + p.fixed);
+    if (p.kernel == 0) {
+        const double rounds = items <= p.resident ? 1.5 : (double)items / (double)p.resident + 0.9;
+        return rounds * ((double)st + p.fixed);
+    }
+    const double c_max = p.w_max * (double)st + p.fixed;
+    const double c_avg = p.work / (double)p.n_units * (double)st + p.fixed;
+    if (items <= p.resident) return c_max;
+    if (items <= 4 * p.resident) {
+        const double c = (double)((items + p.resident - 1) / p.resident) * c_avg;
+        return c > c_max ? c : c_max;
+    }
+    return (double)items * c_avg / (double)p.resident + 0.7 * c_max;
 }
 
 // The split is the S in [1, s_max] of least cost, the smallest such S on ties (S = 1 is always a candidate).
@@ -103,7 +163,8 @@ NB_HD int nb_reduce_threads(int64_t n_act, int n_planes)
 struct DevPlan {
     int stop;                  // 1: t_next > t_end (or the step budget is used up) - every kernel of the step returns at once
     int kernel;
-    int n_act, n_units, n_split, slice_tiles, n_items, ld, n_planes, red_T;
+    int n_act, n_units, n_split, slice_tiles, n_items, ld, red_T;
+    int predict;               // 1: the force kernel predicts the j-records it reads; the predictor kernel returns at once
     double t_next;
     double t_end;
     long long max_split;       // cap on S (0: none), see nb_plan_shape
@@ -123,7 +184,7 @@ NB_HD void nb_fill_devplan(DevPlan* d, const PlanShape& p, int64_t S, int64_t n_
     d->n_split = (int)S;
     d->slice_tiles = (int)st;
     d->n_items = (int)(p.n_units * S);
-    d->ld = (int)(p.n_units * p.unit);
-    d->n_planes = (int)(S * p.sub);
-    d->red_T = nb_reduce_threads(n_act, d->n_planes);
+    d->ld = p.kernel == 0 ? (int)(p.n_units * p.unit) : (int)n_act;
+    d->red_T = nb_reduce_threads(n_act, (int)S);
+    d->predict = p.kernel == 1 && p.n_units <= PIF_MAX_UNITS;
 }

@@ -3,6 +3,7 @@
 // energy.  All are HBM-bandwidth bound; see DESIGN.md for the bytes per particle of each.
 #include "nb_internal.h"
 #include "nb_plan.h"
+#include "nb_predict.h"
 
 namespace {
 
@@ -12,10 +13,10 @@ inline int nblocks(int64_t n, int tpb = TPB) { return (int)((n + tpb - 1) / tpb)
 // massless record far away: contributes exactly 0 to every sum and never overflows
 __device__ __forceinline__ void write_pad_record(const StateArrays& s, int64_t i)
 {
-    s.pj0[i] = make_double4(3e33, 3e33, 3e33, 0.0);
-    s.pj1[i] = make_double4(0.0, 0.0, 0.0, 0.0);
-    s.pj2[i] = make_double2(0.0, 0.0);
-    s.pj3[i] = make_double4(0.0, 0.0, 0.0, 0.0);
+    double2* r = s.rec + i * nb_rec_q(s.order);
+    r[0] = make_double2(3e33, 3e33);
+    r[1] = make_double2(3e33, 0.0);
+    for (int q = 2; q < nb_rec_q(s.order); ++q) r[q] = make_double2(0.0, 0.0);
 }
 
 // ------------------------------------------------------------------ init: AoS inputs -> packed state
@@ -27,63 +28,41 @@ __global__ void init_state_kernel(StateArrays s, int64_t N, int64_t Npad, const 
     if (i < N) {
         s.st0[i] = make_double4(x[3 * i], x[3 * i + 1], x[3 * i + 2], m[i]);
         s.st1[i] = make_double4(v[3 * i], v[3 * i + 1], v[3 * i + 2], 0.0);
-        s.dt[i] = 0.0;
+        s.dt[i] = 0.0; s.tn[i] = 0.0;
     } else {
         s.st0[i] = make_double4(3e33, 3e33, 3e33, 0.0);
         s.st1[i] = zero;
-        s.dt[i] = 1e300;
+        s.dt[i] = 1e300; s.tn[i] = 1e300;
         write_pad_record(s, i);
     }
     s.st2[i] = zero; s.st3[i] = zero; s.st4[i] = zero; s.st5[i] = zero; s.st6[i] = zero;
 }
 
 // ------------------------------------------------------------------ a1: predictor (reading R6)
-// Reads 160 B, writes 80 B per particle.  own_time: D = 0 for every particle (records := stored state).
+// Reads 160 B, writes 80 B per particle (224 B / 112 B at the 8th order).  own_time: D = 0 for every particle (records :=
+// stored state).  The arithmetic is nb_predict_record (nb_predict.h), shared with the force kernel.
+template <int ORDER>
 __global__ void __launch_bounds__(TPB) predict_kernel(StateArrays s, int64_t N, double t, bool own_time, const DevPlan* dp)
 {
     if (dp) {                                              // device-planned block step: the time comes from the scheduler
-        if (dp->stop) return;
+        if (dp->stop || dp->predict) return;               // (predict: the force kernel predicts what it reads)
         t = dp->t_next;
     }
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
-    const double4 p = s.st0[i], q = s.st1[i], r = s.st2[i], u = s.st3[i], w = s.st4[i];
-    const double D = own_time ? 0.0 : t - q.w;
-    const double D2 = D * 0.5, D3 = D * (1.0 / 3.0), D4 = D * 0.25, D5 = D * 0.2;
-    const double x[3] = {p.x, p.y, p.z}, v[3] = {q.x, q.y, q.z}, a[3] = {r.x, r.y, r.z};
-    const double j[3] = {r.w, u.x, u.y}, sn[3] = {u.z, u.w, w.x}, c[3] = {w.y, w.z, w.w};
-    double xp[3], vp[3], ap[3];
-    if (s.order == 8) {                                    // 8th-order variant (R22): two more terms, and the predicted jerk
-        const double4 g = s.st5[i], hq = s.st6[i];
-        const double a4[3] = {g.x, g.y, g.z}, a5[3] = {g.w, hq.x, hq.y};
-        const double D6 = D * (1.0 / 6.0), D7 = D * (1.0 / 7.0);
-        double jp[3];
+    constexpr int Q = nb_rec_q(ORDER);
+    double2 rec[Q];
+    nb_predict_record<ORDER>(nb_load_pstate<ORDER>(s.st0, s.st1, s.st2, s.st3, s.st4, s.st5, s.st6, i), t, own_time, rec);
+    double2* out = s.rec + i * Q;
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            xp[k] = fma(D, fma(D2, fma(D3, fma(D4, fma(D5, fma(D6, fma(D7, a5[k], a4[k]), c[k]), sn[k]), j[k]), a[k]), v[k]), x[k]);
-            vp[k] = fma(D, fma(D2, fma(D3, fma(D4, fma(D5, fma(D6, a5[k], a4[k]), c[k]), sn[k]), j[k]), a[k]), v[k]);
-            ap[k] = fma(D, fma(D2, fma(D3, fma(D4, fma(D5, a5[k], a4[k]), c[k]), sn[k]), j[k]), a[k]);
-            jp[k] = fma(D, fma(D2, fma(D3, fma(D4, a5[k], a4[k]), c[k]), sn[k]), j[k]);
-        }
-        s.pj3[i] = make_double4(jp[0], jp[1], jp[2], 0.0);
-    } else if (s.order == 4) {                                    // 4th-order variant (R21): x to the jerk term, v to D^2/2 jerk
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            xp[k] = fma(D, fma(D2, fma(D3, j[k], a[k]), v[k]), x[k]);
-            vp[k] = fma(D, fma(D2, j[k], a[k]), v[k]);
-            ap[k] = 0.0;                                   // a and jerk do not read it
-        }
-    } else {
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            xp[k] = fma(D, fma(D2, fma(D3, fma(D4, fma(D5, c[k], sn[k]), j[k]), a[k]), v[k]), x[k]);
-            vp[k] = fma(D, fma(D2, fma(D3, fma(D4, c[k], sn[k]), j[k]), a[k]), v[k]);
-            ap[k] = fma(D, fma(D2, fma(D3, c[k], sn[k]), j[k]), a[k]);
-        }
-    }
-    s.pj0[i] = make_double4(xp[0], xp[1], xp[2], p.w);
-    s.pj1[i] = make_double4(vp[0], vp[1], vp[2], ap[0]);
-    s.pj2[i] = make_double2(ap[1], ap[2]);
+    for (int q = 0; q < Q; ++q) out[q] = rec[q];
+}
+
+void launch_predict(const StateArrays& s, int64_t N, double t, bool own_time, const DevPlan* dp, cudaStream_t st)
+{
+    if (s.order == 8) predict_kernel<8><<<nblocks(N), TPB, 0, st>>>(s, N, t, own_time, dp);
+    else if (s.order == 4) predict_kernel<4><<<nblocks(N), TPB, 0, st>>>(s, N, t, own_time, dp);
+    else predict_kernel<6><<<nblocks(N), TPB, 0, st>>>(s, N, t, own_time, dp);
 }
 
 // ------------------------------------------------------------------ time-step level helpers (a5)
@@ -125,7 +104,7 @@ __global__ void startup_kernel(StateArrays s, int64_t N, const double* fa, const
     if (!(r < INFINITY)) k = k_max;
     else if (!(r > 0.0)) k = k_min;
     else k = clampi(ilog2_pos(r), k_min, k_max);
-    s.dt[i] = scalbn(1.0, k);
+    s.dt[i] = scalbn(1.0, k); s.tn[i] = s.dt[i];               // t_i = 0
 }
 
 // ------------------------------------------------------------------ a4 + a5: corrector (reading R10, R11, R12)
@@ -169,7 +148,7 @@ __device__ __forceinline__ void corrector_one(const StateArrays& s, const int32_
         s.st4[i] = make_double4(s1[2], c1[0], c1[1], c1[2]);
         s.st5[i] = make_double4(d4[0], d4[1], d4[2], d5[0]);
         s.st6[i] = make_double4(d5[1], d5[2], 0.0, 0.0);
-        if (dt_shared > 0.0) { s.dt[i] = dt_shared; return; }
+        if (dt_shared > 0.0) { s.dt[i] = dt_shared; s.tn[i] = t_new + dt_shared; return; }
         // dt_crit = eta (A1/A6)^(1/5); level = floor(log2 dt_crit) = floor(ilogb(dt_crit^5)/5) (eta3 carries eta^5 for this order)
         const double n0 = norm3(a1[0], a1[1], a1[2]), n1 = norm3(j1[0], j1[1], j1[2]), n2 = norm3(s1[0], s1[1], s1[2]);
         const double n5 = norm3(d5[0], d5[1], d5[2]), n6 = norm3(d6[0], d6[1], d6[2]), n7 = norm3(d7[0], d7[1], d7[2]);
@@ -185,7 +164,7 @@ __device__ __forceinline__ void corrector_one(const StateArrays& s, const int32_
             const double mm = scalbn(t_new, -(k_old + 1));
             if (mm == rint(mm)) k_new = k_old + 1;
         }
-        s.dt[i] = scalbn(1.0, k_new);
+        s.dt[i] = scalbn(1.0, k_new); s.tn[i] = t_new + s.dt[i];
         return;
     }
     if (s.order == 4) {
@@ -206,7 +185,7 @@ __device__ __forceinline__ void corrector_one(const StateArrays& s, const int32_
         s.st2[i] = make_double4(a1[0], a1[1], a1[2], j1[0]);
         s.st3[i] = make_double4(j1[1], j1[2], d2[0], d2[1]);
         s.st4[i] = make_double4(d2[2], d3[0], d3[1], d3[2]);
-        if (dt_shared > 0.0) { s.dt[i] = dt_shared; return; }
+        if (dt_shared > 0.0) { s.dt[i] = dt_shared; s.tn[i] = t_new + dt_shared; return; }
         // dt_crit = eta A1/A2 (eta3 carries eta itself for this order)
         const double n0 = norm3(a1[0], a1[1], a1[2]), n1 = norm3(j1[0], j1[1], j1[2]);
         const double n2 = norm3(d2[0], d2[1], d2[2]), n3 = norm3(d3[0], d3[1], d3[2]);
@@ -222,7 +201,7 @@ __device__ __forceinline__ void corrector_one(const StateArrays& s, const int32_
             const double mm = scalbn(t_new, -(k_old + 1));
             if (mm == rint(mm)) k_new = k_old + 1;
         }
-        s.dt[i] = scalbn(1.0, k_new);
+        s.dt[i] = scalbn(1.0, k_new); s.tn[i] = t_new + s.dt[i];
         return;
     }
     double a1[3], j1[3], s1[3], x1[3], v1[3], d3[3], d4[3], d5[3];
@@ -250,7 +229,7 @@ __device__ __forceinline__ void corrector_one(const StateArrays& s, const int32_
     s.st3[i] = make_double4(j1[1], j1[2], s1[0], s1[1]);
     s.st4[i] = make_double4(s1[2], d3[0], d3[1], d3[2]);
 
-    if (dt_shared > 0.0) { s.dt[i] = dt_shared; return; }
+    if (dt_shared > 0.0) { s.dt[i] = dt_shared; s.tn[i] = t_new + dt_shared; return; }
 
     // dt_crit = eta (A1/A4)^(1/3); level = floor(log2 dt_crit) = floor(ilogb(dt_crit^3) / 3), no cube root needed
     const double n0 = norm3(a1[0], a1[1], a1[2]), n1 = norm3(j1[0], j1[1], j1[2]), n2 = norm3(s1[0], s1[1], s1[2]);
@@ -268,23 +247,72 @@ __device__ __forceinline__ void corrector_one(const StateArrays& s, const int32_
         const double m = scalbn(t_new, -(k_old + 1));       // exact: t_new / 2^(k_old+1)
         if (m == rint(m)) k_new = k_old + 1;                // grow only on the doubled grid
     }
-    s.dt[i] = scalbn(1.0, k_new);
+    s.dt[i] = scalbn(1.0, k_new); s.tn[i] = t_new + s.dt[i];
 }
 
 __global__ void __launch_bounds__(TPB) corrector_kernel(StateArrays s, const int32_t* idx, int64_t n_act, double dt_shared,
                                                         double t_new, const double* fa, const double* fj, const double* fs,
-                                                        double eta3, int k_min, int k_max, DevPlan* dp, unsigned long long* tmin_bits)
+                                                        double eta3, int k_min, int k_max)
 {
-    if (dp) {                                              // device-planned block step
-        if (dp->stop) return;
-        n_act = dp->n_act; t_new = dp->t_next;
-        if (blockIdx.x == 0 && threadIdx.x == 0) {         // last kernel of the step: book-keeping nobody else reads now
-            dp->steps_done += 1; dp->steps_left -= 1; dp->sum_act += n_act; dp->t_last = t_new;
-            *tmin_bits = ~0ull;                            // "+infinity" for the next step's atomicMin
-        }
-    }
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n_act; k += (int64_t)gridDim.x * blockDim.x)
         corrector_one(s, idx, k, dt_shared, t_new, fa, fj, fs, eta3, k_min, k_max);
+}
+
+// Device-planned block step (nb_run_blocks): the partial-sum reduction of row a3 and the corrector in ONE kernel.  The
+// sums are those of reduce_partials_kernel (nb_force.cu): T threads per active particle, thread `lane` adds slices lane,
+// lane + T, ... in increasing order, binary tree over the T lane sums - the same order, so the same bits - and the thread
+// that holds a particle's total stores it and corrects the particle.  S = 1: the force kernel stored the results itself.
+template <int NC>
+__global__ void __launch_bounds__(RED_THREADS) reduce_correct_kernel(StateArrays s, const int32_t* idx, ForceArgs A, double eta3,
+                                                                     int k_min, int k_max, DevPlan* dp)
+{
+    __shared__ double sm[NC][RED_THREADS];
+    if (dp->stop) return;
+    const int n_act = dp->n_act, S = dp->n_split, T = dp->red_T, ld = dp->ld;
+    const double t_new = dp->t_next;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {             // last kernel of the step: book-keeping nobody else reads now
+        dp->steps_done += 1; dp->steps_left -= 1; dp->sum_act += n_act; dp->t_last = t_new;
+    }
+    if (S <= 1) {
+        for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n_act; k += gridDim.x * blockDim.x)
+            corrector_one(s, idx, k, 0.0, t_new, A.out_a, A.out_j, A.out_s, eta3, k_min, k_max);
+        return;
+    }
+    const int R = RED_THREADS / T;                         // active particles per block and pass
+    const int kl = threadIdx.x % R, lane = threadIdx.x / R;
+    for (int k0 = blockIdx.x * R; k0 < n_act; k0 += gridDim.x * R) {        // uniform over the block
+        const int k = k0 + kl;
+        double r[NC];
+#pragma unroll
+        for (int c = 0; c < NC; ++c) r[c] = 0.0;
+        if (k < n_act) {
+            const size_t plane = (size_t)NC * ld;
+            const double* P = A.partial + (size_t)lane * plane + k;
+            for (int sl = lane; sl < S; sl += T, P += (size_t)T * plane) {
+#pragma unroll
+                for (int c = 0; c < NC; ++c) r[c] += P[(size_t)c * ld];
+            }
+        }
+        for (int off = T >> 1; off > 0; off >>= 1) {
+            if (lane >= off && lane < 2 * off) {
+#pragma unroll
+                for (int c = 0; c < NC; ++c) sm[c][threadIdx.x] = r[c];
+            }
+            __syncthreads();
+            if (lane < off) {
+#pragma unroll
+                for (int c = 0; c < NC; ++c) r[c] += sm[c][threadIdx.x + off * R];
+            }
+            __syncthreads();
+        }
+        if (lane != 0 || k >= n_act) continue;
+        A.out_a[3 * k] = r[0]; A.out_a[3 * k + 1] = r[1]; A.out_a[3 * k + 2] = r[2];
+        A.out_j[3 * k] = r[3]; A.out_j[3 * k + 1] = r[4]; A.out_j[3 * k + 2] = r[5];
+        A.out_s[3 * k] = r[6]; A.out_s[3 * k + 1] = r[7]; A.out_s[3 * k + 2] = r[8];
+        A.out_p[k] = -r[9];
+        if (NC == 13) { A.out_c[3 * k] = r[10]; A.out_c[3 * k + 1] = r[11]; A.out_c[3 * k + 2] = r[12]; }
+        corrector_one(s, idx, k, 0.0, t_new, A.out_a, A.out_j, A.out_s, eta3, k_min, k_max);   // reads back what this thread stored
+    }
 }
 
 // ------------------------------------------------------------------ state I/O
@@ -306,12 +334,12 @@ __global__ void get_kernel(StateArrays s, int field, const int32_t* idx, int64_t
         case NB_J: { double4 p = s.st2[i], q = s.st3[i]; a = p.w; b = q.x; c = q.y; } break;
         case NB_S: { double4 p = s.st3[i], q = s.st4[i]; a = p.z; b = p.w; c = q.x; } break;
         case NB_C: { double4 p = s.st4[i]; a = p.y; b = p.z; c = p.w; } break;
-        case NB_XP: { double4 p = s.pj0[i]; a = p.x; b = p.y; c = p.z; } break;
-        case NB_VP: { double4 p = s.pj1[i]; a = p.x; b = p.y; c = p.z; } break;
-        case NB_AP: { double4 p = s.pj1[i]; double2 q = s.pj2[i]; a = p.w; b = q.x; c = q.y; } break;
+        case NB_XP: { const double2* r = s.rec + i * nb_rec_q(s.order); a = r[0].x; b = r[0].y; c = r[1].x; } break;
+        case NB_VP: { const double2* r = s.rec + i * nb_rec_q(s.order); a = r[2].x; b = r[2].y; c = r[3].x; } break;
+        case NB_AP: { const double2* r = s.rec + i * nb_rec_q(s.order); a = r[3].y; b = r[4].x; c = r[4].y; } break;
         case NB_A4: { double4 p = s.st5[i]; a = p.x; b = p.y; c = p.z; } break;
         case NB_A5: { double4 p = s.st5[i], q = s.st6[i]; a = p.w; b = q.x; c = q.y; } break;
-        case NB_JP: { double4 p = s.pj3[i]; a = p.x; b = p.y; c = p.z; } break;
+        case NB_JP: if (s.order == 8) { const double2* r = s.rec + i * 7; a = r[5].x; b = r[5].y; c = r[6].x; } break;
     }
     if (field_width(field) == 1) out[k] = a;
     else { out[3 * k] = a; out[3 * k + 1] = b; out[3 * k + 2] = c; }
@@ -326,8 +354,8 @@ __global__ void set_kernel(StateArrays s, int field, const int32_t* idx, int64_t
     const double a = one ? in[k] : in[3 * k], b = one ? 0.0 : in[3 * k + 1], c = one ? 0.0 : in[3 * k + 2];
     switch (field) {
         case NB_M: s.st0[i].w = a; break;
-        case NB_T: s.st1[i].w = a; break;
-        case NB_DT: s.dt[i] = a; break;
+        case NB_T: s.st1[i].w = a; s.tn[i] = a + s.dt[i]; break;
+        case NB_DT: s.dt[i] = a; s.tn[i] = s.st1[i].w + a; break;
         case NB_X: s.st0[i].x = a; s.st0[i].y = b; s.st0[i].z = c; break;
         case NB_V: s.st1[i].x = a; s.st1[i].y = b; s.st1[i].z = c; break;
         case NB_A: s.st2[i].x = a; s.st2[i].y = b; s.st2[i].z = c; break;
@@ -339,131 +367,156 @@ __global__ void set_kernel(StateArrays s, int field, const int32_t* idx, int64_t
     }
 }
 
-// ------------------------------------------------------------------ a6: block scheduler
-// scratch layout (bytes): [0] u64 bits of t_next (atomicMin; times are >= 0 so the bit order is the
-// numeric order)  [8] i64 n_act  [16] u32 blocks-done counter  [64...] u32 per-block counts/offsets
-__device__ __forceinline__ double block_min(double v)
-{
-    __shared__ double sm[32];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
-    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
-    __syncthreads();
-    if (threadIdx.x < 32) {
-        v = threadIdx.x < (blockDim.x >> 5) ? sm[threadIdx.x] : INFINITY;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
-    }
-    return v;   // valid in thread 0
-}
-
-__global__ void __launch_bounds__(1024) sched_min_kernel(StateArrays s, int64_t N, unsigned long long* tmin_bits, const DevPlan* dp)
-{
-    if (dp && dp->stop) return;
-    double v = INFINITY;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
-        v = fmin(v, s.st1[i].w + s.dt[i]);
-    v = block_min(v);
-    if (threadIdx.x == 0) atomicMin(tmin_bits, (unsigned long long)__double_as_longlong(v));
-}
-
+// ------------------------------------------------------------------ a6: block scheduler, ONE kernel
+// t_next = min_i tn_i (tn = t + dt, kept by the corrector) and the list { i : tn_i == t_next } in increasing index order.
+// Every block takes 2048 consecutive particles: it finds ITS minimum and compacts the particles that attain it, in order,
+// into its own stretch of `cand`.  The block that finishes last (atomic ticket) takes the minimum over the block minima,
+// scans the counts of the blocks that attain it and copies their candidate lists, in block order, into the active list;
+// in a device-planned block step it then decides whether the step is taken and plans the force launch (nb_plan.h).
+// One pass over 8 B per particle instead of three passes over 16 B.
+// scratch layout (bytes): [0] double t_next  [8] i64 n_act  [16] u32 blocks-done counter
+//                         [64 ...] double bmin[B]; then u32 cnt[B]; then u32 off[B]       (B = blocks)
 constexpr int SCHED_TPB = 1024;
+constexpr int SCHED_CHUNK = 2 * SCHED_TPB;
 
-__global__ void __launch_bounds__(SCHED_TPB) sched_count_kernel(StateArrays s, int64_t N, const unsigned long long* tmin_bits,
-                                                               unsigned int* counts, unsigned int* done, long long* n_act_out,
-                                                               DevPlan* dp, int64_t Npad, int n_sm)
+// exclusive prefix sum of v over the block's 1024 threads in thread order; *total = the block's sum.  wt: 33 words of smem.
+__device__ __forceinline__ unsigned int block_excl_scan(unsigned int v, unsigned int* wt, unsigned int* total)
 {
-    __shared__ unsigned int warp_cnt[32];
-    __shared__ bool last;
-    if (dp && dp->stop) return;
-    const double tn = __longlong_as_double((long long)*tmin_bits);
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool act = i < N && (s.st1[i].w + s.dt[i] == tn);
-    const unsigned int b = __ballot_sync(0xffffffffu, act);
-    if ((threadIdx.x & 31) == 0) warp_cnt[threadIdx.x >> 5] = __popc(b);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    unsigned int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const unsigned int n = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += n; }
+    __syncthreads();                                        // wt may still be read from a previous call
+    if (lane == 31) wt[warp] = inc;
     __syncthreads();
-    if (threadIdx.x == 0) {
-        unsigned int c = 0;
-        for (int w = 0; w < SCHED_TPB / 32; ++w) c += warp_cnt[w];
-        counts[blockIdx.x] = c;
+    if (warp == 0) {
+        const unsigned int w = wt[lane];
+        unsigned int wi = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const unsigned int n = __shfl_up_sync(0xffffffffu, wi, o); if (lane >= o) wi += n; }
+        wt[lane] = wi - w;                                  // exclusive offset of each warp
+        if (lane == 31) wt[32] = wi;
+    }
+    __syncthreads();
+    *total = wt[32];
+    return wt[warp] + inc - v;
+}
+
+__global__ void __launch_bounds__(SCHED_TPB) sched_kernel(StateArrays s, int64_t N, int32_t* cand, int32_t* active, char* scratch,
+                                                         DevPlan* dp, int64_t Npad, int n_sm)
+{
+    __shared__ double red[32];
+    __shared__ unsigned int warp_tot[33];
+    __shared__ bool last;
+    __shared__ double best_c[SCHED_TPB];
+    __shared__ int best_s[SCHED_TPB];
+    if (dp && dp->stop) return;
+    const int B = gridDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    double* bmin_arr = (double*)(scratch + 64);
+    unsigned int* cnt_arr = (unsigned int*)(bmin_arr + B);
+    unsigned int* off_arr = cnt_arr + B;
+    unsigned int* done = (unsigned int*)(scratch + 16);
+
+    // ---- this block's minimum and its candidates
+    const int64_t i0 = (int64_t)blockIdx.x * SCHED_CHUNK + 2 * tid;
+    double v0 = INFINITY, v1 = INFINITY;
+    if (i0 + 1 < N) { const double2 t2 = *(const double2*)(s.tn + i0); v0 = t2.x; v1 = t2.y; }
+    else if (i0 < N) v0 = s.tn[i0];
+    double m = fmin(v0, v1);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmin(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if (lane == 0) red[warp] = m;
+    __syncthreads();
+    m = red[lane];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmin(m, __shfl_xor_sync(0xffffffffu, m, o));
+    const double bmin = m;                                  // every thread has it
+    const bool f0 = v0 == bmin && i0 < N, f1 = v1 == bmin && i0 + 1 < N;
+    const unsigned int c = (unsigned)f0 + (unsigned)f1;
+    unsigned int total;
+    unsigned int o_ = block_excl_scan(c, warp_tot, &total);   // in thread (= index) order
+    int32_t* my = cand + (int64_t)blockIdx.x * SCHED_CHUNK;
+    if (f0) my[o_++] = (int32_t)i0;
+    if (f1) my[o_] = (int32_t)(i0 + 1);
+    if (tid == 0) {
+        bmin_arr[blockIdx.x] = bmin; cnt_arr[blockIdx.x] = total;
         __threadfence();
-        last = atomicAdd(done, 1u) == gridDim.x - 1;
+        last = atomicAdd(done, 1u) == (unsigned)(B - 1);
     }
     __syncthreads();
     if (!last) return;
-    // the last block turns counts[] into exclusive offsets (gridDim.x <= a few thousand), in index order
     __threadfence();
-    __shared__ unsigned int part[SCHED_TPB];
-    const int nb = gridDim.x;
-    const int per = (nb + SCHED_TPB - 1) / SCHED_TPB;
-    unsigned int sum = 0;
-    for (int q = 0; q < per; ++q) { int b2 = threadIdx.x * per + q; if (b2 < nb) sum += __ldcg(counts + b2); }
-    part[threadIdx.x] = sum;
+
+    // ---- the last block: global minimum, offsets of the blocks that attain it, ordered copy
+    double g = INFINITY;
+    for (int b = tid; b < B; b += SCHED_TPB) g = fmin(g, __ldcg(bmin_arr + b));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) g = fmin(g, __shfl_xor_sync(0xffffffffu, g, o));
+    __syncthreads();                                        // red[] is free again
+    if (lane == 0) red[warp] = g;
     __syncthreads();
-    if (threadIdx.x == 0) {
-        unsigned int run = 0;
-        for (int q = 0; q < SCHED_TPB; ++q) { unsigned int v = part[q]; part[q] = run; run += v; }
-        *n_act_out = (long long)run;
+    g = red[lane];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) g = fmin(g, __shfl_xor_sync(0xffffffffu, g, o));
+    const double tn = g;
+    const int per = (B + SCHED_TPB - 1) / SCHED_TPB;        // consecutive blocks per thread
+    unsigned int sum = 0;
+    for (int q = 0; q < per; ++q) {
+        const int b = tid * per + q;
+        if (b < B && __ldcg(bmin_arr + b) == tn) sum += __ldcg(cnt_arr + b);
+    }
+    unsigned int n_tot;
+    unsigned int run = block_excl_scan(sum, warp_tot, &n_tot);
+    const long long n_act = n_tot;
+    if (tid == 0) {
+        ((double*)scratch)[0] = tn;
+        ((long long*)scratch)[1] = n_act;
         *done = 0;
     }
-    __syncthreads();
-    unsigned int run = part[threadIdx.x];
     for (int q = 0; q < per; ++q) {
-        int b2 = threadIdx.x * per + q;
-        if (b2 < nb) { unsigned int v = __ldcg(counts + b2); counts[b2] = run; run += v; }
+        const int b = tid * per + q;
+        if (b < B) {
+            const bool hit = __ldcg(bmin_arr + b) == tn;
+            off_arr[b] = hit ? run : 0xffffffffu;
+            if (hit) run += __ldcg(cnt_arr + b);
+        }
+    }
+    __syncthreads();                                        // off_arr (global) written by this block: visible after the barrier
+    for (int b = warp; b < B; b += SCHED_TPB / 32) {
+        const unsigned int off = __ldcg(off_arr + b);
+        if (off == 0xffffffffu) continue;
+        const unsigned int n = __ldcg(cnt_arr + b);
+        const int32_t* src = cand + (int64_t)b * SCHED_CHUNK;
+        for (unsigned int i = lane; i < n; i += 32) active[off + i] = __ldcg(src + i);
     }
     if (!dp) return;
     // device-planned block step (nb_run_blocks): decide whether the step is taken, and plan the force launch for its
     // n_act with the functions the host uses (nb_plan.h); the candidates S are spread over the block's threads.
-    __syncthreads();
-    __shared__ double best_c[SCHED_TPB];
-    __shared__ int best_s[SCHED_TPB];
-    const long long n_act = *n_act_out;
     const bool stop = tn > dp->t_end || dp->steps_left <= 0 || n_act <= 0;
     if (stop) {
-        if (threadIdx.x == 0) { dp->stop = 1; dp->n_act = 0; }
+        if (tid == 0) { dp->stop = 1; dp->n_act = 0; }
         return;
     }
     const PlanShape sh = nb_plan_shape(Npad, n_act, n_sm, dp->max_split);
-    double c;
-    const int64_t S = nb_best_split(sh, 1 + threadIdx.x, SCHED_TPB, &c);
-    best_c[threadIdx.x] = c; best_s[threadIdx.x] = (int)S;       // S = 0: this thread had no candidate (c = 1e300)
+    double cst;
+    const int64_t S = nb_best_split(sh, 1 + tid, SCHED_TPB, &cst);
+    best_c[tid] = cst; best_s[tid] = (int)S;               // S = 0: this thread had no candidate (cost 1e300)
     __syncthreads();
     for (int o = SCHED_TPB / 2; o > 0; o >>= 1) {
-        if (threadIdx.x < o) {
-            const double c2 = best_c[threadIdx.x + o];
-            const int s2 = best_s[threadIdx.x + o];
-            const double c1 = best_c[threadIdx.x];
-            const int s1 = best_s[threadIdx.x];
+        if (tid < o) {
+            const double c2 = best_c[tid + o];
+            const int s2 = best_s[tid + o];
+            const double c1 = best_c[tid];
+            const int s1 = best_s[tid];
             // least cost; on ties the smaller S (as the host's ascending scan)
-            if (s2 != 0 && (s1 == 0 || c2 < c1 || (c2 == c1 && s2 < s1))) { best_c[threadIdx.x] = c2; best_s[threadIdx.x] = s2; }
+            if (s2 != 0 && (s1 == 0 || c2 < c1 || (c2 == c1 && s2 < s1))) { best_c[tid] = c2; best_s[tid] = s2; }
         }
         __syncthreads();
     }
-    if (threadIdx.x == 0) {
+    if (tid == 0) {
         nb_fill_devplan(dp, sh, best_s[0], n_act);
         dp->t_next = tn;
     }
-}
-
-__global__ void __launch_bounds__(SCHED_TPB) sched_scatter_kernel(StateArrays s, int64_t N, const unsigned long long* tmin_bits,
-                                                                 const unsigned int* offsets, int32_t* active, const DevPlan* dp)
-{
-    __shared__ unsigned int warp_off[32];
-    if (dp && dp->stop) return;
-    const double tn = __longlong_as_double((long long)*tmin_bits);
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool act = i < N && (s.st1[i].w + s.dt[i] == tn);
-    const unsigned int b = __ballot_sync(0xffffffffu, act);
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (lane == 0) warp_off[warp] = __popc(b);
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        unsigned int run = offsets[blockIdx.x];
-        for (int w = 0; w < SCHED_TPB / 32; ++w) { unsigned int v = warp_off[w]; warp_off[w] = run; run += v; }
-    }
-    __syncthreads();
-    if (act) active[warp_off[warp] + __popc(b & ((1u << lane) - 1u))] = (int32_t)i;
 }
 
 // ------------------------------------------------------------------ energy (fixed-order reduction)
@@ -529,7 +582,7 @@ cudaError_t nb_launch_init_state(const StateArrays& s, int64_t N, int64_t Npad, 
 
 cudaError_t nb_launch_predict(const StateArrays& s, int64_t N, double t, bool own_time, cudaStream_t st)
 {
-    predict_kernel<<<nblocks(N), TPB, 0, st>>>(s, N, t, own_time, nullptr);
+    launch_predict(s, N, t, own_time, nullptr, st);
     return cudaGetLastError();
 }
 
@@ -540,12 +593,13 @@ cudaError_t nb_launch_startup(const StateArrays& s, int64_t N, const double* fa,
     return cudaGetLastError();
 }
 
+static double eta_power(int order, double eta) { return order == 4 ? eta : order == 8 ? eta * eta * eta * eta * eta : eta * eta * eta; }
+
 cudaError_t nb_launch_corrector(const StateArrays& s, const int32_t* idx, int64_t n_act, double dt_shared, double t_new,
                                 const double* fa, const double* fj, const double* fs, double eta, int k_min, int k_max,
                                 cudaStream_t st)
 {
-    corrector_kernel<<<nblocks(n_act), TPB, 0, st>>>(s, idx, n_act, dt_shared, t_new, fa, fj, fs, s.order == 4 ? eta : s.order == 8 ? eta * eta * eta * eta * eta : eta * eta * eta,
-                                                     k_min, k_max, nullptr, nullptr);
+    corrector_kernel<<<nblocks(n_act), TPB, 0, st>>>(s, idx, n_act, dt_shared, t_new, fa, fj, fs, eta_power(s.order, eta), k_min, k_max);
     return cudaGetLastError();
 }
 
@@ -561,47 +615,27 @@ cudaError_t nb_launch_set(const StateArrays& s, int field, const int32_t* idx, i
     return cudaGetLastError();
 }
 
-cudaError_t nb_launch_next_block(const StateArrays& s, int64_t N, int32_t* active, void* scratch, cudaStream_t st, int* launches)
+cudaError_t nb_launch_next_block(const StateArrays& s, int64_t N, int32_t* active, int32_t* cand, void* scratch, cudaStream_t st, int* launches)
 {
-    unsigned long long* tmin = (unsigned long long*)scratch;
-    long long* n_act = (long long*)scratch + 1;
-    unsigned int* done = (unsigned int*)((char*)scratch + 16);
-    unsigned int* counts = (unsigned int*)((char*)scratch + 64);
-    cudaError_t e = cudaMemsetAsync(scratch, 0xff, 8, st);          // all-ones > any non-negative double's bits... see below
-    if (e != cudaSuccess) return e;
-    // 0xffff... as an unsigned is larger than the bit pattern of +inf (0x7ff0...), so it is a valid "+infinity"
-    const int nb_min = (int)((N + 4095) / 4096) < 1024 ? (int)((N + 4095) / 4096) : 1024;
-    sched_min_kernel<<<nb_min, 1024, 0, st>>>(s, N, tmin, nullptr);
-    const int nb = nblocks(N, SCHED_TPB);
-    sched_count_kernel<<<nb, SCHED_TPB, 0, st>>>(s, N, tmin, counts, done, n_act, nullptr, 0, 0);
-    sched_scatter_kernel<<<nb, SCHED_TPB, 0, st>>>(s, N, tmin, counts, active, nullptr);
-    *launches += 3;
+    sched_kernel<<<nblocks(N, SCHED_CHUNK), SCHED_TPB, 0, st>>>(s, N, cand, active, (char*)scratch, nullptr, 0, 0);
+    *launches += 1;
     return cudaGetLastError();
 }
 
-cudaError_t nb_launch_devstep_head(const StateArrays& s, int64_t N, int64_t Npad, int n_sm, int32_t* active, void* scratch, DevPlan* dp,
-                                   cudaStream_t st, int* launches)
+cudaError_t nb_launch_devstep_head(const StateArrays& s, int64_t N, int64_t Npad, int n_sm, int32_t* active, int32_t* cand, void* scratch,
+                                   DevPlan* dp, cudaStream_t st, int* launches)
 {
-    unsigned long long* tmin = (unsigned long long*)scratch;         // all ones on entry (memset by the caller, then by the corrector)
-    long long* n_act = (long long*)scratch + 1;
-    unsigned int* done = (unsigned int*)((char*)scratch + 16);
-    unsigned int* counts = (unsigned int*)((char*)scratch + 64);
-    const int nb_min = (int)((N + 4095) / 4096) < 1024 ? (int)((N + 4095) / 4096) : 1024;
-    sched_min_kernel<<<nb_min, 1024, 0, st>>>(s, N, tmin, dp);
-    const int nb = nblocks(N, SCHED_TPB);
-    sched_count_kernel<<<nb, SCHED_TPB, 0, st>>>(s, N, tmin, counts, done, n_act, dp, Npad, n_sm);
-    sched_scatter_kernel<<<nb, SCHED_TPB, 0, st>>>(s, N, tmin, counts, active, dp);
-    predict_kernel<<<nblocks(N), TPB, 0, st>>>(s, N, 0.0, false, dp);
-    *launches += 4;
+    sched_kernel<<<nblocks(N, SCHED_CHUNK), SCHED_TPB, 0, st>>>(s, N, cand, active, (char*)scratch, dp, Npad, n_sm);
+    launch_predict(s, N, 0.0, false, dp, st);
+    *launches += 2;
     return cudaGetLastError();
 }
 
-cudaError_t nb_launch_devstep_tail(const StateArrays& s, int n_sm, const int32_t* active, void* scratch, DevPlan* dp, const double* fa,
-                                   const double* fj, const double* fs, double eta, int k_min, int k_max, cudaStream_t st, int* launches)
+cudaError_t nb_launch_devstep_tail(const StateArrays& s, int n_sm, const int32_t* active, const ForceArgs& fargs, DevPlan* dp,
+                                   double eta, int k_min, int k_max, cudaStream_t st, int* launches)
 {
-    corrector_kernel<<<n_sm * 8, TPB, 0, st>>>(s, active, 0, 0.0, 0.0, fa, fj, fs,
-                                               s.order == 4 ? eta : s.order == 8 ? eta * eta * eta * eta * eta : eta * eta * eta, k_min, k_max, dp,
-                                               (unsigned long long*)scratch);
+    if (s.order == 8) reduce_correct_kernel<13><<<n_sm * 4, RED_THREADS, 0, st>>>(s, active, fargs, eta_power(s.order, eta), k_min, k_max, dp);
+    else reduce_correct_kernel<10><<<n_sm * 4, RED_THREADS, 0, st>>>(s, active, fargs, eta_power(s.order, eta), k_min, k_max, dp);
     *launches += 1;
     return cudaGetLastError();
 }

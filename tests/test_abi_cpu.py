@@ -56,7 +56,7 @@ def test_struct_layouts_match_header(B):
     # nb_config: int, void*, void*, size_t, int, double, double, int, int, int, int  (natural alignment)
     assert C.sizeof(B.nb_config) == 72 and B.nb_config.order.offset == 64 and B.nb_config.check_indices.offset == 68
     assert B.nb_config.workspace.offset == 16 and B.nb_config.eta.offset == 40 and B.nb_config.k_max.offset == 60
-    assert C.sizeof(B.nb_plan) == 48 and B.nb_plan.waves.offset == 40
+    assert C.sizeof(B.nb_plan) == 48 and B.nb_plan.waves.offset == 40 and B.nb_plan.predict_in_force.offset == 32
 
 
 def test_workspace_bytes(B):
@@ -68,23 +68,50 @@ def test_workspace_bytes(B):
     assert 600e6 < big < 1.6e9                               # ~1.3 GB for 2^20 particles: fits 180 GB many times over
 
 
+def wu_units(n_act):
+    """The unit table of the warp-unit shape, restated from include/nb.h and csrc/nb_plan.h: n_act = 32 a + r -> a units of
+    32, then r from its highest bit down, except that a rest missing at most a quarter of the next power of two is padded."""
+    units, k = [(32 * u, 32, 32) for u in range(n_act // 32)], 32 * (n_act // 32)
+    rem = n_act % 32
+    while rem:
+        pc = 1 << (rem - 1).bit_length()
+        p, valid = (pc, rem) if pc - rem <= pc // 4 else (1 << (rem.bit_length() - 1),) * 2
+        units.append((k, p, valid))
+        k += valid; rem -= valid
+    return units
+
+
+def test_warp_unit_decomposition():
+    for n in range(1, 300):
+        u = wu_units(n)
+        assert sum(v for _, _, v in u) == n and u[0][0] == 0
+        assert all(k0 == sum(v for _, _, v in u[:i]) for i, (k0, _, _) in enumerate(u))      # rows are contiguous
+        assert all(p in (1, 2, 4, 8, 16, 32) and p // 4 * 3 <= v <= p for _, p, v in u)       # at most a quarter padded
+        assert sum(p for _, p, _ in u) <= n * 4 / 3 + 1                                         # lanes spent vs particles
+    assert [p for _, p, _ in wu_units(97)] == [32, 32, 32, 1]
+    assert wu_units(31) == [(0, 32, 31)] and wu_units(21) == [(0, 16, 16), (16, 4, 4), (20, 1, 1)]
+
+
 @pytest.mark.parametrize("N", [1, 2, 255, 1024, 5000, 65536, 262144, 1 << 20])
 def test_plan_invariants(B, N):
-    for n_act in sorted({1, 2, 7, 16, 17, 64, 96, 97, 512, 1024, 1025, 4096, 32768, N // 3 + 1, N} & set(range(1, N + 1)) | {N}):
+    for n_act in sorted({1, 2, 7, 16, 17, 64, 96, 97, 512, 1024, 1025, 4096, 16383, 16384, 32768, N // 3 + 1, N} & set(range(1, N + 1)) | {N}):
         for n_sm in (148, 132, 8):
             p = B.nb_plan_force(N, n_act, n_sm)
             Npad = (N + 255) // 256 * 256
-            assert p.kernel == (1 if n_act <= 16 else 2 if n_act <= 96 else 0)
-            assert p.sub == (4 if p.kernel == 2 else 1) and p.unit == (2 if p.kernel == 1 else 128 // p.sub)
-            unit, n_tiles = p.unit, Npad // p.tile
-            assert unit >= 1 and Npad % p.tile == 0 and p.n_units == (n_act + unit - 1) // unit
-            assert 1 <= p.ctas_per_sm <= 32 and p.grid <= n_sm * p.ctas_per_sm
+            assert p.kernel == (0 if n_act >= 16384 else 1)
+            assert p.unit == (128 if p.kernel == 0 else 32) and p.tile == (128 if p.kernel == 0 else 64)
+            n_tiles = Npad // p.tile
+            assert Npad % p.tile == 0
+            assert p.n_units == ((n_act + 127) // 128 if p.kernel == 0 else len(wu_units(n_act)))
+            assert p.predict_in_force == (1 if p.kernel == 1 and p.n_units <= 2 else 0)
+            assert 1 <= p.ctas_per_sm <= 32 and 1 <= p.grid <= n_sm * p.ctas_per_sm
             S, st = p.n_split, p.slice_tiles
-            assert S >= 1 and st >= 1 and p.grid >= 1
+            assert S >= 1 and st >= 1
             assert S * st >= n_tiles and (S - 1) * st < n_tiles            # slices cover all j-tiles, none empty
-            assert S * p.sub * p.n_units * unit <= 8 * Npad + (1 << 19)    # partial-sum buffer capacity
+            rows = p.n_units * 128 if p.kernel == 0 else n_act
+            assert S * rows <= 8 * Npad + (1 << 19)                        # partial-sum buffer capacity
             # small active sets are split so that the device is filled (PAPER.md:59-65)
-            resident = n_sm * p.ctas_per_sm * (8 if p.kernel == 1 else 1)       # lanes-over-j: 8 warps per CTA
+            resident = n_sm * p.ctas_per_sm * (4 if p.kernel == 1 else 1)       # warp units: 4 warps per CTA
             if p.n_units < resident and n_tiles >= 16 * resident:
                 assert p.n_units * S >= 0.5 * resident
 

@@ -84,7 +84,8 @@ def test_config1_force_and_8_steps(B, oracle):
 
 
 # ------------------------------------------------------------------ force kernel shapes, ragged sizes, edge cases
-@pytest.mark.parametrize("N,eps,masses", [(1000, 1e-3, "equal"), (4099, 1e-4, "kroupa"), (2, 0.0, "equal"), (257, 0.0, "kroupa")])
+@pytest.mark.parametrize("N,eps,masses", [(1000, 1e-3, "equal"), (4099, 1e-4, "kroupa"), (2, 0.0, "equal"), (257, 0.0, "kroupa"),
+                                          (16500, 0.0, "kroupa")])
 def test_force_parity_active_sets(B, oracle, N, eps, masses):
     m, x, v = W.plummer(N, 1000 + N, masses)
     g = B.System(m, x, v, eps)
@@ -92,14 +93,16 @@ def test_force_parity_active_sets(B, oracle, N, eps, masses):
     g.nb_predict(2.0 ** -9); g.nb_force(outputs=False); g.nb_corrector(None, 2.0 ** -9)
     g.nb_predict(2.0 ** -9 + 2.0 ** -11)
     rng = np.random.default_rng(N)
-    sizes = sorted({1, 2, 3, 16, 17, 31, 33, 64, 96, 97, 129, 255, 1023, 1024, 1025, 2049, N} & set(range(1, N + 1)) | {N})
+    sizes = sorted({1, 2, 3, 5, 6, 7, 11, 13, 16, 17, 21, 24, 31, 33, 64, 96, 97, 129, 255, 1023, 1024, 1025, 2049, N} & set(range(1, N + 1)) | {N})
+    if N > 10000:
+        sizes = [1, 19, 16383, 16384, N]                 # around the switch to CTA tiles; N = 128 * 128 + 116 is ragged
     for n_act in sizes:
         idx = None if n_act == N else rng.choice(N, n_act, replace=False).astype(np.int32)
         got = g.nb_force(idx)
         ref = oracle_on_gpu_records(oracle, g, eps, idx)
         assert_force_parity(got, ref)
         plan = B.nb_plan_force(N, n_act, 148)
-        assert plan.kernel == (1 if n_act <= 16 else 2 if n_act <= 96 else 0)   # all three kernel shapes
+        assert plan.kernel == (0 if n_act >= 16384 else 1)                      # CTA tiles / warp units
     # permuted full list: row k <-> idx[k]
     perm = rng.permutation(N).astype(np.int32)
     got = g.nb_force(perm)
@@ -378,7 +381,7 @@ def test_config3_full_size_sampled_block_steps(B, oracle):
         assert np.array_equal(get("DT"), o.dt), "time-step levels"
         # resynchronise the oracle's x, v, crackle with the GPU's (round-off level) so that the next schedule stays comparable
         o.x[acto], o.v[acto], o.c[acto] = get("X")[acto], get("V")[acto], get("C")[acto]
-    assert 1 in kernels                                                          # the tiny-active-set shape was exercised
+    assert 1 in kernels                                                          # the warp-unit shape was exercised
     g.nb_free()
 
 
