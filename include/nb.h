@@ -69,7 +69,17 @@ typedef struct {
                                0 = default: on for host-pointer contexts (those calls synchronise anyway), off for
                                device-pointer contexts (calls stay asynchronous; indices are then the caller's contract);
                                1 = always on; -1 = always off. */
+    int precision;          /* nb_precision: 0 = NB_PREC_FP64 (default: everything fp64, the north star's 1e-11);
+                               1 = NB_PREC_MIXED, the throughput mode of the paper's template ("DP ... to
+                               calculate reciprocal distances and to cumulate accelerations", SP elsewhere): position
+                               differences in fp64, the rest of the pair in fp32, fp32 sums flushed into fp64 accumulators
+                               every 128 j-particles.  Applies to 6th-order evaluations that run as CTA tiles (nb_plan.kernel
+                               == 0: large active sets); smaller active sets and all O(N) steps stay fp64.  Accuracy about
+                               1e-6 per particle (measured against the oracle: DESIGN.md 11), so the time-step criterion and
+                               the energy error are those of a single-precision force.  NB_EINVAL with order 4 or 8. */
 } nb_config;
+
+typedef enum { NB_PREC_FP64 = 0, NB_PREC_MIXED = 1 } nb_precision;
 
 /* Selectors of nb_get_state / nb_set_state.  Width = doubles per particle. */
 typedef enum {
@@ -186,8 +196,8 @@ int nb_next_block(nb_ctx* ctx, double* t_next, int32_t* active_idx, int64_t* n_a
  * repeats { nb_next_block; stop if t_next > t_end; nb_predict(t_next); nb_force(internal list);
  * nb_corrector(internal list, per-particle dt) } at most max_steps times.  Every decision of a step -
  * t_next, the active list, n_act, the j-split of the force launch (reading R15; "determined
- * step by step") - is taken on the device, and one step is one replay of a CUDA graph of four kernels
- * (scheduler, predictor, force, reduction + corrector); for small active sets the force kernel predicts the
+ * step by step") - is taken on the device, and a step is four kernels (scheduler, predictor, force, reduction +
+ * corrector) inside a CUDA graph that holds eight steps; for small active sets the force kernel predicts the
  * j-records it reads and the predictor's pass is skipped.  The host enqueues batches of replays and reads
  * the counters after each batch.  The arithmetic and its order are those of the separate calls: states
  * agree bit for bit.  The predicted records (NB_XP ...) are not defined afterwards.
@@ -196,6 +206,15 @@ int nb_next_block(nb_ctx* ctx, double* t_next, int32_t* active_idx, int64_t* n_a
  */
 int nb_run_blocks(nb_ctx* ctx, double t_end, int64_t max_steps, int64_t* steps_done, double* t_last,
                   int64_t* sum_n_act);
+
+/*
+ * nb_step_log — the device's own record of the most recent block steps nb_run_blocks took (up to 8192): for each, the
+ * number of active particles and the device clock (%globaltimer) read by the step's last kernel, in microseconds relative
+ * to the first returned step.  Differences of consecutive stamps are the full cost of a block step on the device, launch
+ * gaps included - the per-step figures of profiles/ come from here.  n_act, t_us: HOST arrays of `capacity` entries.
+ * Returns the number of entries written (oldest first), or a negative nb_status.  Synchronises the stream.
+ */
+int64_t nb_step_log(nb_ctx* ctx, int64_t capacity, int64_t* n_act, double* t_us);
 
 /* Read / write one field for the particles idx[0..n) (h/d; NULL = the first n in index order). */
 int nb_get_state(nb_ctx* ctx, int field, const int32_t* idx, int64_t n, double* out);
@@ -214,6 +233,11 @@ int nb_energy(nb_ctx* ctx, double* kinetic, double* potential);
  * longer list).  Synchronises the stream.  n == 0 is NB_OK.  (the active subset, m <= N.)
  */
 int nb_check_indices(nb_ctx* ctx, const int32_t* idx, int64_t n, int unique);
+
+/* CTAs of force kernel shape `kernel` (nb_plan.kernel: 0 or 1) that the device keeps resident per multiprocessor for this
+ * context's order, as the occupancy calculator reports it; the launch plan assumes nb_plan.ctas_per_sm.  NB_EINVAL (< 0)
+ * on a bad argument. */
+int nb_resident_ctas(const nb_ctx* ctx, int kernel);
 
 /* Kernel launches issued by this context so far (what bench.py reports as gpu_launches). */
 int64_t nb_launch_count(const nb_ctx* ctx);

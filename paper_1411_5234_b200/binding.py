@@ -16,12 +16,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libnb.so")
 
 NB_OK, NB_EINVAL, NB_ENOMEM, NB_ESTATE, NB_ECUDA = 0, -1, -2, -3, -4
+NB_PREC_FP64, NB_PREC_MIXED = 0, 1
 FIELDS = dict(M=0, X=1, V=2, A=3, J=4, S=5, C=6, T=7, DT=8, XP=9, VP=10, AP=11, A4=12, A5=13, JP=14)
 _WIDTH = {0: 1, 7: 1, 8: 1}
 ACTIVE_INTERNAL = C.c_void_p(1)
 
 EXPORTS = ["nb_workspace_bytes", "nb_plan_force", "nb_set_max_split", "nb_init", "nb_predict", "nb_force", "nb_force_crackle", "nb_corrector",
-           "nb_next_block", "nb_run_blocks", "nb_get_state", "nb_set_state", "nb_energy", "nb_check_indices",
+           "nb_next_block", "nb_run_blocks", "nb_get_state", "nb_set_state", "nb_energy", "nb_check_indices", "nb_resident_ctas", "nb_step_log",
            "nb_launch_count", "nb_last_force_ms", "nb_strerror", "nb_last_error", "nb_free"]
 
 
@@ -29,7 +30,7 @@ class nb_config(C.Structure):
     _fields_ = [("device", C.c_int), ("stream", C.c_void_p), ("workspace", C.c_void_p),
                 ("workspace_bytes", C.c_size_t), ("ptrs_on_device", C.c_int),
                 ("eta", C.c_double), ("eta_s", C.c_double), ("k_min", C.c_int), ("k_max", C.c_int), ("order", C.c_int),
-                ("check_indices", C.c_int)]
+                ("check_indices", C.c_int), ("precision", C.c_int)]
 
 
 class nb_plan(C.Structure):
@@ -71,6 +72,8 @@ def lib() -> C.CDLL:
     L.nb_set_state.argtypes = [vp, C.c_int, vp, i64, vp]; L.nb_set_state.restype = C.c_int
     L.nb_energy.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl)]; L.nb_energy.restype = C.c_int
     L.nb_check_indices.argtypes = [vp, vp, i64, C.c_int]; L.nb_check_indices.restype = C.c_int
+    L.nb_resident_ctas.argtypes = [vp, C.c_int]; L.nb_resident_ctas.restype = C.c_int
+    L.nb_step_log.argtypes = [vp, i64, vp, vp]; L.nb_step_log.restype = i64
     L.nb_launch_count.argtypes = [vp]; L.nb_launch_count.restype = i64
     L.nb_last_force_ms.argtypes = [vp]; L.nb_last_force_ms.restype = dbl
     L.nb_strerror.argtypes = [C.c_int]; L.nb_strerror.restype = C.c_char_p
@@ -113,7 +116,7 @@ class System:
     """
 
     def __init__(self, m, x, v, eps, host=True, device=0, eta=0.0, eta_s=0.0, k_min=0, k_max=0, stream=None, order=0,
-                 check_indices=0):
+                 check_indices=0, precision=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1411_5234_b200 needs a CUDA device; there is no CPU fallback")
@@ -129,7 +132,7 @@ class System:
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=f"cuda:{device}")
         base = (self.workspace.data_ptr() + 255) // 256 * 256
         self.cfg = nb_config(device, C.c_void_p(self.stream.cuda_stream), C.c_void_p(base), nbytes,
-                             0 if host else 1, eta, eta_s, k_min, k_max, order, check_indices)
+                             0 if host else 1, eta, eta_s, k_min, k_max, order, check_indices, precision)
         m, x, v = self._in(m, (self.N,)), self._in(x, (self.N, 3)), self._in(v, (self.N, 3))
         self._check(self.L.nb_init(C.byref(self.ctx), self.N, _ptr(m), _ptr(x), _ptr(v), float(eps), C.byref(self.cfg)))
 
@@ -241,6 +244,17 @@ class System:
         """NB_OK (0) or NB_EINVAL (-1): the status itself, not an exception."""
         idx = self._in(idx, dtype=np.int32)
         return self.L.nb_check_indices(self.ctx, _ptr(idx), int(idx.shape[0]), 1 if unique else 0)
+
+    def nb_step_log(self, capacity=8192):
+        """(n_act[int64], t_us[float64]) of the most recent block steps of nb_run_blocks, oldest first."""
+        na, tu = np.empty(capacity, dtype=np.int64), np.empty(capacity, dtype=np.float64)
+        n = self.L.nb_step_log(self.ctx, capacity, C.c_void_p(na.ctypes.data), C.c_void_p(tu.ctypes.data))
+        if n < 0:
+            self._check(int(n))
+        return na[:n], tu[:n]
+
+    def nb_resident_ctas(self, kernel):
+        return self.L.nb_resident_ctas(self.ctx, int(kernel))
 
     def nb_launch_count(self):
         return self.L.nb_launch_count(self.ctx)

@@ -23,7 +23,7 @@ def main():
     ap.add_argument("--N", type=int, default=None)
     ap.add_argument("--t-end", type=float, default=0.125)
     ap.add_argument("--order", type=int, default=6)
-    ap.add_argument("--profile-steps", type=int, default=1500)
+    ap.add_argument("--profile-steps", type=int, default=3000)
     ap.add_argument("--eta", type=float, default=0.0, help="accuracy parameter of the time-step criterion (0: the order's default)")
     a = ap.parse_args()
     import torch
@@ -44,25 +44,19 @@ def main():
           f"{inter:.4e} interactions in {el:.3f} s = {inter / el:.4e} interactions/s; dE/E = {(K1 + W1) / (K0 + W0) - 1:.3e}")
     if a.profile_steps <= 0:
         return
-    rec = []
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    for _ in range(a.profile_steps):
-        e0.record()
-        s, _, n = g.nb_run_blocks(1e30, 1)
-        e1.record()
-        torch.cuda.synchronize()
-        if s == 1:
-            rec.append((n, e0.elapsed_time(e1) * 1e3))
-    rec = np.array(rec)
-    print(f"next {len(rec)} block steps, one graph replay each (CUDA events around the call, host round trip included):")
+    # per-step cost from the device's own step log (nb_step_log): differences of the device clock between consecutive steps
+    g.nb_run_blocks(1e30, a.profile_steps)
+    na, tu = g.nb_step_log(a.profile_steps)
+    rec = np.stack([na[1:], np.diff(tu)], axis=1)
+    print(f"next {len(rec)} block steps in one nb_run_blocks call; cost per step = difference of the device clock (nb_step_log):")
     print("| n_act | steps | median us/step | min us/step | mean n_act | FP64-pipe floor us (106 cycles per pair) |")
     print("|---|---|---|---|---|---|")
     for lo, hi in ((1, 1), (2, 4), (5, 16), (17, 32), (33, 96), (97, 256), (257, 1024), (1025, 8192), (8193, N)):
         sel = (rec[:, 0] >= lo) & (rec[:, 0] <= hi)
         if sel.any():
-            na, us = rec[sel, 0], rec[sel, 1]
-            floor = na.mean() * (N - 1) * 106 / (148 * 4 * 32 * 1.965e9) * 1e6
-            print(f"| {lo}..{hi} | {int(sel.sum())} | {np.median(us):.1f} | {us.min():.1f} | {na.mean():.1f} | {floor:.1f} |")
+            na_, us = rec[sel, 0], rec[sel, 1]
+            floor = na_.mean() * (N - 1) * 106 / (148 * 4 * 32 * 1.965e9) * 1e6
+            print(f"| {lo}..{hi} | {int(sel.sum())} | {np.median(us):.1f} | {us.min():.1f} | {na_.mean():.1f} | {floor:.1f} |")
     g.nb_free()
 
 

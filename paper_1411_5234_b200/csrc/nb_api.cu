@@ -38,6 +38,7 @@ struct Layout {
     uint32_t* idx_bitmap;               // one bit per particle + one flag word: index-list verification (nb_config.check_indices)
     int* queue;                         // work queue of the force kernels (2 counters)
     DevPlan* devplan;                   // plan and counters of the device-planned block steps (nb_run_blocks)
+    unsigned long long* steplog;        // [0] steps logged so far, then NB_STEP_LOG x (n_act, device clock in ns)
     size_t bytes;
     Layout(void* base, int64_t Npad)
     {
@@ -47,6 +48,7 @@ struct Layout {
         s.tn = c.take<double>(Npad);
         s.rec = c.take<double2>(Npad * REC_Q_MAX);          // 80-B records (112 B at the 8th order)
         s.st5 = c.take<double4>(Npad); s.st6 = c.take<double4>(Npad);
+        s.recm = c.take<float4>(Npad * 4);                  // mixed-precision records (used only with NB_PREC_MIXED)
         fa = c.take<double>(3 * Npad); fj = c.take<double>(3 * Npad); fs = c.take<double>(3 * Npad); fp = c.take<double>(Npad);
         fc = c.take<double>(3 * Npad); s.fc = fc; s.order = 6;
         partial = c.take<double>(13 * partial_rows(Npad));   // 10 components, 13 at the 8th order
@@ -56,6 +58,7 @@ struct Layout {
         idx_bitmap = c.take<uint32_t>(Npad / 32 + 64);      // [Npad/32] bits, then the flag word
         queue = c.take<int>(64);
         devplan = c.take<DevPlan>(1);
+        steplog = c.take<unsigned long long>(1 + 2 * NB_STEP_LOG);
         bytes = c.off;
     }
 };
@@ -79,6 +82,7 @@ struct nb_ctx {
     int64_t forced_n = -1;         // n_act of the last nb_force since the last predict (-1: none)
     int64_t sched_n = -1;          // length of the internal active list (-1: none)
     int64_t launches = 0;
+    int occ_li = 0, occ_wu = 0;    // CTAs of each force kernel shape that fit one SM (the plan assumes LI/WU_CTAS_PER_SM)
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     cudaGraphExec_t step_graph = nullptr;   // one device-planned block step (built on first use)
     bool ev_valid = false;
@@ -120,7 +124,7 @@ ForceArgs base_force_args(const nb_ctx* ctx)
 {
     ForceArgs A{};
     const StateArrays& s = ctx->L.s;
-    A.rec = s.rec;
+    A.rec = s.rec; A.recm = s.recm;
     A.st0 = s.st0; A.st1 = s.st1; A.st2 = s.st2; A.st3 = s.st3; A.st4 = s.st4; A.st5 = s.st5; A.st6 = s.st6;
     A.eps2 = eps2_is_zero(ctx->eps) ? 0.0 : ctx->eps * ctx->eps;
     A.partial = ctx->L.partial;
@@ -133,6 +137,7 @@ ForceArgs base_force_args(const nb_ctx* ctx)
 // of the force launch) -> predictor (returns at once when the force kernel predicts for itself) -> force (either shape,
 // from the plan) -> partial-sum reduction + corrector.
 constexpr int STEP_GRAPH_KERNELS = 4;
+constexpr int STEPS_PER_GRAPH = 8;      // block steps per graph replay: graph-to-graph hand-over costs more than an edge inside one
 
 int build_step_graph(nb_ctx* ctx)
 {
@@ -145,11 +150,14 @@ int build_step_graph(nb_ctx* ctx)
         ForceArgs A = base_force_args(ctx);
         A.idx = ctx->L.idx_sched;
         A.dp = ctx->L.devplan;
-        e = nb_launch_devstep_head(ctx->L.s, ctx->N, ctx->Npad, ctx->n_sm, ctx->L.idx_sched, ctx->L.idx_tmp, ctx->L.scratch, ctx->L.devplan,
-                                   cs, &launches);
-        if (e == cudaSuccess) e = nb_launch_force_devplan(A, eps2_is_zero(ctx->eps), ctx->order, ctx->n_sm, (int)ctx->Npad, cs, &launches);
-        if (e == cudaSuccess)
-            e = nb_launch_devstep_tail(ctx->L.s, ctx->n_sm, ctx->L.idx_sched, A, ctx->L.devplan, ctx->eta, ctx->k_min, ctx->k_max, cs, &launches);
+        for (int k = 0; k < STEPS_PER_GRAPH && e == cudaSuccess; ++k) {
+            e = nb_launch_devstep_head(ctx->L.s, ctx->N, ctx->Npad, ctx->n_sm, ctx->L.idx_sched, ctx->L.idx_tmp, ctx->L.scratch, ctx->L.devplan,
+                                       cs, &launches);
+            if (e == cudaSuccess) e = nb_launch_force_devplan(A, eps2_is_zero(ctx->eps), ctx->order, ctx->n_sm, (int)ctx->Npad, cs, &launches);
+            if (e == cudaSuccess)
+                e = nb_launch_devstep_tail(ctx->L.s, ctx->n_sm, ctx->L.idx_sched, A, ctx->L.devplan, ctx->L.steplog, ctx->eta, ctx->k_min,
+                                           ctx->k_max, cs, &launches);
+        }
         const cudaError_t e2 = cudaStreamEndCapture(cs, &graph);
         if (e == cudaSuccess) e = e2;
     }
@@ -157,7 +165,7 @@ int build_step_graph(nb_ctx* ctx)
     if (graph) cudaGraphDestroy(graph);
     cudaStreamDestroy(cs);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "block-step graph");
-    return launches == STEP_GRAPH_KERNELS ? NB_OK : NB_ECUDA;
+    return launches == STEP_GRAPH_KERNELS * STEPS_PER_GRAPH ? NB_OK : NB_ECUDA;
 }
 
 // Verify a DEVICE index list: all in [0, N) and, if `unique`, pairwise different.  One kernel marks a bitmap and raises
@@ -207,7 +215,7 @@ int plan_force(int64_t N, int64_t n_act, int n_sm, int64_t max_split, nb_plan* p
     if (!plan || N < 1 || n_act < 1 || n_act > N || n_sm < 1 || N > (int64_t(1) << 30) || max_split < 0) return NB_EINVAL;
     const PlanShape sh = nb_plan_shape(pad_n(N), n_act, n_sm, max_split);
     double cost;
-    const int64_t S = nb_best_split(sh, 1, 1, &cost);
+    const int64_t S = nb_best_split(sh, 0, 1, &cost);
     int64_t st;
     nb_split_cost(sh, S, &st);
     nb_plan p{};
@@ -274,6 +282,8 @@ int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const dou
     const int k_max = (cfg->k_min == 0 && cfg->k_max == 0) ? -3 : cfg->k_max;
     if (k_min > k_max || k_min < -1000 || k_max > 1000 || cfg->eta < 0 || cfg->eta_s < 0) return NB_EINVAL;
     if (cfg->order != 0 && cfg->order != 4 && cfg->order != 6 && cfg->order != 8) return NB_EINVAL;
+    if (cfg->precision != NB_PREC_FP64 && cfg->precision != NB_PREC_MIXED) return NB_EINVAL;
+    if (cfg->precision == NB_PREC_MIXED && cfg->order != 0 && cfg->order != 6) return NB_EINVAL;
     const int64_t Npad = pad_n(N);
     if (!cfg->workspace || ((uintptr_t)cfg->workspace % ALIGN) != 0 || cfg->workspace_bytes < Layout(nullptr, Npad).bytes)
         return NB_ENOMEM;
@@ -292,14 +302,17 @@ int nb_init(nb_ctx** out, int64_t N, const double* m, const double* x, const dou
     ctx->k_min = k_min; ctx->k_max = k_max;
     ctx->L = Layout(cfg->workspace, Npad);
     ctx->L.s.order = ctx->order;
+    if (cfg->precision != NB_PREC_MIXED) ctx->L.s.recm = nullptr;
 
     ON_DEVICE(ctx);
     CU(cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, ctx->device), "device attribute");
     CU(nb_force_setup(), "kernel attributes");
+    nb_force_occupancy(ctx->order, &ctx->occ_li, &ctx->occ_wu);
     CU(cudaEventCreate(&ctx->ev0), "event");
     CU(cudaEventCreate(&ctx->ev1), "event");
     CU(cudaMemsetAsync(ctx->L.scratch, 0, scratch_bytes(Npad), ctx->stream), "memset scratch");
     CU(cudaMemsetAsync(ctx->L.queue, 0, 64 * sizeof(int), ctx->stream), "memset queue");
+    CU(cudaMemsetAsync(ctx->L.steplog, 0, sizeof(unsigned long long), ctx->stream), "memset step log");
 
     const double *dm = m, *dx = x, *dv = v;
     if (!ctx->on_device) {
@@ -422,17 +435,17 @@ int nb_run_blocks(nb_ctx* ctx, double t_end, int64_t max_steps, int64_t* steps_d
     ctx->predicted = false; ctx->forced_n = -1; ctx->sched_n = -1;
     // The host cannot know when the device stops, so it enqueues batches of steps and looks at the counters after each;
     // steps enqueued after the stop flag is up return at once (every kernel checks it).
-    int64_t enqueued = 0;
-    int batch = 8;
+    int64_t enqueued = 0;                                   // block steps enqueued so far
+    int batch = 1;                                          // graph replays per batch (STEPS_PER_GRAPH block steps each)
     while (max_steps > 0) {
-        const int64_t n = std::min<int64_t>(batch, max_steps - enqueued);
+        const int64_t n = std::min<int64_t>(batch, (max_steps - enqueued + STEPS_PER_GRAPH - 1) / STEPS_PER_GRAPH);
         for (int64_t k = 0; k < n; ++k) CU(cudaGraphLaunch(ctx->step_graph, ctx->stream), "block-step graph launch");
-        enqueued += n;
-        ctx->launches += n * STEP_GRAPH_KERNELS;
+        enqueued += n * STEPS_PER_GRAPH;
+        ctx->launches += n * STEP_GRAPH_KERNELS * STEPS_PER_GRAPH;
         CU(cudaMemcpyAsync(&h, ctx->L.devplan, sizeof h, cudaMemcpyDeviceToHost, ctx->stream), "read step control");
         CU(cudaStreamSynchronize(ctx->stream), "nb_run_blocks");
         if (h.stop || enqueued >= max_steps) break;
-        if (batch < 64) batch *= 2;
+        if (batch < 16) batch *= 2;
     }
     if (steps_done) *steps_done = h.steps_done;
     if (t_last) *t_last = h.t_last;
@@ -514,6 +527,35 @@ int nb_check_indices(nb_ctx* ctx, const int32_t* idx, int64_t n, int unique)
         didx = ctx->L.idx_tmp;
     }
     return verify_idx(ctx, didx, n, unique != 0);
+}
+
+int64_t nb_step_log(nb_ctx* ctx, int64_t capacity, int64_t* n_act, double* t_us)
+{
+    if (!ctx || capacity < 0 || (capacity > 0 && (!n_act || !t_us))) return NB_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if (guard.err != cudaSuccess) return NB_ECUDA;
+    static_assert(sizeof(unsigned long long) == 8, "log entries are 64-bit");
+    unsigned long long* h = new (std::nothrow) unsigned long long[1 + 2 * NB_STEP_LOG];
+    if (!h) return NB_ENOMEM;
+    int64_t n = NB_ECUDA;
+    if (cudaMemcpyAsync(h, ctx->L.steplog, (1 + 2 * NB_STEP_LOG) * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream) == cudaSuccess &&
+        cudaStreamSynchronize(ctx->stream) == cudaSuccess) {
+        const unsigned long long total = h[0];
+        n = (int64_t)std::min<unsigned long long>(std::min<unsigned long long>(total, NB_STEP_LOG), (unsigned long long)capacity);
+        for (int64_t k = 0; k < n; ++k) {                   // the last n steps, oldest first
+            const unsigned long long pos = (total - (unsigned long long)n + (unsigned long long)k) % NB_STEP_LOG;
+            n_act[k] = (int64_t)h[1 + 2 * pos];
+            t_us[k] = (double)(h[2 + 2 * pos] - h[2 + 2 * ((total - (unsigned long long)n) % NB_STEP_LOG)]) * 1e-3;
+        }
+    }
+    delete[] h;
+    return n;
+}
+
+int nb_resident_ctas(const nb_ctx* ctx, int kernel)
+{
+    if (!ctx || kernel < 0 || kernel > 1) return NB_EINVAL;
+    return kernel == 0 ? ctx->occ_li : ctx->occ_wu;
 }
 
 int64_t nb_launch_count(const nb_ctx* ctx) { return ctx ? ctx->launches : 0; }

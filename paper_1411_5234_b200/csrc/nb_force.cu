@@ -22,6 +22,7 @@
 #include "nb_internal.h"
 #include "nb_plan.h"
 #include "nb_predict.h"
+#include "nb_reduce.h"
 
 namespace {
 
@@ -316,6 +317,53 @@ __device__ __forceinline__ void pair_o8(const IPart& pi, const JRec& J, const do
 }
 
 // ---------------------------------------------------------------------------------------------
+// Mixed precision (nb_config.precision = NB_PREC_MIXED; HiGPUs uses DP "to calculate reciprocal distances
+// and to cumulate accelerations" and SP elsewhere).  Position differences in fp64, converted once; everything else of the
+// pair in fp32 (46 FP32-pipe instructions + 3 DADD + 3 F2F + 1 MUFU.RSQ); the fp32 sums of one j-tile are flushed into
+// fp64 accumulators by the caller.  The formulas are those of pair2 (R3); the order is left to ptxas.
+// ---------------------------------------------------------------------------------------------
+struct IPartM { double x, y, z; float vx, vy, vz, ax, ay, az; };
+struct SumsF { float ax, ay, az, jx, jy, jz, sx, sy, sz, p; };
+struct JRecM { double x, y, z; float m, vx, vy, vz, ax, ay, az; };
+
+__device__ __forceinline__ double f2_as_double(float lo, float hi) { return __hiloint2double(__float_as_int(hi), __float_as_int(lo)); }
+
+__device__ __forceinline__ JRecM load_recm(const float4* r)
+{
+    const float4 a = r[0], b = r[1], c = r[2], d = r[3];
+    return JRecM{f2_as_double(a.x, a.y), f2_as_double(a.z, a.w), f2_as_double(b.x, b.y), b.z, b.w, c.x, c.y, c.z, c.w, d.x};
+}
+
+__device__ __forceinline__ float rsqrt_f32(float s)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(s));
+    return y;
+}
+
+template <bool EPS0, bool MASK>
+__device__ __forceinline__ void pair_mixed(const IPartM& pi, const JRecM& J, const float eps2, const bool self, SumsF& S)
+{
+    const float dx = (float)(J.x - pi.x), dy = (float)(J.y - pi.y), dz = (float)(J.z - pi.z);   // DP difference, then SP
+    const float dvx = J.vx - pi.vx, dvy = J.vy - pi.vy, dvz = J.vz - pi.vz;
+    const float dax = J.ax - pi.ax, day = J.ay - pi.ay, daz = J.az - pi.az;
+    float s = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, eps2)));
+    if (EPS0 && MASK) s = self ? 1.f : s;                // eps = 0: keep the masked self pair finite
+    const float y = rsqrt_f32(s);                        // MUFU.RSQ: about 2^-22 relative
+    const float rv = fmaf(dx, dvx, fmaf(dy, dvy, dz * dvz));
+    const float B = fmaf(dx, dax, fmaf(dy, day, fmaf(dz, daz, fmaf(dvx, dvx, fmaf(dvy, dvy, dvz * dvz)))));
+    const float yy = y * y, mr = J.m * y, q = mr * yy, z = -3.f * yy;
+    const float alpha = yy * rv, c1 = z * rv;            // c1 = -3 alpha
+    const float c3 = fmaf(c1, alpha, z * B), c2 = c1 + c1;   // -3 beta, -6 alpha
+    const float ux = fmaf(c1, dx, dvx), uy = fmaf(c1, dy, dvy), uz = fmaf(c1, dz, dvz);
+    const float wx = fmaf(c2, ux, fmaf(c3, dx, dax)), wy = fmaf(c2, uy, fmaf(c3, dy, day)), wz = fmaf(c2, uz, fmaf(c3, dz, daz));
+    S.ax = fmaf(q, dx, S.ax); S.ay = fmaf(q, dy, S.ay); S.az = fmaf(q, dz, S.az);
+    S.jx = fmaf(q, ux, S.jx); S.jy = fmaf(q, uy, S.jy); S.jz = fmaf(q, uz, S.jz);
+    S.sx = fmaf(q, wx, S.sx); S.sy = fmaf(q, wy, S.sy); S.sz = fmaf(q, wz, S.sz);
+    S.p += (MASK && self) ? 0.f : mr;                    // j != i (eq. 1)
+}
+
+// ---------------------------------------------------------------------------------------------
 // records: one predicted particle is Q = 5 (7 at the 8th order) double2, nb_internal.h
 // ---------------------------------------------------------------------------------------------
 template <int ORDER>
@@ -442,8 +490,9 @@ __device__ __forceinline__ void li_body(const ForceArgs& A, double2* smem, unsig
     };
 
     uint32_t uses = 0;   // j-tiles this CTA has consumed so far: stage = uses % STAGES, parity = (uses / STAGES) & 1
-    for (;;) {
-        if (tid == 0) next_item = atomicAdd(A.queue, 1);
+    for (int round = 0;; ++round) {
+        // the first item is the CTA's own number, further ones come from the queue (which counts from gridDim.x)
+        if (tid == 0) next_item = round == 0 ? (int)blockIdx.x : (int)gridDim.x + atomicAdd(A.queue, 1);
         __syncthreads();
         const int item = next_item;
         __syncthreads();                                   // everyone has read next_item before it is overwritten
@@ -506,6 +555,74 @@ __device__ __forceinline__ void li_body(const ForceArgs& A, double2* smem, unsig
 }
 
 // ---------------------------------------------------------------------------------------------
+// CTA tiles in mixed precision (6th order): li_body's structure over the 64-B records; the fp32 sums of a j-tile (128
+// pairs per particle) are added into the fp64 accumulators after every tile ("DP ... to cumulate")
+// ---------------------------------------------------------------------------------------------
+constexpr uint32_t LIM_TILE_BYTES = LI_TJ * 64;
+
+template <bool EPS0>
+__device__ __forceinline__ void li_mixed_body(const ForceArgs& A, double2* smem_, unsigned long long* full)
+{
+    float4* smem = (float4*)smem_;
+    __shared__ int next_item_m;
+    const int tid = threadIdx.x;
+    const float eps2 = (float)A.eps2;
+
+    auto stage_tile = [&](int tile, int st) {
+        const uint32_t bar = smem_u32(&full[st]);
+        mbar_expect_tx(bar, LIM_TILE_BYTES);
+        bulk_g2s(smem_u32(smem + (size_t)st * LI_TJ * 4), A.recm + (size_t)tile * LI_TJ * 4, LIM_TILE_BYTES, bar);
+    };
+
+    uint32_t uses = 0;
+    for (int round = 0;; ++round) {
+        if (tid == 0) next_item_m = round == 0 ? (int)blockIdx.x : (int)gridDim.x + atomicAdd(A.queue, 1);
+        __syncthreads();
+        const int item = next_item_m;
+        __syncthreads();
+        if (item >= A.n_items) break;
+        const int unit = item % A.n_units, slice = item / A.n_units;
+        const int t0 = slice * A.slice_tiles;
+        const int nt = min(A.slice_tiles, A.n_tiles - t0);
+        if (tid == 0)
+            for (int f = 0; f < LI_STAGES && f < nt; ++f) stage_tile(t0 + f, (uses + f) & (LI_STAGES - 1));
+
+        const int k = unit * LI_UNIT + tid;
+        const bool valid = k < A.n_act;
+        const int kk = valid ? k : 0;
+        const int ii = A.idx ? A.idx[kk] : kk;
+        const JRecM me = load_recm(A.recm + (size_t)ii * 4);
+        const IPartM pi{me.x, me.y, me.z, me.vx, me.vy, me.vz, me.ax, me.ay, me.az};
+        Sums acc{0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+
+        for (int t = 0; t < nt; ++t) {
+            const uint32_t u = uses + t;
+            const int st = u & (LI_STAGES - 1);
+            mbar_wait(smem_u32(&full[st]), (u / LI_STAGES) & 1);
+            const int jbase = (t0 + t) * LI_TJ;
+            const bool own = (unsigned)(ii - jbase) < (unsigned)LI_TJ;
+            const float4* tp = smem + (size_t)st * LI_TJ * 4;
+            SumsF f{0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+            if (__any_sync(0xffffffffu, own)) {
+#pragma unroll 4
+                for (int jj = 0; jj < LI_TJ; ++jj) pair_mixed<EPS0, true>(pi, load_recm(tp + jj * 4), eps2, jbase + jj == ii, f);
+            } else {
+#pragma unroll 4
+                for (int jj = 0; jj < LI_TJ; ++jj) pair_mixed<EPS0, false>(pi, load_recm(tp + jj * 4), eps2, false, f);
+            }
+            acc.ax += (double)f.ax; acc.ay += (double)f.ay; acc.az += (double)f.az;
+            acc.jx += (double)f.jx; acc.jy += (double)f.jy; acc.jz += (double)f.jz;
+            acc.sx += (double)f.sx; acc.sy += (double)f.sy; acc.sz += (double)f.sz; acc.p += (double)f.p;
+            __syncthreads();
+            if (tid == 0 && t + LI_STAGES < nt) stage_tile(t0 + t + LI_STAGES, st);
+        }
+        uses += nt;
+        if (valid || A.n_split > 1) store_sums<6>(A, slice, k, acc);
+    }
+    if (tid == 0) queue_retire(A.queue, gridDim.x);
+}
+
+// ---------------------------------------------------------------------------------------------
 // warp units: a work item is (unit of p particles, j-slice), one warp per item
 // ---------------------------------------------------------------------------------------------
 template <bool EPS0, int ORDER, bool PREDICT>
@@ -523,18 +640,19 @@ __device__ __forceinline__ void wu_body(const ForceArgs& A, double2* smem, unsig
         bulk_g2s(smem_u32(ring + (size_t)st * WU_TJ * Q), A.rec + (size_t)tile * WU_TJ * Q, TILE_BYTES, bar);
     };
 
+    // every worker's first item is its own number (no queue traffic at all when there is at most one item per warp);
+    // further items come from the queue, which counts from n_workers
     const int n_workers = gridDim.x * WU_WARPS;
-    const bool queued = A.n_items > n_workers;              // at most one item per warp: no queue traffic at all
+    const bool queued = A.n_items > n_workers;
     uint32_t uses = 0;
     for (int round = 0;; ++round) {
         int item;
-        if (queued) {
+        if (round == 0) item = (int)(blockIdx.x * WU_WARPS + warp);
+        else if (queued) {
             item = 0;
-            if (lane == 0) item = atomicAdd(A.queue, 1);
+            if (lane == 0) item = n_workers + atomicAdd(A.queue, 1);
             item = __shfl_sync(0xffffffffu, item, 0);
-        } else {
-            item = round == 0 ? (int)(blockIdx.x * WU_WARPS + warp) : A.n_items;
-        }
+        } else item = A.n_items;
         if (item >= A.n_items) break;
         const int unit = item % A.n_units, slice = item / A.n_units;
         const int t0 = slice * A.slice_tiles;
@@ -642,6 +760,14 @@ __global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_li_kernel(co
     li_body<EPS0, ORDER>(A, dyn_smem, bars);
 }
 
+template <bool EPS0>
+__global__ void __launch_bounds__(LI_THREADS, LI_CTAS_PER_SM) force_lim_kernel(const ForceArgs A)
+{
+    __shared__ alignas(8) unsigned long long bars[N_BARS];
+    init_barriers(bars);
+    li_mixed_body<EPS0>(A, dyn_smem, bars);
+}
+
 template <bool EPS0, int ORDER>
 __global__ void __launch_bounds__(WU_THREADS, WU_CTAS_PER_SM) force_wu_kernel(const ForceArgs A)
 {
@@ -663,54 +789,24 @@ __global__ void __launch_bounds__(WU_THREADS, WU_CTAS_PER_SM) force_step_kernel(
     // CTAs (warps) beyond the work return before any set-up; with a queue the retire count needs every worker
     if (kernel == 1 && A.n_items <= (int)(gridDim.x * WU_WARPS) && (int)(blockIdx.x * WU_WARPS) >= A.n_items) return;
     init_barriers(bars);
-    if (kernel == 0) li_body<EPS0, ORDER>(A, dyn_smem, bars);
+    if (kernel == 0 && ORDER == 6 && A.recm) li_mixed_body<EPS0>(A, dyn_smem, bars);
+    else if (kernel == 0) li_body<EPS0, ORDER>(A, dyn_smem, bars);
     else if (A.predict) wu_body<EPS0, ORDER, true>(A, dyn_smem, bars);
     else wu_body<EPS0, ORDER, false>(A, dyn_smem, bars);
 }
 
 // ---------------------------------------------------------------------------------------------
-// partial-sum reduction (row a3).  T threads per active particle (T a power of two chosen from S on the host):
-// thread `lane` adds slices lane, lane + T, ... in increasing order, then the T lane sums are combined by a binary
-// tree in shared memory.  The order depends only on (S, T): bitwise reproducible.  T = 1 is the plain loop over
-// slices (large active sets, few slices: the loads of neighbouring threads coalesce over k).
+// partial-sum reduction (row a3) after nb_force: the fixed-order sum of nb_reduce.h, one pass per RED_THREADS / T particles
 // ---------------------------------------------------------------------------------------------
 template <int NC>
 __global__ void __launch_bounds__(RED_THREADS) reduce_partials_kernel(const ForceArgs A, int T)
 {
     __shared__ double sm[NC][RED_THREADS];
-    const int R = RED_THREADS / T;                         // active particles per block and pass
-    const int kl = threadIdx.x % R, lane = threadIdx.x / R;
+    const int R = RED_THREADS / T;
     for (int k0 = blockIdx.x * R; k0 < A.n_act; k0 += gridDim.x * R) {      // uniform over the block
-        const int k = k0 + kl;
         double r[NC];
-#pragma unroll
-        for (int c = 0; c < NC; ++c) r[c] = 0.0;
-        if (k < A.n_act) {
-            const size_t plane = (size_t)NC * A.ld;
-            const double* P = A.partial + (size_t)lane * plane + k;
-            for (int s = lane; s < A.n_split; s += T, P += (size_t)T * plane) {
-#pragma unroll
-                for (int c = 0; c < NC; ++c) r[c] += P[(size_t)c * A.ld];
-            }
-        }
-        for (int off = T >> 1; off > 0; off >>= 1) {
-            if (lane >= off && lane < 2 * off) {
-#pragma unroll
-                for (int c = 0; c < NC; ++c) sm[c][threadIdx.x] = r[c];
-            }
-            __syncthreads();
-            if (lane < off) {
-#pragma unroll
-                for (int c = 0; c < NC; ++c) r[c] += sm[c][threadIdx.x + off * R];
-            }
-            __syncthreads();
-        }
-        if (lane != 0 || k >= A.n_act) continue;
-        A.out_a[3 * k] = r[0]; A.out_a[3 * k + 1] = r[1]; A.out_a[3 * k + 2] = r[2];
-        A.out_j[3 * k] = r[3]; A.out_j[3 * k + 1] = r[4]; A.out_j[3 * k + 2] = r[5];
-        A.out_s[3 * k] = r[6]; A.out_s[3 * k + 1] = r[7]; A.out_s[3 * k + 2] = r[8];
-        A.out_p[k] = -r[9];
-        if (NC == 13) { A.out_c[3 * k] = r[10]; A.out_c[3 * k + 1] = r[11]; A.out_c[3 * k + 2] = r[12]; }
+        int k;
+        if (nb_reduce_pass<NC>(A.partial, A.ld, A.n_split, T, A.n_act, k0, sm, r, &k)) nb_store_totals<NC>(A, k, r);
     }
 }
 
@@ -728,26 +824,31 @@ constexpr size_t step_smem(int order) { return li_smem(order) > wu_smem(order) ?
         else                 { if (eps_is_zero) { CALL(true, 6); } else { CALL(false, 6); } } \
     } while (0)
 
-// dynamic shared memory above 48 KiB has to be allowed per kernel (warp units at the 8th order: 56 KiB)
+// dynamic shared memory above 48 KiB has to be allowed per kernel (warp units at the 8th order: 56 KiB), and four CTAs
+// of 40-56 KiB per SM need the largest shared-memory carve-out (the default heuristic may leave room for only two)
 cudaError_t nb_force_setup()
 {
     cudaError_t e = cudaSuccess;
     const bool eps_is_zero_values[2] = {false, true};
     for (int order : {4, 6, 8})
         for (bool eps_is_zero : eps_is_zero_values) {
+#define SETUP1(K, BYTES)                                                                                                          \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(BYTES));                 \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(K, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)
 #define SETUP(E, O)                                                                                                              \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(force_li_kernel<E, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)li_smem(O)); \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(force_wu_kernel<E, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wu_smem(O)); \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(force_step_kernel<E, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)step_smem(O))
+    SETUP1((force_li_kernel<E, O>), li_smem(O)); SETUP1((force_wu_kernel<E, O>), wu_smem(O)); SETUP1((force_step_kernel<E, O>), step_smem(O))
             NB_DISPATCH(SETUP);
 #undef SETUP
+#undef SETUP1
         }
     return e;
 }
 
 cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps_is_zero, int order, cudaStream_t st, int* launches)
 {
-#define LI(E, O) force_li_kernel<E, O><<<plan.grid, LI_THREADS, li_smem(O), st>>>(args)
+#define LI(E, O)                                                                                         \
+    if (O == 6 && args.recm) force_lim_kernel<E><<<plan.grid, LI_THREADS, LI_STAGES * LIM_TILE_BYTES, st>>>(args); \
+    else force_li_kernel<E, O><<<plan.grid, LI_THREADS, li_smem(O), st>>>(args)
 #define WU(E, O) force_wu_kernel<E, O><<<plan.grid, WU_THREADS, wu_smem(O), st>>>(args)
     if (plan.kernel == 0) NB_DISPATCH(LI);
     else NB_DISPATCH(WU);
@@ -779,8 +880,12 @@ cudaError_t nb_launch_force_devplan(const ForceArgs& args_, bool eps_is_zero, in
     return cudaGetLastError();
 }
 
-void nb_force_occupancy(int* li, int* wu)
+void nb_force_occupancy(int order, int* li, int* wu)
 {
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(li, force_li_kernel<false, 6>, LI_THREADS, li_smem(6));
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(wu, force_wu_kernel<false, 6>, WU_THREADS, wu_smem(6));
+    const bool eps_is_zero = false;
+#define OCC(E, O)                                                                                                   \
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(li, force_li_kernel<E, O>, LI_THREADS, li_smem(O));                \
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(wu, force_wu_kernel<E, O>, WU_THREADS, wu_smem(O))
+    NB_DISPATCH(OCC);
+#undef OCC
 }

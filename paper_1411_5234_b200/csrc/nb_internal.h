@@ -10,6 +10,8 @@
 //   bank conflicts: all lanes reading one record (broadcast) and every lane reading its own record (16-B pieces at an
 //   80-B / 112-B stride fall into eight different 16-B bank groups per quarter warp).
 //   Padded to a multiple of NB_PAD particles with massless records far away (they contribute exactly 0).
+//   Mixed precision (nb_config.precision) adds a second record array of 64 B per particle, four 16-B pieces:
+//     (x, y) fp64 | z fp64, (m, vx) fp32 | (vy, vz, ax, ay) fp32 | (az, -, -, -) fp32
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -39,12 +41,14 @@ constexpr int WU_CTAS_PER_SM = 4;
 constexpr int WU_TJ = 64;                    // j-records per stage of a warp's ring
 constexpr int WU_STAGES = 2;
 constexpr int RED_THREADS = 256;             // threads per block of the partial-sum reduction
+constexpr int NB_STEP_LOG = 8192;            // block steps the device-side step log of nb_run_blocks remembers
 
 struct DevPlan;   // nb_plan.h
 
 struct ForceArgs {
     const double2* rec;      // predicted records (padded), nb_rec_q(order) double2 each
     const double4 *st0, *st1, *st2, *st3, *st4, *st5, *st6;   // state: read when the kernel predicts the records itself
+    const float4* recm;      // mixed-precision records (64 B: x, y, z fp64; m, vx, vy, vz, ax, ay, az fp32), or nullptr
     const int32_t* idx;      // active indices or nullptr (i = k)
     int n_act;
     int n_units;             // i-tiles (kernel 0) or warp units (kernel 1)
@@ -69,12 +73,13 @@ cudaError_t nb_force_setup();   // once per process and device: shared-memory at
 cudaError_t nb_launch_force(const nb_plan& plan, const ForceArgs& args, bool eps_is_zero, int order, cudaStream_t st, int* launches);
 // device-planned (nb_run_blocks): ONE launch at the full grid; the kernel takes shape and sizes from the DevPlan
 cudaError_t nb_launch_force_devplan(const ForceArgs& args, bool eps_is_zero, int order, int n_sm, int Npad, cudaStream_t st, int* launches);
-void nb_force_occupancy(int* li_ctas_per_sm, int* wu_ctas_per_sm);
+void nb_force_occupancy(int order, int* li_ctas_per_sm, int* wu_ctas_per_sm);
 
 // nb_step.cu
 struct StateArrays {
     double4 *st0, *st1, *st2, *st3, *st4; double* dt; double* tn; double2* rec;
     double4 *st5, *st6;   // 8th order: st5 = (a4x, a4y, a4z, a5x), st6 = (a5y, a5z, -, -), a4 = d4a/dt4, a5 = d5a/dt5
+    float4* recm;         // mixed precision (nb_config.precision): 64-B records written beside rec, else nullptr
     const double* fc;     // 8th order: crackle of the last evaluation, row k <-> active_idx[k]
     int order;            // 4, 6 or 8
 };
@@ -95,6 +100,6 @@ cudaError_t nb_launch_next_block(const StateArrays& s, int64_t N, int32_t* activ
 cudaError_t nb_launch_devstep_head(const StateArrays& s, int64_t N, int64_t Npad, int n_sm, int32_t* active, int32_t* cand, void* scratch,
                                    DevPlan* dp, cudaStream_t st, int* launches);
 cudaError_t nb_launch_devstep_tail(const StateArrays& s, int n_sm, const int32_t* active, const ForceArgs& fargs, DevPlan* dp,
-                                   double eta, int k_min, int k_max, cudaStream_t st, int* launches);
+                                   unsigned long long* steplog, double eta, int k_min, int k_max, cudaStream_t st, int* launches);
 cudaError_t nb_launch_energy(const StateArrays& s, int64_t N, const double* pot, double* scratch, cudaStream_t st, int* launches);
 cudaError_t nb_launch_check_idx(const int32_t* idx, int64_t n, int64_t N, uint32_t* bitmap, uint32_t* flag, bool unique, cudaStream_t st);

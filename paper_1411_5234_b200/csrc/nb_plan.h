@@ -19,12 +19,15 @@ NB_HD int64_t nb_max64(int64_t a, int64_t b) { return a > b ? a : b; }
 NB_HD int nb_pow2ceil(int v) { int p = 1; while (p < v) p <<= 1; return p; }
 NB_HD int nb_pow2floor(int v) { int p = 1; while (2 * p <= v) p <<= 1; return p; }
 
-// n_act at and above which the evaluation runs as CTA tiles of 128 particles (kernel 0); below, as warp units (kernel 1)
-#ifdef NB_EXP_LI_MIN_ACT   /* TEMPORARY experiment switch, removed before commit */
-constexpr int64_t LI_MIN_ACT = NB_EXP_LI_MIN_ACT;
-#else
-constexpr int64_t LI_MIN_ACT = 16384;
-#endif
+// Which shape: CTA tiles of 128 particles run the pipe 6-12 % better than warp units (shared j-tiles, longer items;
+// measured) but leave the lanes of a ragged last tile idle; warp units waste nothing.  CTA tiles are taken
+// from 256 active particles on when at least 93 % of their lanes hold a particle.
+constexpr int64_t LI_MIN_ACT = 256;
+NB_HD bool nb_use_cta_tiles(int64_t n_act)
+{
+    const int64_t lanes = (n_act + LI_UNIT - 1) / LI_UNIT * LI_UNIT;
+    return n_act >= LI_MIN_ACT && n_act * 100 >= lanes * 93;
+}
 // block steps whose evaluation has at most this many warp units let the force kernel predict the j-records itself
 constexpr int PIF_MAX_UNITS = 2;
 
@@ -86,7 +89,7 @@ NB_HD PlanShape nb_plan_shape(int64_t Npad, int64_t n_act, int n_sm, int64_t max
 {
     PlanShape p;
     const int64_t rows = nb_partial_rows(Npad);
-    if (n_act >= LI_MIN_ACT) {
+    if (nb_use_cta_tiles(n_act)) {
         // CTA tiles: a work item is (i-tile of 128 particles, j-slice); resident = CTAs on the device
         p.kernel = 0; p.unit = LI_UNIT; p.tile = LI_TJ; p.ctas_per_sm = LI_CTAS_PER_SM; p.fixed = 2.0;
         p.n_units = (n_act + LI_UNIT - 1) / LI_UNIT;
@@ -96,7 +99,7 @@ NB_HD PlanShape nb_plan_shape(int64_t Npad, int64_t n_act, int n_sm, int64_t max
         p.s_max = nb_min64(nb_min64(rows / (p.n_units * LI_UNIT), 2048), p.n_tiles / 2);
     } else {
         // warp units: a work item is (unit, j-slice); resident = warps on the device
-        p.kernel = 1; p.unit = 32; p.tile = WU_TJ; p.ctas_per_sm = WU_CTAS_PER_SM; p.fixed = 0.5;
+        p.kernel = 1; p.unit = 32; p.tile = WU_TJ; p.ctas_per_sm = WU_CTAS_PER_SM; p.fixed = 1.0;
         p.n_units = nb_wu_count(n_act, &p.work, &p.w_max);
         p.n_tiles = Npad / WU_TJ;
         p.resident = (int64_t)n_sm * WU_CTAS_PER_SM * WU_WARPS;
@@ -135,15 +138,54 @@ NB_HD double nb_split_cost(const PlanShape& p, int64_t S, int64_t* slice_tiles)
     return (double)items * c_avg / (double)p.resident + 0.7 * c_max;
 }
 
-// The split is the S in [1, s_max] of least cost, the smallest such S on ties (S = 1 is always a candidate).
-NB_HD int64_t nb_best_split(const PlanShape& p, int64_t s_begin, int64_t s_stride, double* best_cost)
+// The candidates for S.  The cost above is piecewise: flat or falling up to a whole number of rounds (items = k x
+// resident), and beyond a few rounds smooth with a minimum near S* = sqrt(tail x n_tiles x resident / (n_units x
+// fixed)).  So instead of all S in [1, s_max] (tens of thousands of 64-bit divisions - microseconds of every block step
+// when the plan is made on the device) only these are examined: S = 1, S = s_max, the largest S with items <= k x
+// resident for k = 1 .. 4, and S*; each with the neighbouring slice lengths.  Candidate c -> a valid S (one that leaves
+// no slice empty) or 0.
+constexpr int NB_SPLIT_CANDIDATES = 24;
+
+NB_HD int64_t nb_isqrt_floor(double x)
+{
+    int64_t r = 1;
+    while ((double)(r * 2) * (double)(r * 2) <= x) r *= 2;            // no libm: identical on host and device
+    for (int64_t b = r / 2; b > 0; b /= 2)
+        if ((double)(r + b) * (double)(r + b) <= x) r += b;
+    return r;
+}
+
+NB_HD int64_t nb_split_candidate(const PlanShape& p, int c)
+{
+    int64_t target;                                         // an S to aim for; snapped to a valid one below
+    const int group = c / 3, var = c % 3;                   // var: slice length st, st + 1, st - 1
+    if (group == 0) target = 1;
+    else if (group == 1) target = p.s_max;
+    else if (group <= 5) target = (int64_t)(group - 1) * p.resident / p.n_units;
+    else if (group == 6) {
+        const double tail = p.kernel == 0 ? 0.9 : 0.7 * p.w_max;
+        target = nb_isqrt_floor(tail * (double)p.n_tiles * (double)p.resident / ((double)p.n_units * p.fixed));
+    } else target = p.n_units <= p.resident ? p.resident / p.n_units * 2 / 3 : 0;    // group 7: a round two thirds full
+    if (target < 1) return 0;
+    target = nb_min64(target, p.s_max);
+    int64_t st = (p.n_tiles + target - 1) / target + (var == 1 ? 1 : var == 2 ? -1 : 0);
+    if (st < 1 || st > p.n_tiles) return 0;
+    const int64_t S = (p.n_tiles + st - 1) / st;
+    return S >= 1 && S <= p.s_max ? S : 0;
+}
+
+// The split is the candidate S of least cost, the smallest such S on ties.  Candidates c_begin, c_begin + c_stride, ...
+// (the host takes all of them, the device spreads them over a warp).
+NB_HD int64_t nb_best_split(const PlanShape& p, int c_begin, int c_stride, double* best_cost)
 {
     int64_t best = 0;
     double bc = 1e300;
-    for (int64_t S = s_begin; S <= p.s_max; S += s_stride) {
+    for (int c = c_begin; c < NB_SPLIT_CANDIDATES; c += c_stride) {
+        const int64_t S = nb_split_candidate(p, c);
+        if (S == 0) continue;
         int64_t st;
-        const double c = nb_split_cost(p, S, &st);
-        if (c >= 0.0 && c < bc) { bc = c; best = S; }
+        const double cost = nb_split_cost(p, S, &st);
+        if (cost >= 0.0 && (cost < bc || (cost == bc && S < best))) { bc = cost; best = S; }
     }
     *best_cost = bc;
     return best;

@@ -4,6 +4,7 @@
 #include "nb_internal.h"
 #include "nb_plan.h"
 #include "nb_predict.h"
+#include "nb_reduce.h"
 
 namespace {
 
@@ -17,6 +18,14 @@ __device__ __forceinline__ void write_pad_record(const StateArrays& s, int64_t i
     r[0] = make_double2(3e33, 3e33);
     r[1] = make_double2(3e33, 0.0);
     for (int q = 2; q < nb_rec_q(s.order); ++q) r[q] = make_double2(0.0, 0.0);
+    if (s.recm) {
+        const double far = 3e33;
+        const float lo = __int_as_float(__double2loint(far)), hi = __int_as_float(__double2hiint(far));
+        s.recm[4 * i] = make_float4(lo, hi, lo, hi);
+        s.recm[4 * i + 1] = make_float4(lo, hi, 0.f, 0.f);
+        s.recm[4 * i + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
+        s.recm[4 * i + 3] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
 }
 
 // ------------------------------------------------------------------ init: AoS inputs -> packed state
@@ -56,6 +65,15 @@ __global__ void __launch_bounds__(TPB) predict_kernel(StateArrays s, int64_t N, 
     double2* out = s.rec + i * Q;
 #pragma unroll
     for (int q = 0; q < Q; ++q) out[q] = rec[q];
+    if (s.recm) {                                          // mixed precision: fp64 position, fp32 copies of the rest
+        float4* om = s.recm + i * 4;
+        om[0] = make_float4(__int_as_float(__double2loint(rec[0].x)), __int_as_float(__double2hiint(rec[0].x)),
+                            __int_as_float(__double2loint(rec[0].y)), __int_as_float(__double2hiint(rec[0].y)));
+        om[1] = make_float4(__int_as_float(__double2loint(rec[1].x)), __int_as_float(__double2hiint(rec[1].x)),
+                            (float)rec[1].y, (float)rec[2].x);
+        om[2] = make_float4((float)rec[2].y, (float)rec[3].x, (float)rec[3].y, (float)rec[4].x);
+        om[3] = make_float4((float)rec[4].y, 0.f, 0.f, 0.f);
+    }
 }
 
 void launch_predict(const StateArrays& s, int64_t N, double t, bool own_time, const DevPlan* dp, cudaStream_t st)
@@ -259,12 +277,11 @@ __global__ void __launch_bounds__(TPB) corrector_kernel(StateArrays s, const int
 }
 
 // Device-planned block step (nb_run_blocks): the partial-sum reduction of row a3 and the corrector in ONE kernel.  The
-// sums are those of reduce_partials_kernel (nb_force.cu): T threads per active particle, thread `lane` adds slices lane,
-// lane + T, ... in increasing order, binary tree over the T lane sums - the same order, so the same bits - and the thread
-// that holds a particle's total stores it and corrects the particle.  S = 1: the force kernel stored the results itself.
+// sums are those of reduce_partials_kernel (nb_force.cu), both call nb_reduce_pass (nb_reduce.h) - the same order, so the
+// same bits - and the thread that holds a particle's total stores it and corrects the particle.  S = 1: the force kernel stored the results itself.
 template <int NC>
 __global__ void __launch_bounds__(RED_THREADS) reduce_correct_kernel(StateArrays s, const int32_t* idx, ForceArgs A, double eta3,
-                                                                     int k_min, int k_max, DevPlan* dp)
+                                                                     int k_min, int k_max, DevPlan* dp, unsigned long long* steplog)
 {
     __shared__ double sm[NC][RED_THREADS];
     if (dp->stop) return;
@@ -272,6 +289,12 @@ __global__ void __launch_bounds__(RED_THREADS) reduce_correct_kernel(StateArrays
     const double t_new = dp->t_next;
     if (blockIdx.x == 0 && threadIdx.x == 0) {             // last kernel of the step: book-keeping nobody else reads now
         dp->steps_done += 1; dp->steps_left -= 1; dp->sum_act += n_act; dp->t_last = t_new;
+        // step log (nb_step_log): n_act and the device clock, in a ring of NB_STEP_LOG entries after the running count
+        unsigned long long now;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+        const unsigned long long pos = steplog[0]++;
+        steplog[1 + 2 * (pos % NB_STEP_LOG)] = (unsigned long long)n_act;
+        steplog[2 + 2 * (pos % NB_STEP_LOG)] = now;
     }
     if (S <= 1) {
         for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n_act; k += gridDim.x * blockDim.x)
@@ -279,38 +302,11 @@ __global__ void __launch_bounds__(RED_THREADS) reduce_correct_kernel(StateArrays
         return;
     }
     const int R = RED_THREADS / T;                         // active particles per block and pass
-    const int kl = threadIdx.x % R, lane = threadIdx.x / R;
     for (int k0 = blockIdx.x * R; k0 < n_act; k0 += gridDim.x * R) {        // uniform over the block
-        const int k = k0 + kl;
         double r[NC];
-#pragma unroll
-        for (int c = 0; c < NC; ++c) r[c] = 0.0;
-        if (k < n_act) {
-            const size_t plane = (size_t)NC * ld;
-            const double* P = A.partial + (size_t)lane * plane + k;
-            for (int sl = lane; sl < S; sl += T, P += (size_t)T * plane) {
-#pragma unroll
-                for (int c = 0; c < NC; ++c) r[c] += P[(size_t)c * ld];
-            }
-        }
-        for (int off = T >> 1; off > 0; off >>= 1) {
-            if (lane >= off && lane < 2 * off) {
-#pragma unroll
-                for (int c = 0; c < NC; ++c) sm[c][threadIdx.x] = r[c];
-            }
-            __syncthreads();
-            if (lane < off) {
-#pragma unroll
-                for (int c = 0; c < NC; ++c) r[c] += sm[c][threadIdx.x + off * R];
-            }
-            __syncthreads();
-        }
-        if (lane != 0 || k >= n_act) continue;
-        A.out_a[3 * k] = r[0]; A.out_a[3 * k + 1] = r[1]; A.out_a[3 * k + 2] = r[2];
-        A.out_j[3 * k] = r[3]; A.out_j[3 * k + 1] = r[4]; A.out_j[3 * k + 2] = r[5];
-        A.out_s[3 * k] = r[6]; A.out_s[3 * k + 1] = r[7]; A.out_s[3 * k + 2] = r[8];
-        A.out_p[k] = -r[9];
-        if (NC == 13) { A.out_c[3 * k] = r[10]; A.out_c[3 * k + 1] = r[11]; A.out_c[3 * k + 2] = r[12]; }
+        int k;
+        if (!nb_reduce_pass<NC>(A.partial, ld, S, T, n_act, k0, sm, r, &k)) continue;
+        nb_store_totals<NC>(A, k, r);
         corrector_one(s, idx, k, 0.0, t_new, A.out_a, A.out_j, A.out_s, eta3, k_min, k_max);   // reads back what this thread stored
     }
 }
@@ -448,8 +444,17 @@ __global__ void __launch_bounds__(SCHED_TPB) sched_kernel(StateArrays s, int64_t
     __threadfence();
 
     // ---- the last block: global minimum, offsets of the blocks that attain it, ordered copy
+    // thread t looks after blocks t * per .. t * per + per - 1 (per = 1 up to 2^21 particles)
+    const int per = (B + SCHED_TPB - 1) / SCHED_TPB;
     double g = INFINITY;
-    for (int b = tid; b < B; b += SCHED_TPB) g = fmin(g, __ldcg(bmin_arr + b));
+    double bm0 = INFINITY;                                  // per == 1: this thread's block, kept in registers
+    unsigned int cn0 = 0;
+    if (per == 1) {
+        if (tid < B) { bm0 = __ldcg(bmin_arr + tid); cn0 = __ldcg(cnt_arr + tid); }
+        g = bm0;
+    } else {
+        for (int b = tid; b < B; b += SCHED_TPB) g = fmin(g, __ldcg(bmin_arr + b));
+    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) g = fmin(g, __shfl_xor_sync(0xffffffffu, g, o));
     __syncthreads();                                        // red[] is free again
@@ -459,12 +464,13 @@ __global__ void __launch_bounds__(SCHED_TPB) sched_kernel(StateArrays s, int64_t
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) g = fmin(g, __shfl_xor_sync(0xffffffffu, g, o));
     const double tn = g;
-    const int per = (B + SCHED_TPB - 1) / SCHED_TPB;        // consecutive blocks per thread
     unsigned int sum = 0;
-    for (int q = 0; q < per; ++q) {
-        const int b = tid * per + q;
-        if (b < B && __ldcg(bmin_arr + b) == tn) sum += __ldcg(cnt_arr + b);
-    }
+    if (per == 1) sum = bm0 == tn ? cn0 : 0;
+    else
+        for (int q = 0; q < per; ++q) {
+            const int b = tid * per + q;
+            if (b < B && __ldcg(bmin_arr + b) == tn) sum += __ldcg(cnt_arr + b);
+        }
     unsigned int n_tot;
     unsigned int run = block_excl_scan(sum, warp_tot, &n_tot);
     const long long n_act = n_tot;
@@ -473,48 +479,57 @@ __global__ void __launch_bounds__(SCHED_TPB) sched_kernel(StateArrays s, int64_t
         ((long long*)scratch)[1] = n_act;
         *done = 0;
     }
-    for (int q = 0; q < per; ++q) {
-        const int b = tid * per + q;
-        if (b < B) {
-            const bool hit = __ldcg(bmin_arr + b) == tn;
-            off_arr[b] = hit ? run : 0xffffffffu;
-            if (hit) run += __ldcg(cnt_arr + b);
+    if (per == 1) {
+        // offsets and counts of the blocks that attain the minimum go through shared memory (best_s / best_c are free)
+        unsigned int* s_off = (unsigned int*)best_s;
+        unsigned int* s_cnt = (unsigned int*)best_c;
+        s_off[tid] = run; s_cnt[tid] = sum;                 // sum = 0: nothing to copy
+        __syncthreads();
+        for (int b = warp; b < B; b += SCHED_TPB / 32) {
+            const unsigned int n = s_cnt[b], off = s_off[b];
+            const int32_t* src = cand + (int64_t)b * SCHED_CHUNK;
+            for (unsigned int i = lane; i < n; i += 32) active[off + i] = __ldcg(src + i);
         }
-    }
-    __syncthreads();                                        // off_arr (global) written by this block: visible after the barrier
-    for (int b = warp; b < B; b += SCHED_TPB / 32) {
-        const unsigned int off = __ldcg(off_arr + b);
-        if (off == 0xffffffffu) continue;
-        const unsigned int n = __ldcg(cnt_arr + b);
-        const int32_t* src = cand + (int64_t)b * SCHED_CHUNK;
-        for (unsigned int i = lane; i < n; i += 32) active[off + i] = __ldcg(src + i);
+        __syncthreads();                                    // best_s / best_c are reused by the plan below
+    } else {
+        for (int q = 0; q < per; ++q) {
+            const int b = tid * per + q;
+            if (b < B) {
+                const bool hit = __ldcg(bmin_arr + b) == tn;
+                off_arr[b] = hit ? run : 0xffffffffu;
+                if (hit) run += __ldcg(cnt_arr + b);
+            }
+        }
+        __syncthreads();                                    // off_arr (global) written by this block: visible after the barrier
+        for (int b = warp; b < B; b += SCHED_TPB / 32) {
+            const unsigned int off = __ldcg(off_arr + b);
+            if (off == 0xffffffffu) continue;
+            const unsigned int n = __ldcg(cnt_arr + b);
+            const int32_t* src = cand + (int64_t)b * SCHED_CHUNK;
+            for (unsigned int i = lane; i < n; i += 32) active[off + i] = __ldcg(src + i);
+        }
     }
     if (!dp) return;
     // device-planned block step (nb_run_blocks): decide whether the step is taken, and plan the force launch for its
-    // n_act with the functions the host uses (nb_plan.h); the candidates S are spread over the block's threads.
+    // n_act with the functions the host uses (nb_plan.h); the candidates S are spread over one warp.
     const bool stop = tn > dp->t_end || dp->steps_left <= 0 || n_act <= 0;
     if (stop) {
         if (tid == 0) { dp->stop = 1; dp->n_act = 0; }
         return;
     }
+    if (warp != 0) return;
     const PlanShape sh = nb_plan_shape(Npad, n_act, n_sm, dp->max_split);
     double cst;
-    const int64_t S = nb_best_split(sh, 1 + tid, SCHED_TPB, &cst);
-    best_c[tid] = cst; best_s[tid] = (int)S;               // S = 0: this thread had no candidate (cost 1e300)
-    __syncthreads();
-    for (int o = SCHED_TPB / 2; o > 0; o >>= 1) {
-        if (tid < o) {
-            const double c2 = best_c[tid + o];
-            const int s2 = best_s[tid + o];
-            const double c1 = best_c[tid];
-            const int s1 = best_s[tid];
-            // least cost; on ties the smaller S (as the host's ascending scan)
-            if (s2 != 0 && (s1 == 0 || c2 < c1 || (c2 == c1 && s2 < s1))) { best_c[tid] = c2; best_s[tid] = s2; }
-        }
-        __syncthreads();
+    long long S = nb_best_split(sh, lane, 32, &cst);          // S = 0: this lane had no candidate (cost 1e300)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double c2 = __shfl_xor_sync(0xffffffffu, cst, o);
+        const long long s2 = __shfl_xor_sync(0xffffffffu, S, o);
+        // least cost; on ties the smaller S (as the host's scan)
+        if (s2 != 0 && (S == 0 || c2 < cst || (c2 == cst && s2 < S))) { cst = c2; S = s2; }
     }
-    if (tid == 0) {
-        nb_fill_devplan(dp, sh, best_s[0], n_act);
+    if (lane == 0) {
+        nb_fill_devplan(dp, sh, S, n_act);
         dp->t_next = tn;
     }
 }
@@ -632,10 +647,10 @@ cudaError_t nb_launch_devstep_head(const StateArrays& s, int64_t N, int64_t Npad
 }
 
 cudaError_t nb_launch_devstep_tail(const StateArrays& s, int n_sm, const int32_t* active, const ForceArgs& fargs, DevPlan* dp,
-                                   double eta, int k_min, int k_max, cudaStream_t st, int* launches)
+                                   unsigned long long* steplog, double eta, int k_min, int k_max, cudaStream_t st, int* launches)
 {
-    if (s.order == 8) reduce_correct_kernel<13><<<n_sm * 4, RED_THREADS, 0, st>>>(s, active, fargs, eta_power(s.order, eta), k_min, k_max, dp);
-    else reduce_correct_kernel<10><<<n_sm * 4, RED_THREADS, 0, st>>>(s, active, fargs, eta_power(s.order, eta), k_min, k_max, dp);
+    if (s.order == 8) reduce_correct_kernel<13><<<n_sm * 4, RED_THREADS, 0, st>>>(s, active, fargs, eta_power(s.order, eta), k_min, k_max, dp, steplog);
+    else reduce_correct_kernel<10><<<n_sm * 4, RED_THREADS, 0, st>>>(s, active, fargs, eta_power(s.order, eta), k_min, k_max, dp, steplog);
     *launches += 1;
     return cudaGetLastError();
 }

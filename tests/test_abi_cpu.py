@@ -54,7 +54,7 @@ def test_build_staleness_tracks_every_header(B):
 
 def test_struct_layouts_match_header(B):
     # nb_config: int, void*, void*, size_t, int, double, double, int, int, int, int  (natural alignment)
-    assert C.sizeof(B.nb_config) == 72 and B.nb_config.order.offset == 64 and B.nb_config.check_indices.offset == 68
+    assert C.sizeof(B.nb_config) == 80 and B.nb_config.order.offset == 64 and B.nb_config.check_indices.offset == 68 and B.nb_config.precision.offset == 72
     assert B.nb_config.workspace.offset == 16 and B.nb_config.eta.offset == 40 and B.nb_config.k_max.offset == 60
     assert C.sizeof(B.nb_plan) == 48 and B.nb_plan.waves.offset == 40 and B.nb_plan.predict_in_force.offset == 32
 
@@ -94,11 +94,11 @@ def test_warp_unit_decomposition():
 
 @pytest.mark.parametrize("N", [1, 2, 255, 1024, 5000, 65536, 262144, 1 << 20])
 def test_plan_invariants(B, N):
-    for n_act in sorted({1, 2, 7, 16, 17, 64, 96, 97, 512, 1024, 1025, 4096, 16383, 16384, 32768, N // 3 + 1, N} & set(range(1, N + 1)) | {N}):
+    for n_act in sorted({1, 2, 7, 16, 17, 64, 96, 97, 255, 256, 300, 512, 1024, 1025, 1100, 4096, 16383, 16384, 32768, N // 3 + 1, N} & set(range(1, N + 1)) | {N}):
         for n_sm in (148, 132, 8):
             p = B.nb_plan_force(N, n_act, n_sm)
             Npad = (N + 255) // 256 * 256
-            assert p.kernel == (0 if n_act >= 16384 else 1)
+            assert p.kernel == (0 if n_act >= 256 and n_act * 100 >= 93 * 128 * ((n_act + 127) // 128) else 1)
             assert p.unit == (128 if p.kernel == 0 else 32) and p.tile == (128 if p.kernel == 0 else 64)
             n_tiles = Npad // p.tile
             assert Npad % p.tile == 0
@@ -130,13 +130,13 @@ def test_argument_validation_without_gpu(B):
     L = B.lib()
     ctx = C.c_void_p()
     m = np.ones(4); x = np.zeros((4, 3)); v = np.zeros((4, 3))
-    cfg = B.nb_config(0, None, None, 0, 0, 0, 0, 0, 0, 0, 0)
+    cfg = B.nb_config(0, None, None, 0, 0, 0, 0, 0, 0, 0, 0, 0)
     pm, px, pv = B._ptr(m), B._ptr(x), B._ptr(v)
     assert L.nb_init(C.byref(ctx), 4, pm, px, pv, 1e-3, C.byref(cfg)) == B.NB_ENOMEM       # no workspace
     assert L.nb_init(C.byref(ctx), 0, pm, px, pv, 1e-3, C.byref(cfg)) == B.NB_EINVAL
     assert L.nb_init(C.byref(ctx), 4, None, px, pv, 1e-3, C.byref(cfg)) == B.NB_EINVAL
     assert L.nb_init(C.byref(ctx), 4, pm, px, pv, float("nan"), C.byref(cfg)) == B.NB_EINVAL
-    bad = B.nb_config(0, None, None, 0, 0, 0, 0, -3, -20, 0, 0)                                   # k_min > k_max
+    bad = B.nb_config(0, None, None, 0, 0, 0, 0, -3, -20, 0, 0, 0)                                   # k_min > k_max
     assert L.nb_init(C.byref(ctx), 4, pm, px, pv, 1e-3, C.byref(bad)) == B.NB_EINVAL
     assert L.nb_predict(None, 0.0) == B.NB_EINVAL
     assert L.nb_force(None, None, 0, None, None, None, None) == B.NB_EINVAL

@@ -93,16 +93,16 @@ def test_force_parity_active_sets(B, oracle, N, eps, masses):
     g.nb_predict(2.0 ** -9); g.nb_force(outputs=False); g.nb_corrector(None, 2.0 ** -9)
     g.nb_predict(2.0 ** -9 + 2.0 ** -11)
     rng = np.random.default_rng(N)
-    sizes = sorted({1, 2, 3, 5, 6, 7, 11, 13, 16, 17, 21, 24, 31, 33, 64, 96, 97, 129, 255, 1023, 1024, 1025, 2049, N} & set(range(1, N + 1)) | {N})
+    sizes = sorted({1, 2, 3, 5, 6, 7, 11, 13, 16, 17, 21, 24, 31, 33, 64, 96, 97, 129, 255, 256, 300, 1023, 1024, 1025, 2049, N} & set(range(1, N + 1)) | {N})
     if N > 10000:
-        sizes = [1, 19, 16383, 16384, N]                 # around the switch to CTA tiles; N = 128 * 128 + 116 is ragged
+        sizes = [1, 19, 5000, 16383, N]                  # warp units (5000: 39 full tiles + 8) and ragged CTA tiles (N = 128 * 128 + 116)
     for n_act in sizes:
         idx = None if n_act == N else rng.choice(N, n_act, replace=False).astype(np.int32)
         got = g.nb_force(idx)
         ref = oracle_on_gpu_records(oracle, g, eps, idx)
         assert_force_parity(got, ref)
         plan = B.nb_plan_force(N, n_act, 148)
-        assert plan.kernel == (0 if n_act >= 16384 else 1)                      # CTA tiles / warp units
+        assert plan.kernel == (0 if n_act >= 256 and n_act * 100 >= 93 * 128 * ((n_act + 127) // 128) else 1)   # CTA tiles / warp units
     # permuted full list: row k <-> idx[k]
     perm = rng.permutation(N).astype(np.int32)
     got = g.nb_force(perm)
@@ -233,7 +233,7 @@ def test_state_io_and_errors(B):
     # workspace too small / bad arguments
     import torch
     ws = torch.empty(4096, dtype=torch.uint8, device="cuda:0")
-    cfg = B.nb_config(0, None, C.c_void_p(ws.data_ptr()), 4096, 0, 0, 0, 0, 0, 0, 0)
+    cfg = B.nb_config(0, None, C.c_void_p(ws.data_ptr()), 4096, 0, 0, 0, 0, 0, 0, 0, 0)
     ctx = C.c_void_p()
     mm = np.ascontiguousarray(m)
     args = (B._ptr(mm), B._ptr(np.ascontiguousarray(x)), B._ptr(np.ascontiguousarray(v)))
@@ -750,3 +750,67 @@ def test_tiny_softening_is_treated_as_zero(B, oracle):
         got = g1.nb_force(idx)
         assert_force_parity(got, oracle_on_gpu_records(oracle, g1, 0.0, idx))
     g0.nb_free(); g1.nb_free()
+
+
+# ------------------------------------------------------------------ f4: mixed precision, f1: the step log
+def test_mixed_precision_accuracy_against_oracle(B, oracle, capsys):
+    """nb_config.precision = NB_PREC_MIXED: fp64 position differences and accumulation, fp32 elsewhere (the precision scheme of
+    the paper's template), for evaluations that run as CTA tiles.  Its per-particle error against the long-double
+    oracle is MEASURED here and bounded; smaller active sets must still be fp64-exact."""
+    N, eps = 20000, 1e-4
+    m, x, v = W.plummer(N, 4242)
+    g = B.System(m, x, v, eps, precision=B.NB_PREC_MIXED)
+    g64 = B.System(m, x, v, eps)
+    t = 2.0 ** -8
+    for s_ in (g, g64):
+        s_.nb_predict(t)
+    assert B.nb_plan_force(N, N).kernel == 0
+    got = g.nb_force()
+    ref = oracle_on_gpu_records(oracle, g64, eps, None)
+    errs = [relvec(a, b) for a, b in zip(got[:3], ref[:3])] + [np.abs(got[3] / ref[3] - 1)]
+    with capsys.disabled():
+        print("\n[mixed precision] N = %d all active, error vs oracle: " % N +
+              ", ".join(f"{n} max {e.max():.2e} median {np.median(e):.2e}" for n, e in zip(("acc", "jerk", "snap", "pot"), errs)))
+    assert errs[0].max() > 1e-9                                                  # this really is the fp32 pair arithmetic
+    for e, bound in zip(errs, (2e-5, 1e-4, 1e-3, 2e-6)):
+        assert e.max() <= bound, (e.max(), bound)
+    assert np.median(errs[0]) <= 2e-6 and np.median(errs[1]) <= 5e-6 and np.median(errs[2]) <= 2e-5
+    # Newton's third law holds to fp32 round-off of the pair terms
+    for arr in got[:3]:
+        assert np.abs((m[:, None] * arr).sum(0)).max() <= 1e-5 * (m[:, None] * np.abs(arr)).sum()
+    # a small active set runs as warp units: fp64 as ever
+    idx = W.active_set(N, 100, 3)
+    assert_force_parity(g.nb_force(idx), oracle_on_gpu_records(oracle, g, eps, idx))
+    # a few shared steps: energy conserved to single-precision-force level, run_blocks works in this mode too
+    K0, W0 = g.nb_energy()
+    for k in range(1, 5):
+        g.nb_predict(k * 2.0 ** -10); g.nb_force(outputs=False); g.nb_corrector(None, 2.0 ** -10)
+    K1, W1 = g.nb_energy()
+    E0_64 = sum(g64.nb_energy())
+    for k in range(1, 5):
+        g64.nb_predict(k * 2.0 ** -10); g64.nb_force(outputs=False); g64.nb_corrector(None, 2.0 ** -10)
+    d_mixed, d_64 = (K1 + W1) / (K0 + W0) - 1, sum(g64.nb_energy()) / E0_64 - 1
+    with capsys.disabled():
+        print(f"[mixed precision] dE/E over 4 shared steps: mixed {d_mixed:.3e}, fp64 {d_64:.3e}")
+    assert abs(d_mixed) < 1e-4 and abs(d_mixed - d_64) < 2e-5
+    steps, _, _ = g.nb_run_blocks(1e30, 5)
+    assert steps == 5 and np.isfinite(g.nb_get_state("X")).all()
+    g.nb_free(); g64.nb_free()
+    with pytest.raises(B.NBError):
+        B.System(m, x, v, eps, precision=B.NB_PREC_MIXED, order=4)
+    with pytest.raises(B.NBError):
+        B.System(m, x, v, eps, precision=7)
+
+
+def test_step_log_records_every_block_step(B):
+    N = 3000
+    m, x, v = W.plummer(N, 515, "kroupa")
+    g = B.System(m, x, v, 1e-4)
+    s1, _, a1 = g.nb_run_blocks(1e30, 40)
+    na, tu = g.nb_step_log()
+    assert s1 == 40 and na.size == 40 and na.sum() == a1 and tu[0] == 0.0 and np.all(np.diff(tu) > 0)
+    s2, _, a2 = g.nb_run_blocks(1e30, 25)
+    na2, tu2 = g.nb_step_log(30)
+    assert na2.size == 30 and na2[5:].sum() == a2 and np.array_equal(na2[:5], na[-5:])   # the last 30 of 65, oldest first
+    assert np.all((na2 >= 1) & (na2 <= N))
+    g.nb_free()
