@@ -245,6 +245,7 @@ int force_internal(nb_ctx* ctx, const int32_t* didx, int64_t n_act)
     A.n_tiles = (int)(ctx->Npad / plan.tile);
     A.n_items = plan.n_units * plan.n_split;
     A.ld = plan.kernel == 0 ? plan.n_units * plan.unit : (int)n_act;
+    A.slice_minor = nb_slice_minor(nb_reduce_threads(n_act, plan.n_split));
 
     int launches = 0;
     CU(cudaEventRecord(ctx->ev0, ctx->stream), "event record");

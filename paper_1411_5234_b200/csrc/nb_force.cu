@@ -391,18 +391,19 @@ __device__ __forceinline__ IPart load_ipart(const ForceArgs& A, int i)
     return ipart_of(load_rec<ORDER>(A.rec + (size_t)i * Q));
 }
 
-// partial planes are [slice][NC][ld] with NC = 10 (a, jerk, snap, pot), 13 at the 8th order (+ crackle)
+// partial sums: NC = 10 components (a, jerk, snap, pot), 13 at the 8th order (+ crackle), per slice and row
 template <int ORDER>
 __device__ __forceinline__ void store_sums(const ForceArgs& A, int slice, int k, const Sums& S)
 {
     constexpr int NC = ORDER == 8 ? 13 : 10;
     if (A.n_split > 1) {
-        double* P = A.partial + (size_t)slice * NC * A.ld + k;      // plane (slice, c) is contiguous in k
-        const size_t ld = A.ld;
-        P[0] = S.ax; P[ld] = S.ay; P[2 * ld] = S.az;
-        P[3 * ld] = S.jx; P[4 * ld] = S.jy; P[5 * ld] = S.jz;
-        P[6 * ld] = S.sx; P[7 * ld] = S.sy; P[8 * ld] = S.sz; P[9 * ld] = S.p;
-        if (ORDER == 8) { P[10 * ld] = S.cx; P[11 * ld] = S.cy; P[12 * ld] = S.cz; }
+        const PartialLayout L(NC, A.ld, A.n_split, A.slice_minor != 0);     // nb_reduce.h: [s][c][k] or [c][k][s]
+        double* P = A.partial + (size_t)slice * L.stride_s + (size_t)k * L.stride_k;
+        const size_t sc = L.stride_c;
+        P[0] = S.ax; P[sc] = S.ay; P[2 * sc] = S.az;
+        P[3 * sc] = S.jx; P[4 * sc] = S.jy; P[5 * sc] = S.jz;
+        P[6 * sc] = S.sx; P[7 * sc] = S.sy; P[8 * sc] = S.sz; P[9 * sc] = S.p;
+        if (ORDER == 8) { P[10 * sc] = S.cx; P[11 * sc] = S.cy; P[12 * sc] = S.cz; }
     } else {
         A.out_a[3 * k] = S.ax; A.out_a[3 * k + 1] = S.ay; A.out_a[3 * k + 2] = S.az;
         A.out_j[3 * k] = S.jx; A.out_j[3 * k + 1] = S.jy; A.out_j[3 * k + 2] = S.jz;
@@ -460,7 +461,7 @@ __device__ __forceinline__ bool take_devplan(ForceArgs& A)
     const DevPlan* d = A.dp;
     if (d->stop) return false;
     A.n_act = d->n_act; A.n_units = d->n_units; A.n_split = d->n_split; A.slice_tiles = d->slice_tiles;
-    A.n_items = d->n_items; A.ld = d->ld; A.predict = d->predict; A.t_pred = d->t_next;
+    A.n_items = d->n_items; A.ld = d->ld; A.predict = d->predict; A.t_pred = d->t_next; A.slice_minor = nb_slice_minor(d->red_T);
     return true;
 }
 

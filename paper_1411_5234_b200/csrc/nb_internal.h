@@ -41,6 +41,8 @@ constexpr int WU_CTAS_PER_SM = 4;
 constexpr int WU_TJ = 64;                    // j-records per stage of a warp's ring
 constexpr int WU_STAGES = 2;
 constexpr int RED_THREADS = 256;             // threads per block of the partial-sum reduction
+// partial sums are laid out [c][k][s] when a whole reduction block works on one particle (T = RED_THREADS), else [s][c][k]
+__host__ __device__ constexpr bool nb_slice_minor(int T) { return T == RED_THREADS; }
 constexpr int NB_STEP_LOG = 8192;            // block steps the device-side step log of nb_run_blocks remembers
 
 struct DevPlan;   // nb_plan.h
@@ -57,11 +59,12 @@ struct ForceArgs {
     int n_tiles;             // total j-tiles (Npad / tile)
     int n_items;             // n_units * n_split
     int ld;                  // rows of a partial plane
+    int slice_minor;         // layout of the partial sums (nb_reduce.h: PartialLayout, nb_slice_minor)
     int predict;             // 1: the kernel predicts every j-record it reads from the state, to time t_pred (device-planned
                              //    block steps with few units: saves the predictor's pass over all N)
     double t_pred;
     double eps2;
-    double* partial;         // [S][NC][ld] when S > 1; NC = 10 components (a, jerk, snap, pot), 13 at the 8th order
+    double* partial;         // S x NC x ld partial sums when S > 1; NC = 10 components (a, jerk, snap, pot), 13 at the 8th order
     const DevPlan* dp;       // non-null: the launch was planned on the device (nb_run_blocks); overrides the plan fields above
     int* queue;              // work queue: [0] next item, [1] finished workers (both 0 between launches)
     double* out_a; double* out_j; double* out_s; double* out_p;   // [n_act][3] x3, [n_act]

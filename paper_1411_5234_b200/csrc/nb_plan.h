@@ -115,7 +115,8 @@ NB_HD PlanShape nb_plan_shape(int64_t Npad, int64_t n_act, int n_sm, int64_t max
 // or warps); an item of a unit of weight w costs w * slice_tiles + fixed.
 // CTA tiles (kernel 0): co-resident CTAs do not get equal shares of the FP64 pipe, so a single round of equal items
 // ends with the slow CTA of every SM running alone (measured 0.78 of the issue bound against 0.86 with ten rounds):
-// one round counts 1.5, more rounds items / resident + 0.9 for the tail.
+// up to eight rounds the rounds are counted whole plus half a round (745 slices x 4 tiles = 5.03 rounds measured 0.814,
+// 592 x 4 = 4.00 rounds 0.833), more rounds items / resident + 0.9 for the tail.
 // Warp units (kernel 1): up to one round the largest item decides; up to four rounds the last round is counted whole;
 // beyond that the queue balances the workers up to a tail of about 0.7 of the largest item.
 NB_HD double nb_split_cost(const PlanShape& p, int64_t S, int64_t* slice_tiles)
@@ -125,7 +126,8 @@ NB_HD double nb_split_cost(const PlanShape& p, int64_t S, int64_t* slice_tiles)
     if ((p.n_tiles + st - 1) / st != S) return -1.0;
     const int64_t items = p.n_units * S;
     if (p.kernel == 0) {
-        const double rounds = items <= p.resident ? 1.5 : (double)items / (double)p.resident + 0.9;
+        const double rounds = items <= 8 * p.resident ? (double)((items + p.resident - 1) / p.resident) + 0.5
+                                                      : (double)items / (double)p.resident + 0.9;
         return rounds * ((double)st + p.fixed);
     }
     const double c_max = p.w_max * (double)st + p.fixed;
