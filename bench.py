@@ -31,12 +31,14 @@ from paper_1411_5234_b200 import workloads as W  # noqa: E402
 
 METRIC = "fp64 pairwise interactions/s (acc+jerk+snap) at N=2^20"
 UNIT = "interactions/s"
-FLOP_EXEC = 86   # algorithmic flop per interaction: 2*32 FMA + 11 MUL + 11 ADD.  The shipped SASS executes 85 of them
-                 # on the FP64 pipe (32 DFMA + 11 DMUL + 10 DADD) and one (2 c1) as an exponent increment on the integer pipe
+FLOP_EXEC = 86   # ALGORITHMIC flop per interaction: 2*32 FMA + 11 MUL + 11 ADD; this is what roofline.achieved counts
+FLOP_PIPE = 85   # of which the shipped SASS executes 85 on the FP64 pipe (32 DFMA + 11 DMUL + 10 DADD, profiles/r02_sass_tables.md);
+                 # the 86th (2 c1) is an exponent increment on the integer pipe.  roofline.frac_pipe_executed uses this count
 FLOP_CONV = 97   # customary acc+jerk+snap operation count of the Hermite-6 literature (a labelled convention)
 FP64_LANES_PER_SM = 64
 DT_BENCH = 2.0 ** -14
-TRAFFIC_NCU_BYTES = 652.8e6 + 646.1e6   # per force launch at N = 2^20, from the committed ncu capture (profiles/)
+# dram__bytes_read.sum + dram__bytes_write.sum per force launch, by N, from the committed ncu --set full captures (profiles/)
+TRAFFIC = {}
 
 
 def n_cores() -> int:
@@ -263,15 +265,30 @@ def run_ours(args, cfg_dict):
     pipe_probe = P.dfma_sources(sm_max_mhz, local)            # cycles per DFMA: 2 / 3 / 3-with-reuse register sources
     f_ms = float(np.mean(force_ms))
     achieved = FLOP_EXEC * inter_per_step / (f_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "force_li_kernel<false, 1, 6> (+ reduce_partials_kernel<10>)", "achieved": achieved,
+    roofline = {"bound": "alu", "kernel": "force_li_kernel<false, 6> (+ reduce_partials_kernel<10>)", "achieved": achieved,
                 "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
+                "frac_pipe_executed": FLOP_PIPE * inter_per_step / (f_ms * 1e-3) / 1e12 / peak_nominal,
                 "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max_mhz:.0f} MHz (DESIGN.md)",
                 "peak_measured_dfma": peak_measured, "frac_of_measured_dfma": achieved / peak_measured,
                 "flop_per_interaction": FLOP_EXEC, "pipe_probe": pipe_probe, "tflops_conv97": FLOP_CONV * inter_per_step / (f_ms * 1e-3) / 1e12,
                 "kernel_ms": f_ms, "kernel_share_of_step": f_ms * args.steps / ms,
                 "interactions_per_s_kernel": inter_per_step / (f_ms * 1e-3),
-                "traffic": TRAFFIC_NCU_BYTES if N == W.CONFIGS[4].N else None,
-                "traffic_source": "profiles/r01_force_li_full.md (dram__bytes_read.sum + dram__bytes_write.sum, one ncu --set full capture)"}
+                "traffic": TRAFFIC.get(N),
+                "traffic_source": "profiles/r02_force_li_full.md (dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture "
+                                  "of this kernel at this N; null at sizes that were not captured)"}
+
+    # ---- the paper's own precision scheme, measured beside the fp64 path on the same workload: one evaluation
+    gm = B.System(torch.tensor(m, device=dev), torch.tensor(x, device=dev), torch.tensor(v, device=dev), c.eps, host=False, device=local,
+                  precision=B.NB_PREC_MIXED)
+    gm.nb_predict(DT_BENCH)
+    mixed_ms = []
+    for _ in range(2):
+        gm.nb_force(None, outputs=False)
+        mixed_ms.append(gm.nb_last_force_ms())
+    gm.nb_free()
+    mixed = {"what": "nb_config.precision = NB_PREC_MIXED (fp64 position differences and accumulation, fp32 pair arithmetic); NOT the headline: "
+                     "about 1e-6 per particle against the oracle (tests/test_gpu_parity.py::test_mixed_precision_accuracy_against_oracle)",
+             "interactions_per_s_kernel": inter_per_step / (min(mixed_ms) * 1e-3), "kernel_ms": min(mixed_ms), "speedup_over_fp64": f_ms / min(mixed_ms)}
 
     # ---- the oracle timed beside it (rank 0, bounded sample)
     cpu_val, sample = time_oracle_sample(m, x, v, np.zeros_like(x), c.eps, args.cpu_seconds, 31)
@@ -282,7 +299,7 @@ def run_ours(args, cfg_dict):
             "dtype": "f64", "data": "synthetic", "config": cfg_dict, "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps},
-            "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}
+            "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "mixed_precision": mixed}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -301,8 +318,9 @@ def main():
     cfg_dict = {"workload": f"BASELINE.json configs[3]: N={N} equal-mass Plummer sphere (seeded, Henon units), eps=1e-4, fp64, "
                             "all N active; step = nb_predict + nb_force(all) + nb_corrector(all)",
                 "N": N, "n_act": N, "eps": 1e-4, "dt": DT_BENCH,
-                "parallelism": "single GPU" if args.gpus == 1 else f"{args.gpus} independent replicas",
-                "l2": "per-step working set (state 168 MB + j-records 84 MB + partial sums 671 MB + results 84 MB) exceeds the 126 MB L2"}
+                "parallelism": "single GPU" if args.gpus == 1 else f"{args.gpus} independent replicas, one system per GPU, no collective "
+                                                                    "(the path is not sharded in this build: DESIGN.md 9)",
+                "l2": "per-step working set (state 176 MB + j-records 84 MB + partial sums 671 MB + results 84 MB) exceeds the 126 MB L2"}
     if args.impl == "reference":
         run_reference(args, cfg_dict)
     else:

@@ -116,7 +116,7 @@ class System:
     """
 
     def __init__(self, m, x, v, eps, host=True, device=0, eta=0.0, eta_s=0.0, k_min=0, k_max=0, stream=None, order=0,
-                 check_indices=0, precision=0):
+                 check_indices=0, precision=0, guard_bytes=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1411_5234_b200 needs a CUDA device; there is no CPU fallback")
@@ -129,8 +129,12 @@ class System:
         torch.cuda.set_device(device)
         self.stream = stream if stream is not None else torch.cuda.current_stream(device)
         nbytes = self.L.nb_workspace_bytes(self.N)
-        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=f"cuda:{device}")
-        base = (self.workspace.data_ptr() + 255) // 256 * 256
+        # guard_bytes > 0: bands of 0xA5 before and after the workspace that nothing may touch (guards_intact(); compute-sanitizer
+        # is not available on every pool, this is the memory-safety check that always is)
+        self._guard = (int(guard_bytes) + 255) // 256 * 256
+        self.workspace = torch.full((nbytes + 256 + 2 * self._guard,), 0xA5, dtype=torch.uint8, device=f"cuda:{device}")
+        base = (self.workspace.data_ptr() + self._guard + 255) // 256 * 256
+        self._ws_off, self._ws_bytes = base - self.workspace.data_ptr(), nbytes
         self.cfg = nb_config(device, C.c_void_p(self.stream.cuda_stream), C.c_void_p(base), nbytes,
                              0 if host else 1, eta, eta_s, k_min, k_max, order, check_indices, precision)
         m, x, v = self._in(m, (self.N,)), self._in(x, (self.N, 3)), self._in(v, (self.N, 3))
@@ -255,6 +259,12 @@ class System:
 
     def nb_resident_ctas(self, kernel):
         return self.L.nb_resident_ctas(self.ctx, int(kernel))
+
+    def guards_intact(self):
+        """True if no byte outside [workspace, workspace + nb_workspace_bytes) of the allocation was written."""
+        self._torch.cuda.synchronize()
+        lo, hi = self.workspace[:self._ws_off], self.workspace[self._ws_off + self._ws_bytes:]
+        return bool((lo == 0xA5).all().item()) and bool((hi == 0xA5).all().item())
 
     def nb_launch_count(self):
         return self.L.nb_launch_count(self.ctx)

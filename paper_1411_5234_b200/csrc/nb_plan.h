@@ -34,15 +34,15 @@ constexpr int PIF_MAX_UNITS = 2;
 // ---------------------------------------------------------------------------------------------------------------
 // Warp units (kernel 1).  n_act = 32 n_full + rem.  The first n_full units hold 32 particles each.  The remainder is
 // decomposed from its highest bit down into units of p = 16, 8, ... 1 particles, every one full, EXCEPT that a rest
-// which nearly fills the next power of two (at most a quarter of it missing) becomes one padded unit: 31 -> one unit
-// of 32 with 31 valid lanes rather than 16 + 8 + 4 + 2 + 1 (five units, each streaming all j-records).
+// which nearly fills the next power of two (at most an eighth of it, or one particle, missing) becomes one padded unit:
+// 31 -> one unit of 32 with 31 valid lanes rather than 16 + 8 + 4 + 2 + 1 (five units, each streaming all j-records).
 // unit u -> first row k0, width p (lanes are split p ways over particles, 32/p ways over the records of a step) and
 // the number of valid particles.
 // ---------------------------------------------------------------------------------------------------------------
 NB_HD void nb_wu_rest_step(int rem, int* p, int* valid)
 {
     const int pc = nb_pow2ceil(rem);
-    if (pc - rem <= pc / 4) { *p = pc; *valid = rem; }
+    if (pc - rem <= (pc >= 16 ? pc / 8 : 1)) { *p = pc; *valid = rem; }
     else { *p = nb_pow2floor(rem); *valid = *p; }
 }
 
@@ -118,7 +118,11 @@ NB_HD PlanShape nb_plan_shape(int64_t Npad, int64_t n_act, int n_sm, int64_t max
 // up to eight rounds the rounds are counted whole plus half a round (745 slices x 4 tiles = 5.03 rounds measured 0.814,
 // 592 x 4 = 4.00 rounds 0.833), more rounds items / resident + 0.9 for the tail.
 // Warp units (kernel 1): up to one round the largest item decides; up to four rounds the last round is counted whole;
-// beyond that the queue balances the workers up to a tail of about 0.7 of the largest item.
+// beyond that the queue balances the workers up to a tail of about 0.7 of the largest item.  (For nb_force alone half a
+// round of twice as long slices measured up to 15 % faster at N = 2^18 - 8 particles: 24.2 against 28.8 us - but the same
+// plan serves the device-planned block steps, where the force kernel predicts its j-records and more, shorter slices win:
+// 41.5 against 48.2 us per step for 5-16 active particles.  One plan for both keeps nb_run_blocks bitwise equal to the
+// separate calls, and the block step is the case the j-split exists for.)
 NB_HD double nb_split_cost(const PlanShape& p, int64_t S, int64_t* slice_tiles)
 {
     const int64_t st = (p.n_tiles + S - 1) / S;
@@ -167,7 +171,7 @@ NB_HD int64_t nb_split_candidate(const PlanShape& p, int c)
     else if (group == 6) {
         const double tail = p.kernel == 0 ? 0.9 : 0.7 * p.w_max;
         target = nb_isqrt_floor(tail * (double)p.n_tiles * (double)p.resident / ((double)p.n_units * p.fixed));
-    } else target = p.n_units <= p.resident ? p.resident / p.n_units * 2 / 3 : 0;    // group 7: a round two thirds full
+    } else target = 2 * p.n_units <= p.resident ? p.resident / (2 * p.n_units) : 0;  // group 7: half a round
     if (target < 1) return 0;
     target = nb_min64(target, p.s_max);
     int64_t st = (p.n_tiles + target - 1) / target + (var == 1 ? 1 : var == 2 ? -1 : 0);

@@ -814,3 +814,26 @@ def test_step_log_records_every_block_step(B):
     assert na2.size == 30 and na2[5:].sum() == a2 and np.array_equal(na2[:5], na[-5:])   # the last 30 of 65, oldest first
     assert np.all((na2 >= 1) & (na2 <= N))
     g.nb_free()
+
+
+def test_workspace_guard_bands_stay_untouched(B):
+    """Memory safety without compute-sanitizer (closed on this pool, profiles/r02_sanitizer.md): 1 MiB bands of 0xA5 on both
+    sides of the workspace must survive every kernel of the library - all force shapes at ragged sizes, block steps through
+    the graph and by separate calls, the index check, state I/O, the other orders and the mixed-precision records."""
+    N = 4099                                                 # ragged: pads to 4352
+    m, x, v = W.plummer(N, 616, "kroupa")
+    for kw in (dict(), dict(order=4), dict(order=8), dict(precision=B.NB_PREC_MIXED)):
+        g = B.System(m, x, v, 1e-4, guard_bytes=1 << 20, **kw)
+        assert g.guards_intact()
+        g.nb_run_blocks(1e30, 20)
+        for _ in range(4):
+            tn, n, act = g.nb_next_block()
+            g.nb_predict(tn); g.nb_force(act, outputs=False); g.nb_corrector(act, 0.0)
+        g.nb_predict(tn)
+        for n_act in (1, 5, 17, 31, 100, 300, 1024, 4000, N):
+            g.nb_force(None if n_act == N else W.active_set(N, n_act, n_act))
+        assert g.nb_check_indices(np.array([N - 1, 0, N - 1], dtype=np.int32)) == B.NB_EINVAL
+        g.nb_set_state("X", x[-3:], np.array([N - 1, N - 2, N - 3], dtype=np.int32))
+        g.nb_get_state("S"); g.nb_energy(); g.nb_step_log()
+        assert g.guards_intact(), kw
+        g.nb_free()
