@@ -38,7 +38,7 @@ FLOP_CONV = 97   # customary acc+jerk+snap operation count of the Hermite-6 lite
 FP64_LANES_PER_SM = 64
 DT_BENCH = 2.0 ** -14
 # dram__bytes_read.sum + dram__bytes_write.sum per force launch, by N, from the committed ncu --set full captures (profiles/)
-TRAFFIC = {}
+TRAFFIC = {1048576: 656.7e6 + 647.6e6, 262144: 41.2e6 + 160.5e6}
 
 
 def n_cores() -> int:

@@ -132,7 +132,9 @@ class System:
         # guard_bytes > 0: bands of 0xA5 before and after the workspace that nothing may touch (guards_intact(); compute-sanitizer
         # is not available on every pool, this is the memory-safety check that always is)
         self._guard = (int(guard_bytes) + 255) // 256 * 256
-        self.workspace = torch.full((nbytes + 256 + 2 * self._guard,), 0xA5, dtype=torch.uint8, device=f"cuda:{device}")
+        self.workspace = torch.empty(nbytes + 256 + 2 * self._guard, dtype=torch.uint8, device=f"cuda:{device}")
+        if self._guard:
+            self.workspace.fill_(0xA5)
         base = (self.workspace.data_ptr() + self._guard + 255) // 256 * 256
         self._ws_off, self._ws_bytes = base - self.workspace.data_ptr(), nbytes
         self.cfg = nb_config(device, C.c_void_p(self.stream.cuda_stream), C.c_void_p(base), nbytes,

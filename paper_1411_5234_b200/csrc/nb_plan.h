@@ -91,7 +91,7 @@ NB_HD PlanShape nb_plan_shape(int64_t Npad, int64_t n_act, int n_sm, int64_t max
     const int64_t rows = nb_partial_rows(Npad);
     if (nb_use_cta_tiles(n_act)) {
         // CTA tiles: a work item is (i-tile of 128 particles, j-slice); resident = CTAs on the device
-        p.kernel = 0; p.unit = LI_UNIT; p.tile = LI_TJ; p.ctas_per_sm = LI_CTAS_PER_SM; p.fixed = 2.0;
+        p.kernel = 0; p.unit = LI_UNIT; p.tile = LI_TJ; p.ctas_per_sm = LI_CTAS_PER_SM; p.fixed = 4.0;
         p.n_units = (n_act + LI_UNIT - 1) / LI_UNIT;
         p.work = (double)p.n_units; p.w_max = 1.0;
         p.n_tiles = Npad / LI_TJ;
@@ -137,10 +137,7 @@ NB_HD double nb_split_cost(const PlanShape& p, int64_t S, int64_t* slice_tiles)
     const double c_max = p.w_max * (double)st + p.fixed;
     const double c_avg = p.work / (double)p.n_units * (double)st + p.fixed;
     if (items <= p.resident) return c_max;
-    if (items <= 4 * p.resident) {
-        const double c = (double)((items + p.resident - 1) / p.resident) * c_avg;
-        return c > c_max ? c : c_max;
-    }
+    if (items <= 4 * p.resident) return (double)((items + p.resident - 1) / p.resident) * c_max;   // a round lasts as long as its heaviest item
     return (double)items * c_avg / (double)p.resident + 0.7 * c_max;
 }
 
