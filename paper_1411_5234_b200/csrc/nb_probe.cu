@@ -84,6 +84,13 @@ __global__ void __launch_bounds__(256) mixed_rate_kernel(double* out, int iters,
         fa[k] = threadIdx.x + k; fb[k] = seed * (k + 1) + threadIdx.x * 1e-6f; fd[k] = seed * 0.1f * (k + 2) + threadIdx.x * 1e-6f;
         lo[k] = 0.f; da[k] = threadIdx.x + 0.5 * k; db[k] = (double)seed * (k + 3) + threadIdx.x * 1e-9;
     }
+    unsigned long long pa[8], pb[8], pd[8];                  // packed pairs of floats for the f32x2 streams
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        pa[k] = ((unsigned long long)__float_as_uint(fa[k]) << 32) | __float_as_uint(fa[k] + 0.5f);
+        pb[k] = ((unsigned long long)__float_as_uint(fb[k]) << 32) | __float_as_uint(fb[k] * 1.5f);
+        pd[k] = ((unsigned long long)__float_as_uint(fd[k]) << 32) | __float_as_uint(fd[k] * 0.5f);
+    }
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
@@ -103,12 +110,14 @@ __global__ void __launch_bounds__(256) mixed_rate_kernel(double* out, int iters,
                 if (KIND == 5) { P_DFMA(da[k], da[k], 0.999999, 1e-7); P_FFMA(fa[k], fb[k], fd[k], fa[k]); }   // both pipes, 1:1
                 if (KIND == 6) P_FFMA(fa[k], fb[0], fd[k], fa[k]);                       // FFMA, one source shared by the run
                 if (KIND == 7) P_FFMA(fa[k], fa[k], 0.999999f, 1e-7f);                   // FFMA, one register and two immediates
+                if (KIND == 8) asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(pa[k]) : "l"(pb[k]), "l"(pd[k]));   // FFMA2: two fp32 FMAs per lane, three register pairs
+                if (KIND == 9) asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(pa[k]) : "l"(pb[0]), "l"(pd[k]));   // FFMA2, one source shared by the run
             }
         }
     }
     double r = 0;
 #pragma unroll
-    for (int k = 0; k < 8; ++k) r += (double)fa[k] + da[k] + (double)lo[k];
+    for (int k = 0; k < 8; ++k) r += (double)fa[k] + da[k] + (double)lo[k] + (double)__uint_as_float((unsigned)pa[k]) + (double)__uint_as_float((unsigned)(pa[k] >> 32));
     if (r == 12345.678) out[blockIdx.x] = r;
 }
 
@@ -195,7 +204,7 @@ int nbp_dfma_sources(int device, void* stream, void* workspace, size_t workspace
 
 int nbp_mixed_rates(int device, void* stream, void* workspace, size_t workspace_bytes, int kind, double sm_mhz, double* cycles)
 {
-    if (!workspace || workspace_bytes < 65536 || !cycles || kind < 0 || kind > 7 || !(sm_mhz > 0)) return -1;
+    if (!workspace || workspace_bytes < 65536 || !cycles || kind < 0 || kind > 9 || !(sm_mhz > 0)) return -1;
     DeviceGuard g(device);
     if (g.err != cudaSuccess) return -4;
     cudaStream_t st = (cudaStream_t)stream;
@@ -214,7 +223,9 @@ int nbp_mixed_rates(int device, void* stream, void* workspace, size_t workspace_
             case 4: mixed_rate_kernel<4><<<n_sm * 3, 256, 0, st>>>(out, iters, seed); break;
             case 5: mixed_rate_kernel<5><<<n_sm * 3, 256, 0, st>>>(out, iters, seed); break;
             case 6: mixed_rate_kernel<6><<<n_sm * 3, 256, 0, st>>>(out, iters, seed); break;
-            default: mixed_rate_kernel<7><<<n_sm * 3, 256, 0, st>>>(out, iters, seed); break;
+            case 7: mixed_rate_kernel<7><<<n_sm * 3, 256, 0, st>>>(out, iters, seed); break;
+            case 8: mixed_rate_kernel<8><<<n_sm * 3, 256, 0, st>>>(out, iters, seed); break;
+            default: mixed_rate_kernel<9><<<n_sm * 3, 256, 0, st>>>(out, iters, seed); break;
         }
     }, &ms);
     if (rc != 0) return rc;

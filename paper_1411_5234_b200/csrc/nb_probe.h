@@ -32,6 +32,8 @@ int nbp_dfma_sources(int device, void* stream, void* workspace, size_t workspace
  *   kind 5  DFMA (2-source) and FFMA interleaved 1:1 - do the FP32 and FP64 pipes issue side by side?
  *   kind 6  FFMA with one source shared by the run (operand-reuse cache)
  *   kind 7  FFMA with one register and two immediates
+ *   kind 8  FFMA2 (fma.rn.f32x2: two fp32 FMAs per lane on register pairs, sm_100), three register-pair sources
+ *   kind 9  FFMA2 with one source shared by the run
  * `cycles` = sub-partition cycles per warp instruction of the named kind (kinds 1-4: per element;
  * kind 5: per DFMA+FFMA pair). */
 int nbp_mixed_rates(int device, void* stream, void* workspace, size_t workspace_bytes, int kind, double sm_mhz, double* cycles);

@@ -12,7 +12,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libnbprobe.so")
 EXPORTS = ["nbp_fp64_peak", "nbp_dfma_sources", "nbp_mixed_rates"]
 MIXED_KINDS = ("ffma_three_sources", "f2f_round_trip_d2f_f2d", "f2f_round_trip_plus_dadd", "f2d_dadd_fadd",
-               "float_float_accumulate", "dfma_plus_ffma_pair", "ffma_one_source_reused", "ffma_immediates")
+               "float_float_accumulate", "dfma_plus_ffma_pair", "ffma_one_source_reused", "ffma_immediates",
+               "ffma2_three_sources", "ffma2_one_source_reused")
 _lib = None
 
 
