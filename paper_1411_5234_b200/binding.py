@@ -13,7 +13,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libnb.so")
+LIB_PATH = os.environ.get("NB_LIB") or os.path.join(_HERE, "libnb.so")   # NB_LIB: another build of the same library (build comparisons)
 
 NB_OK, NB_EINVAL, NB_ENOMEM, NB_ESTATE, NB_ECUDA = 0, -1, -2, -3, -4
 NB_PREC_FP64, NB_PREC_MIXED = 0, 1

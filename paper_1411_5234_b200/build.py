@@ -1,11 +1,17 @@
 """Build libnb.so (the product) and libnbprobe.so (measurement aids) in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_1411_5234_b200.build [--force]
+    python -m paper_1411_5234_b200.build [--force] [-v]
+
+nb_force.cu takes one more step: between ptxas and the host compile its cubin goes through sass_sched.py, which puts the FP64
+pair loops into the order they are written in (see that file).  NB_SASS_SCHED=0 in the environment builds without that step
+(the GPU tests compare the two builds bit for bit).
 """
 from __future__ import annotations
 
 import glob
 import os
+import shlex
+import shutil
 import subprocess
 import sys
 
@@ -42,6 +48,44 @@ def stale() -> bool:
     return False
 
 
+SCHEDULED = ["nb_force.cu"]          # sources whose cubin goes through sass_sched.py
+
+
+def sass_sched_enabled() -> bool:
+    return os.environ.get("NB_SASS_SCHED", "1") != "0"
+
+
+def _compile_scheduled(src: str, obj: str, objdir: str, verbose: bool) -> None:
+    """nvcc -c with the intermediate files kept; then the cubin is rescheduled and the last two steps of nvcc's own recipe
+    (fatbinary, host compile of the .cudafe1.cpp that embeds the fat binary) are run again on it."""
+    from . import sass_sched
+    keep = os.path.join(objdir, "keep_" + os.path.basename(src).replace(".cu", ""))
+    shutil.rmtree(keep, ignore_errors=True)
+    os.makedirs(keep)
+    base = [_nvcc()] + NVCC_FLAGS + ["--keep", "--keep-dir", keep, "-c", src, "-o", obj]
+    out = subprocess.run(base + (["-Xptxas", "-v"] if verbose else []), stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+    if verbose or out.returncode != 0:
+        sys.stderr.write(out.stdout)
+    if out.returncode != 0:
+        raise RuntimeError("nvcc failed: " + " ".join(base))
+    stem = os.path.basename(src).replace(".cu", "")
+    cubin = os.path.join(keep, stem + ".cubin")
+    shutil.copy(cubin, cubin + ".ptxas")                               # what ptxas emitted, for comparison
+    log = open(os.path.join(keep, "sass_sched.log"), "w")
+    sass_sched.run(cubin + ".ptxas", cubin, src, report=True, log=log)
+    log.close()
+    if verbose:
+        sys.stderr.write(open(log.name).read())
+    dry = subprocess.run(base + ["--dryrun"], stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True, check=True).stdout
+    steps = [l[3:] for l in dry.split("\n") if l.startswith("#$ ")]
+    redo = [l for l in steps if l.startswith("fatbinary ")] + [l for l in steps if l.startswith("gcc ") and " -c " in l and ".cudafe1.cpp" in l]
+    if len(redo) != 2:
+        raise RuntimeError("unexpected nvcc recipe: " + dry)
+    env = dict(os.environ, PATH=os.path.dirname(_nvcc()) + os.pathsep + os.environ.get("PATH", ""))
+    for l in redo:
+        subprocess.run(shlex.split(l), check=True, env=env)
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not stale():
         return LIB
@@ -50,9 +94,14 @@ def build(force: bool = False, verbose: bool = False) -> str:
     procs, objs = [], {}
     for s in SOURCES + PROBE_SOURCES:
         o = os.path.join(objdir, s.replace(".cu", ".o"))
+        objs[s] = o
+        if s in SCHEDULED and sass_sched_enabled():
+            continue
         cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, s), "-o", o]
         procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
-        objs[s] = o
+    for s in SCHEDULED:
+        if sass_sched_enabled():
+            _compile_scheduled(os.path.join(CSRC, s), objs[s], objdir, verbose)
     for cmd, p in procs:
         out, _ = p.communicate()
         if verbose or p.returncode != 0:
