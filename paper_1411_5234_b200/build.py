@@ -20,6 +20,8 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnb.so")
 PROBE_LIB = os.path.join(HERE, "libnbprobe.so")          # measurement aids (csrc/nb_probe.h), loaded by bench.py only
+PTXAS_LIB = os.path.join(HERE, "libnb_ptxas.so")         # the same library with nb_force.cu as ptxas scheduled it: only the test
+                                                         # that compares the two builds bit for bit loads it (NB_LIB=...)
 SOURCES = ["nb_api.cu", "nb_force.cu", "nb_step.cu"]
 PROBE_SOURCES = ["nb_probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -68,6 +70,7 @@ def _compile_scheduled(src: str, obj: str, objdir: str, verbose: bool) -> None:
         sys.stderr.write(out.stdout)
     if out.returncode != 0:
         raise RuntimeError("nvcc failed: " + " ".join(base))
+    shutil.copy(obj, obj.replace(".o", ".ptxas.o"))                    # the object as nvcc made it (for libnb_ptxas.so)
     stem = os.path.basename(src).replace(".cu", "")
     cubin = os.path.join(keep, stem + ".cubin")
     shutil.copy(cubin, cubin + ".ptxas")                               # what ptxas emitted, for comparison
@@ -110,6 +113,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
     arch = ["-gencode", "arch=compute_100a,code=sm_100a"]
     subprocess.run([_nvcc(), "-shared", "-o", LIB] + [objs[s] for s in SOURCES] + arch, check=True)
+    if sass_sched_enabled():
+        subprocess.run([_nvcc(), "-shared", "-o", PTXAS_LIB] + [objs[s].replace(".o", ".ptxas.o") if s in SCHEDULED else objs[s]
+                                                                for s in SOURCES] + arch, check=True)
+    elif os.path.exists(PTXAS_LIB):
+        os.remove(PTXAS_LIB)
     subprocess.run([_nvcc(), "-shared", "-o", PROBE_LIB] + [objs[s] for s in PROBE_SOURCES] + arch, check=True)
     return LIB
 

@@ -503,8 +503,13 @@ def build_values(blk, live_out, body):
             for r in range(base, base + w):
                 if r not in cur: new([r], fixed=True)                                # live into the block
                 ids.append(find(cur[r]))
+            # One operand made of several values: halves that were written separately (a MUFU.RSQ64H result over a zeroed low
+            # word).  If one of them has been read before, the later write changed a live value in place (2 c by an add to the
+            # high word of c): then the order of those reads and that write matters, and the whole thing keeps its registers.
+            inplace = len(set(ids)) > 1 and any(vals[x].uses for x in set(ids))
             v = ids[0]
             for x in ids[1:]: v = merge(v, x)
+            if inplace: vals[v].fixed = True
             vals[v].align = max(vals[v].align, w)
             vals[v].uses.append(k)
             if ins.sfields is None: vals[v].fixed = True

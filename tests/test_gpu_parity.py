@@ -837,3 +837,29 @@ def test_workspace_guard_bands_stay_untouched(B):
         g.nb_get_state("S"); g.nb_energy(); g.nb_step_log()
         assert g.guards_intact(), kw
         g.nb_free()
+
+
+# ------------------------------------------------------------------ the rescheduled machine code against ptxas's own
+def test_sass_sched_build_is_bitwise_the_ptxas_build(B, tmp_path):
+    """sass_sched.py permutes and re-registers the instructions of the FP64 pair loops; the arithmetic is untouched, so every
+    result has to be bit-identical to the library built from the cubin as ptxas emitted it (libnb_ptxas.so, build.py)."""
+    import os, subprocess, sys
+    from paper_1411_5234_b200 import build
+    if not build.sass_sched_enabled() or not os.path.exists(build.PTXAS_LIB):
+        pytest.skip("built without sass_sched (NB_SASS_SCHED=0)")
+    log = os.path.join(build.HERE, "build", "keep_nb_force", "sass_sched.log")
+    if os.path.exists(log):
+        assert "sass_sched: 0 blocks rescheduled" not in open(log).read(), "the scheduler changed nothing: nothing to compare"
+    files = {}
+    for name, libpath in (("sched", build.LIB), ("ptxas", build.PTXAS_LIB)):
+        files[name] = str(tmp_path / f"{name}.npz")
+        env = dict(os.environ, NB_LIB=libpath)
+        subprocess.run([sys.executable, "-m", "paper_1411_5234_b200.dump_case", files[name]], check=True, env=env,
+                       cwd=os.path.dirname(build.HERE))
+    a, b = np.load(files["sched"]), np.load(files["ptxas"])
+    assert sorted(a.files) == sorted(b.files) and len(a.files) > 90
+    for k in a.files:
+        x, y = a[k], b[k]
+        assert x.dtype == y.dtype and x.shape == y.shape
+        assert not np.isnan(x).any(), k
+        assert np.array_equal(x.view(np.uint64), y.view(np.uint64)), (k, int((x != y).sum()))
