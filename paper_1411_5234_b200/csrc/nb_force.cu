@@ -87,7 +87,12 @@ __device__ __forceinline__ double twice(double c)
 
 
 // NB_SCHED_BEGIN (sass_sched.py puts the machine code of these lines back into the order written here)
-template <bool EPS0, bool MASK>
+// PINNED: for the instantiations sass_sched.py does not reschedule (warp units and block steps at the 6th order).  There a
+// branch that is never taken (v >= 0) but that ptxas cannot see through stands before each pair's run of 18 DFMAs; the sums are
+// live on its taken side, so ptxas cannot interleave the two runs and chains the sources through the reuse cache itself
+// (21-25 of 48 three-source DFMAs left uncovered instead of 29-33).
+#define PIN(v) if (PINNED && __double2hiint(v) < 0) return;
+template <bool EPS0, bool MASK, bool PINNED = false>
 __device__ __forceinline__ void pair2(const IPart& pi, const JRec (&J)[2], const double eps2, const bool (&self)[2], Sums& S)
 {
     // ONE FP64 instruction per source line, in the order the pipe is to see them (pair 0 and pair 1 of the two records):
@@ -177,6 +182,7 @@ __device__ __forceinline__ void pair2(const IPart& pi, const JRec (&J)[2], const
     VMUL(c31, z1, B1);
     VTWICE(c20, c10);
     VTWICE(c21, c11);
+    PIN(s0)
     // u = dv + c1 dx, w = da + c3 dx + c2 u, sums += q (dx, u, w): 18 three-source DFMAs per pair in one run;
     // each shares a source with its predecessor in the same slot (A: c1, c3, q, c2; B: d_c, u_c)
     if (MASK) mr0 = self[0] ? 0.0 : mr0;              // j != i (eq. 1); a, jerk, snap get exactly 0 from the self pair
@@ -199,6 +205,7 @@ __device__ __forceinline__ void pair2(const IPart& pi, const JRec (&J)[2], const
     VFMA(S.sx, q0, wx0, S.sx);
     VFMA(S.sy, q0, wy0, S.sy);
     VFMA(S.sz, q0, wz0, S.sz);
+    PIN(yy0)
     if (MASK) mr1 = self[1] ? 0.0 : mr1;              // j != i (eq. 1); a, jerk, snap get exactly 0 from the self pair
     VADD(S.p, S.p, mr1);
     VFMA(ux1, c11, dx1, dvx1);
@@ -219,6 +226,7 @@ __device__ __forceinline__ void pair2(const IPart& pi, const JRec (&J)[2], const
     VFMA(S.sx, q1, wx1, S.sx);
     VFMA(S.sy, q1, wy1, S.sy);
     VFMA(S.sz, q1, wz1, S.sz);
+    PIN(yy1)
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -748,7 +756,7 @@ __device__ __forceinline__ void wu_body(const ForceArgs& A, double2* smem, unsig
                     const JRec J[2] = {load_rec<ORDER>(lp + r * Q), load_rec<ORDER>(lp + (r + LJ) * Q)};
                     const bool self[2] = {jl + r == ii, jl + r + LJ == ii};
                     if (ORDER == 4) pair2_o4<EPS0, true>(pi, J, A.eps2, self, acc);
-                    else pair2<EPS0, true>(pi, J, A.eps2, self, acc);
+                    else pair2<EPS0, true, true>(pi, J, A.eps2, self, acc);
                 }
             } else {
 #pragma unroll 1
@@ -756,7 +764,7 @@ __device__ __forceinline__ void wu_body(const ForceArgs& A, double2* smem, unsig
                     const JRec J[2] = {load_rec<ORDER>(lp + r * Q), load_rec<ORDER>(lp + (r + LJ) * Q)};
                     const bool self[2] = {false, false};
                     if (ORDER == 4) pair2_o4<EPS0, false>(pi, J, A.eps2, self, acc);
-                    else pair2<EPS0, false>(pi, J, A.eps2, self, acc);
+                    else pair2<EPS0, false, true>(pi, J, A.eps2, self, acc);
                 }
             }
             __syncwarp();                                      // every lane is done with the stage
