@@ -75,7 +75,12 @@ def _compile_scheduled(src: str, obj: str, objdir: str, verbose: bool) -> None:
     cubin = os.path.join(keep, stem + ".cubin")
     shutil.copy(cubin, cubin + ".ptxas")                               # what ptxas emitted, for comparison
     log = open(os.path.join(keep, "sass_sched.log"), "w")
-    sass_sched.run(cubin + ".ptxas", cubin, src, report=True, log=log)
+    try:
+        sass_sched.run(cubin + ".ptxas", cubin, src, report=True, log=log)
+    except Exception as e:                          # the tool is an optimisation: without it the library is ptxas's code
+        log.write(f"sass_sched: FAILED ({type(e).__name__}: {e}); 0 blocks rescheduled, the cubin is left as ptxas emitted it\n")
+        sys.stderr.write(f"WARNING: sass_sched failed ({type(e).__name__}: {e}); {os.path.basename(src)} keeps ptxas's schedule\n")
+        shutil.copy(cubin + ".ptxas", cubin)
     log.close()
     if verbose:
         sys.stderr.write(open(log.name).read())
