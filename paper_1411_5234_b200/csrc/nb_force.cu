@@ -12,6 +12,9 @@
 //            lanes-over-i (p = 32) to lanes-over-j (p = 1); the 32/p lane sums of a particle are combined with a
 //            warp-shuffle butterfly.  In a device-planned block step with few units the warp PREDICTS the records of
 //            its slice from the state instead of reading them (the predictor's pass over all N is skipped).
+// The FP64 instructions of the pair evaluation are written one per source line between NB_SCHED_BEGIN / NB_SCHED_END, in the order
+// the FP64 pipe is to see them (operand-reuse chains); build.py passes this file's cubin through sass_sched.py, which
+// puts the machine code of the CTA-tile loops back into that order after ptxas (results bit-identical, tests compare).
 // ORDER = 6 is the scheme of the north star (a, jerk, snap, pot); 4 (a, jerk, pot) and 8 (+ crackle) are the other
 // Hermite orders the paper names (R21, R22).
 // Work items (i-unit, j-slice) are handed out by an atomic queue, not by a static stride: warps of

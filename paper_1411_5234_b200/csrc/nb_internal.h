@@ -24,7 +24,8 @@ __host__ __device__ constexpr int nb_rec_q(int order) { return order == 8 ? 7 : 
 // Force kernel shapes (nb.h: nb_plan.kernel).
 // 0  "CTA tiles": a CTA of 128 threads owns 128 active particles (one per thread) and streams j-tiles of 128 records
 //    through shared memory, double-buffered (one bulk copy per tile, mbarrier); all lanes read the same record.
-//    pair2 (nb_force.cu) needs 114 registers: 16 warps (4 per scheduler) per SM as 4 CTAs; CTA shapes that leave the
+//    pair2 (nb_force.cu) needs 106 registers as ptxas orders it, up to 126 in source order (sass_sched.py): 16 warps (4 per
+//    scheduler) per SM as 4 CTAs, 128 registers each at most; CTA shapes that leave the
 //    four schedulers with unequal warp counts (5 x 96, 3 x 160) measured 15-27 % slower.
 // 1  "warp units": every WARP is its own worker with a private double-buffered ring of 64-record tiles.  A unit is
 //    p = 32, 16, ... 1 active particles; the warp's lanes are split p ways over particles and 32/p ways over the records
