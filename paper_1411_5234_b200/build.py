@@ -57,6 +57,11 @@ def sass_sched_enabled() -> bool:
     return os.environ.get("NB_SASS_SCHED", "1") != "0"
 
 
+def _flags():
+    # NB_SASS_SCHED=all (not run on a GPU yet, see sass_sched.EXPERIMENTAL): every pair loop is rescheduled, none keeps the branches
+    return NVCC_FLAGS + (["-DNB_PIN_UNSCHEDULED=false"] if os.environ.get("NB_SASS_SCHED") == "all" else [])
+
+
 def _compile_scheduled(src: str, obj: str, objdir: str, verbose: bool) -> None:
     """nvcc -c with the intermediate files kept; then the cubin is rescheduled and the last two steps of nvcc's own recipe
     (fatbinary, host compile of the .cudafe1.cpp that embeds the fat binary) are run again on it."""
@@ -64,7 +69,7 @@ def _compile_scheduled(src: str, obj: str, objdir: str, verbose: bool) -> None:
     keep = os.path.join(objdir, "keep_" + os.path.basename(src).replace(".cu", ""))
     shutil.rmtree(keep, ignore_errors=True)
     os.makedirs(keep)
-    base = [_nvcc()] + NVCC_FLAGS + ["--keep", "--keep-dir", keep, "-c", src, "-o", obj]
+    base = [_nvcc()] + _flags() + ["--keep", "--keep-dir", keep, "-c", src, "-o", obj]
     out = subprocess.run(base + (["-Xptxas", "-v"] if verbose else []), stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     if verbose or out.returncode != 0:
         sys.stderr.write(out.stdout)

@@ -95,6 +95,9 @@ __device__ __forceinline__ double twice(double c)
 // live on its taken side, so ptxas cannot interleave the two runs and chains the sources through the reuse cache itself
 // (21-25 of 48 three-source DFMAs left uncovered instead of 29-33).
 #define PIN(v) if (PINNED && __double2hiint(v) < 0) return;
+#ifndef NB_PIN_UNSCHEDULED
+#define NB_PIN_UNSCHEDULED true        // build.py: false with NB_SASS_SCHED=all (then sass_sched.py reschedules those loops too)
+#endif
 template <bool EPS0, bool MASK, bool PINNED = false>
 __device__ __forceinline__ void pair2(const IPart& pi, const JRec (&J)[2], const double eps2, const bool (&self)[2], Sums& S)
 {
@@ -759,7 +762,7 @@ __device__ __forceinline__ void wu_body(const ForceArgs& A, double2* smem, unsig
                     const JRec J[2] = {load_rec<ORDER>(lp + r * Q), load_rec<ORDER>(lp + (r + LJ) * Q)};
                     const bool self[2] = {jl + r == ii, jl + r + LJ == ii};
                     if (ORDER == 4) pair2_o4<EPS0, true>(pi, J, A.eps2, self, acc);
-                    else pair2<EPS0, true, true>(pi, J, A.eps2, self, acc);
+                    else pair2<EPS0, true, NB_PIN_UNSCHEDULED>(pi, J, A.eps2, self, acc);
                 }
             } else {
 #pragma unroll 1
@@ -767,7 +770,7 @@ __device__ __forceinline__ void wu_body(const ForceArgs& A, double2* smem, unsig
                     const JRec J[2] = {load_rec<ORDER>(lp + r * Q), load_rec<ORDER>(lp + (r + LJ) * Q)};
                     const bool self[2] = {false, false};
                     if (ORDER == 4) pair2_o4<EPS0, false>(pi, J, A.eps2, self, acc);
-                    else pair2<EPS0, false, true>(pi, J, A.eps2, self, acc);
+                    else pair2<EPS0, false, NB_PIN_UNSCHEDULED>(pi, J, A.eps2, self, acc);
                 }
             }
             __syncwarp();                                      // every lane is done with the stage
@@ -840,6 +843,7 @@ template <bool EPS0, int ORDER>
 __global__ void __launch_bounds__(WU_THREADS, WU_CTAS_PER_SM) force_wu_kernel(const ForceArgs A)
 {
     __shared__ alignas(8) unsigned long long bars[N_BARS];
+    if (!NB_PIN_UNSCHEDULED) reg_ballast<58>(A);           // only where sass_sched.py reschedules this kernel too
     init_barriers(bars);
     wu_body<EPS0, ORDER, false>(A, dyn_smem, bars);
 }
