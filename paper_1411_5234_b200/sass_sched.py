@@ -73,8 +73,9 @@ class Skip(Exception):
 
 
 # the kernels whose rescheduled loops have run on the B200 (GPU tests at 1e-11 against the oracle, bit for bit against ptxas's
-# own code, the bench): force_li_kernel<*, 4 | 6> and force_step_kernel<*, 4>
-VALIDATED_KERNELS = r"force_li_kernelILb[01]ELi[46]E|force_step_kernelILb[01]ELi4E"
+# own code, the bench): force_li_kernel<*, 4 | 6>.  (The CTA-tile loop inside force_step_kernel<*, 4> was rescheduled in that
+# build too, but it is not certain that a test took that path, so it is left out.)
+VALIDATED_KERNELS = r"force_li_kernelILb[01]ELi[46]E"
 
 
 def EXPERIMENTAL():
