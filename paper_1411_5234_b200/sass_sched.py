@@ -73,9 +73,10 @@ class Skip(Exception):
 
 
 # the kernels whose rescheduled loops have run on the B200 (GPU tests at 1e-11 against the oracle, bit for bit against ptxas's
-# own code, the bench): force_li_kernel<*, 4 | 6>.  (The CTA-tile loop inside force_step_kernel<*, 4> was rescheduled in that
-# build too, but it is not certain that a test took that path, so it is left out.)
-VALIDATED_KERNELS = r"force_li_kernelILb[01]ELi[46]E"
+# own code, the bench): force_li_kernel<eps = 0 or > 0, 6> and force_li_kernel<eps > 0, 4>.  (force_li_kernel<eps = 0, 4> and
+# the CTA-tile loop inside force_step_kernel<*, 4> were rescheduled in that build too, but it is not certain that a test took
+# those paths, so they are left out.)
+VALIDATED_KERNELS = r"force_li_kernelILb[01]ELi6E|force_li_kernelILb0ELi4E"
 
 
 def EXPERIMENTAL():
