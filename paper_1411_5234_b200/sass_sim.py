@@ -29,9 +29,22 @@ from . import sass_sched as S
 
 
 def loop_blocks(cubin, kernel_part, n_fp64=106):
+    """the bodies of the loops of a kernel that hold n_fp64 FP64 instructions: everything from the target of a backward branch
+    to that branch, across inner never-taken branches (the pinning branches of pair2<.., PINNED = true>), in program order"""
+    import re
     funcs = S.disassemble(cubin)
     name = [k for k in funcs if kernel_part in k][0]
-    return [b.ins for b in S.basic_blocks(funcs[name]) if sum(1 for i in b.ins if i.klass == "FP64") == n_fp64]
+    ins, labels = [], {}
+    for it in funcs[name]:
+        if isinstance(it, tuple): labels[it[1]] = len(ins)
+        else: ins.append(it)
+    out = []
+    for n, i in enumerate(ins):
+        m = re.search(r"BRA(\.U)?\s.*`\((\.L_x_\d+)\)", i.text)
+        if m and labels.get(m.group(2), n + 1) <= n:
+            body = ins[labels[m.group(2)]: n + 1]
+            if sum(1 for x in body if x.klass == "FP64") == n_fp64: out.append(body)
+    return out
 
 
 def simulate(blk, seeds=(37, 53, 71, 97), **kw):
