@@ -3,7 +3,7 @@ schedule reach when four warps share the scheduler?
 
     python -m paper_1411_5234_b200.sass_sim [CUBIN ...]      # default: the ptxas and the rescheduled cubin of the last build
 
-It is a MODEL, calibrated on the three all-active measurements there are (profiles/r02_sass_sched.md), and it is used for one
+It is a MODEL with guessed latencies, checked against the six all-active measurements there are (profiles/r02_sass_sim.md), used for one
 thing: to say where the modelled single-warp pipe efficiency of sass_table / sass_sched (0.891, 0.991) and the measured
 fractions of the issue bound (0.855, 0.932) part ways.  What it models, per cycle of one scheduler:
 
