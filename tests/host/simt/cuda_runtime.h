@@ -1,0 +1,335 @@
+// tests/host/simt/cuda_runtime.h — TEST INFRASTRUCTURE (tests/test_simt_host_cpu.py): a stand-in for <cuda_runtime.h> with which
+// the WHOLE library (nb_api.cu, nb_force.cu, nb_step.cu and their headers) compiles with g++ and runs on the host, one CUDA thread =
+// one fibre, so that the kernels' structure - work queue, j-split, tile staging, shuffle reductions, partial-sum layouts, the
+// fixed-order reduction, the one-kernel scheduler, the device-planned block step and its graph - can be compared with the oracle
+// through the library's real C ABI where there is no GPU (and where compute-sanitizer is closed: profiles/r02_sanitizer.md).
+//
+// What it is: the SIMT execution model, restated for one OS thread.  A launch runs its CTAs one after the other; inside a CTA
+// every thread is a ucontext fibre that runs until it has to wait (__syncthreads, __syncwarp, a shuffle / vote, an mbarrier);
+// barriers count the threads that have not exited; shuffles and votes exchange through a per-warp slot array between two warp
+// barriers.  Shared memory is `static` storage (CTAs do not overlap).  Global-memory atomics are plain operations.  Streams are
+// in order and synchronous; a stream capture records the launches as closures and a graph launch replays them.
+// What it is not: a product path (nothing under paper_1411_5234_b200/ refers to it; the library refuses to run without a CUDA
+// device), a model of timing, of memory ordering or of races between CTAs, or a check of the machine code.  The GPU parity
+// tests (-m gpu) remain the proof for the B200.
+#pragma once
+#include <ucontext.h>
+
+#include <cmath>
+#include <cstddef>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <ctime>
+#include <functional>
+#include <tuple>
+#include <utility>
+#include <vector>
+
+#define NB_SIMT_HOST 1
+
+// ---------------------------------------------------------------------------------------------------------------
+// qualifiers and vector types
+// ---------------------------------------------------------------------------------------------------------------
+#define __global__
+#define __device__
+#define __host__
+#define __forceinline__ inline
+#define __launch_bounds__(...)
+#define __align__(n) alignas(n)
+#define __shared__ static
+
+struct alignas(16) double2 { double x, y; };
+struct alignas(32) double4 { double x, y, z, w; };
+struct alignas(16) float4 { float x, y, z, w; };
+struct uint3 { unsigned x, y, z; };
+static inline double2 make_double2(double x, double y) { return double2{x, y}; }
+static inline double4 make_double4(double x, double y, double z, double w) { return double4{x, y, z, w}; }
+static inline float4 make_float4(float x, float y, float z, float w) { return float4{x, y, z, w}; }
+
+// ---------------------------------------------------------------------------------------------------------------
+// the engine
+// ---------------------------------------------------------------------------------------------------------------
+namespace simt {
+
+constexpr int MAX_THREADS = 1024;
+constexpr size_t STACK_BYTES = 96 * 1024;
+
+struct Warp {
+    int alive = 0, arrived = 0;
+    unsigned gen = 0;
+    unsigned long long slot[32];
+};
+
+struct Fibre {
+    ucontext_t ctx;
+    uint3 tid{0, 0, 0};
+    int lane = 0, warp = 0;
+    bool done = true;
+};
+
+struct Cta {
+    uint3 bid{0, 0, 0}, bdim{1, 1, 1}, gdim{1, 1, 1};
+    int alive = 0, arrived = 0;
+    unsigned gen = 0;
+    Warp warps[MAX_THREADS / 32];
+};
+
+struct State {
+    Fibre fib[MAX_THREADS];
+    char* stacks = nullptr;
+    ucontext_t main_ctx;
+    Fibre* self = nullptr;
+    Cta cta;
+    std::function<void()> body;               // the kernel call of the launch that is running
+    bool capturing = false;
+    std::vector<std::function<void()>>* capture = nullptr;
+    long long launches = 0, switches = 0, progress = 0;   // progress: arrivals, releases, exits, completed copies
+    unsigned long long clock = 0;
+};
+
+inline State& S() { static State s; return s; }
+
+inline void yield() { State& s = S(); ++s.switches; swapcontext(&s.self->ctx, &s.main_ctx); }
+
+inline void fibre_entry()
+{
+    State& s = S();
+    s.body();
+    Fibre* f = s.self;
+    f->done = true;
+    s.progress += 1;
+    s.cta.alive -= 1;
+    s.cta.warps[f->warp].alive -= 1;
+    swapcontext(&f->ctx, &s.main_ctx);
+}
+
+// barrier over the threads of the CTA that have not exited
+inline void cta_barrier()
+{
+    Cta& c = S().cta;
+    const unsigned g = c.gen;
+    c.arrived += 1; S().progress += 1;
+    while (c.gen == g) {
+        if (c.arrived >= c.alive) { c.arrived = 0; c.gen += 1; break; }
+        yield();
+    }
+}
+
+inline void warp_barrier()
+{
+    State& s = S();
+    Warp& w = s.cta.warps[s.self->warp];
+    const unsigned g = w.gen;
+    w.arrived += 1; s.progress += 1;
+    while (w.gen == g) {
+        if (w.arrived >= w.alive) { w.arrived = 0; w.gen += 1; break; }
+        yield();
+    }
+}
+
+// run one CTA to completion: round-robin over its fibres until all have exited
+inline void run_cta(unsigned block, unsigned bid, unsigned grid)
+{
+    State& s = S();
+    if (!s.stacks) s.stacks = (char*)aligned_alloc(4096, STACK_BYTES * MAX_THREADS);
+    if (block > (unsigned)MAX_THREADS) { fprintf(stderr, "simt: block of %u threads\n", block); abort(); }
+    Cta& c = s.cta;
+    c.bid = uint3{bid, 0, 0}; c.bdim = uint3{block, 1, 1}; c.gdim = uint3{grid, 1, 1};
+    c.alive = (int)block; c.arrived = 0; c.gen = 0;
+    for (unsigned w = 0; w < (block + 31) / 32; ++w) {
+        c.warps[w].alive = (int)(block - 32 * w < 32 ? block - 32 * w : 32);
+        c.warps[w].arrived = 0; c.warps[w].gen = 0;
+    }
+    for (unsigned t = 0; t < block; ++t) {
+        Fibre& f = s.fib[t];
+        f.tid = uint3{t, 0, 0}; f.lane = (int)(t & 31); f.warp = (int)(t >> 5); f.done = false;
+        getcontext(&f.ctx);
+        f.ctx.uc_stack.ss_sp = s.stacks + STACK_BYTES * t;
+        f.ctx.uc_stack.ss_size = STACK_BYTES;
+        f.ctx.uc_link = nullptr;
+        makecontext(&f.ctx, (void (*)())fibre_entry, 0);
+    }
+    while (c.alive > 0) {
+        const long long before = s.progress;
+        for (unsigned t = 0; t < block; ++t) {
+            Fibre& f = s.fib[t];
+            if (f.done) continue;
+            s.self = &f;
+            swapcontext(&s.main_ctx, &f.ctx);
+        }
+        s.self = nullptr;
+        // a fibre yields only while it waits for something another fibre of the CTA has to do: a whole round in which nobody
+        // arrived anywhere, left, or completed a copy will repeat for ever (a barrier some thread never reaches)
+        if (s.progress == before && c.alive > 0) { fprintf(stderr, "simt: deadlock in CTA %u (%d threads waiting)\n", bid, c.alive); abort(); }
+    }
+}
+
+template <class... P, class... A>
+inline void launch(void (*kernel)(P...), long long grid, long long block, size_t /*smem*/, void* /*stream*/, A&&... args)
+{
+    State& s = S();
+    std::tuple<std::decay_t<P>...> held(std::forward<A>(args)...);      // kernel arguments are passed by value
+    auto run = [kernel, grid, block, held]() {
+        State& st = S();
+        st.launches += 1;
+        st.body = [kernel, &held]() { std::apply(kernel, held); };
+        for (long long b = 0; b < grid; ++b) run_cta((unsigned)block, (unsigned)b, (unsigned)grid);
+        st.body = nullptr;
+    };
+    if (s.capturing) s.capture->push_back(run);
+    else run();
+}
+
+inline unsigned long long clock_ns() { return S().clock += 1000; }
+
+}  // namespace simt
+
+#define threadIdx (simt::S().self->tid)
+#define blockIdx (simt::S().cta.bid)
+#define blockDim (simt::S().cta.bdim)
+#define gridDim (simt::S().cta.gdim)
+
+// ---------------------------------------------------------------------------------------------------------------
+// device intrinsics
+// ---------------------------------------------------------------------------------------------------------------
+static inline void __syncthreads() { simt::cta_barrier(); }
+static inline void __syncwarp(unsigned = 0xffffffffu) { simt::warp_barrier(); }
+static inline void __threadfence() {}
+
+namespace simt {
+template <class T>
+inline T warp_exchange(T v, int src)          // src: lane to read from (own value if it lies outside the warp)
+{
+    static_assert(sizeof(T) <= 8, "shuffles move at most 64 bits");
+    State& s = S();
+    Warp& w = s.cta.warps[s.self->warp];
+    unsigned long long bits = 0;
+    memcpy(&bits, &v, sizeof(T));
+    w.slot[s.self->lane] = bits;
+    warp_barrier();
+    const unsigned long long got = (src >= 0 && src < 32) ? w.slot[src] : bits;
+    warp_barrier();                           // nobody overwrites a slot before everybody has read
+    T r;
+    memcpy(&r, &got, sizeof(T));
+    return r;
+}
+}  // namespace simt
+
+template <class T> static inline T __shfl_xor_sync(unsigned, T v, int o) { return simt::warp_exchange(v, simt::S().self->lane ^ o); }
+template <class T> static inline T __shfl_sync(unsigned, T v, int src) { return simt::warp_exchange(v, src & 31); }
+template <class T> static inline T __shfl_up_sync(unsigned, T v, unsigned o)
+{
+    const int lane = simt::S().self->lane;
+    return simt::warp_exchange(v, lane - (int)o >= 0 ? lane - (int)o : -1);
+}
+static inline int __any_sync(unsigned, int pred)
+{
+    simt::State& s = simt::S();
+    simt::Warp& w = s.cta.warps[s.self->warp];
+    w.slot[s.self->lane] = pred ? 1 : 0;
+    simt::warp_barrier();
+    int any = 0;
+    const int first = 32 * s.self->warp;
+    for (int l = 0; l < 32 && first + l < (int)s.cta.bdim.x; ++l)
+        if (!s.fib[first + l].done && w.slot[l]) any = 1;
+    simt::warp_barrier();
+    return any;
+}
+
+template <class T> static inline T __ldcg(const T* p) { return *p; }
+static inline int __double2hiint(double x) { int64_t b; memcpy(&b, &x, 8); return (int)(b >> 32); }
+static inline int __double2loint(double x) { int64_t b; memcpy(&b, &x, 8); return (int)(b & 0xffffffff); }
+static inline double __hiloint2double(int hi, int lo)
+{
+    const uint64_t b = ((uint64_t)(uint32_t)hi << 32) | (uint32_t)lo;
+    double x; memcpy(&x, &b, 8); return x;
+}
+static inline int __float_as_int(float f) { int b; memcpy(&b, &f, 4); return b; }
+static inline float __int_as_float(int b) { float f; memcpy(&f, &b, 4); return f; }
+static inline int __ffs(int v) { return __builtin_ffs(v); }
+static inline int min(int a, int b) { return a < b ? a : b; }
+static inline int max(int a, int b) { return a > b ? a : b; }
+
+// atomics on global memory: one OS thread, so plain read-modify-write
+template <class T> static inline T atomicAdd(T* p, T v) { const T old = *p; *p = old + v; return old; }
+static inline unsigned atomicAdd(unsigned* p, int v) { const unsigned old = *p; *p = old + (unsigned)v; return old; }
+template <class T> static inline T atomicOr(T* p, T v) { const T old = *p; *p = old | v; return old; }
+
+// ---------------------------------------------------------------------------------------------------------------
+// the CUDA runtime calls the library makes: one device, in-order synchronous streams, memory = host memory
+// ---------------------------------------------------------------------------------------------------------------
+enum cudaError_t { cudaSuccess = 0, cudaErrorInvalidValue = 1 };
+enum cudaMemcpyKind { cudaMemcpyHostToHost, cudaMemcpyHostToDevice, cudaMemcpyDeviceToHost, cudaMemcpyDeviceToDevice };
+enum { cudaStreamNonBlocking = 1, cudaStreamCaptureModeThreadLocal = 1 };
+enum { cudaDevAttrMultiProcessorCount = 16 };
+enum { cudaFuncAttributeMaxDynamicSharedMemorySize = 8, cudaFuncAttributePreferredSharedMemoryCarveout = 9, cudaSharedmemCarveoutMaxShared = 100 };
+typedef struct simt_stream_st* cudaStream_t;
+typedef struct simt_event_st* cudaEvent_t;
+typedef std::vector<std::function<void()>>* cudaGraph_t;
+typedef std::vector<std::function<void()>>* cudaGraphExec_t;
+
+static inline const char* cudaGetErrorString(cudaError_t e) { return e == cudaSuccess ? "no error" : "simt: invalid value"; }
+static inline cudaError_t cudaGetLastError() { return cudaSuccess; }
+static inline cudaError_t cudaGetDevice(int* d) { *d = 0; return cudaSuccess; }
+static inline cudaError_t cudaSetDevice(int d) { return d == 0 ? cudaSuccess : cudaErrorInvalidValue; }
+static inline cudaError_t cudaDeviceGetAttribute(int* v, int attr, int)
+{
+    if (attr != cudaDevAttrMultiProcessorCount) return cudaErrorInvalidValue;
+    const char* e = getenv("NB_SIMT_SMS");                  // how many SMs the emulated device reports (the launch plans depend on it)
+    *v = e ? atoi(e) : 148;
+    return *v >= 1 ? cudaSuccess : cudaErrorInvalidValue;
+}
+static inline cudaError_t cudaMemcpyAsync(void* dst, const void* src, size_t n, cudaMemcpyKind, cudaStream_t)
+{
+    if (simt::S().capturing) return cudaErrorInvalidValue;  // the library captures kernel launches only
+    memmove(dst, src, n);
+    return cudaSuccess;
+}
+static inline cudaError_t cudaMemsetAsync(void* dst, int v, size_t n, cudaStream_t)
+{
+    if (simt::S().capturing) return cudaErrorInvalidValue;
+    memset(dst, v, n);
+    return cudaSuccess;
+}
+static inline cudaError_t cudaStreamSynchronize(cudaStream_t) { return cudaSuccess; }
+static inline cudaError_t cudaStreamCreateWithFlags(cudaStream_t* s, unsigned) { *s = nullptr; return cudaSuccess; }
+static inline cudaError_t cudaStreamDestroy(cudaStream_t) { return cudaSuccess; }
+static inline cudaError_t cudaEventCreate(cudaEvent_t* e) { *e = nullptr; return cudaSuccess; }
+static inline cudaError_t cudaEventDestroy(cudaEvent_t) { return cudaSuccess; }
+static inline cudaError_t cudaEventRecord(cudaEvent_t, cudaStream_t) { return cudaSuccess; }
+static inline cudaError_t cudaEventSynchronize(cudaEvent_t) { return cudaSuccess; }
+static inline cudaError_t cudaEventElapsedTime(float* ms, cudaEvent_t, cudaEvent_t) { *ms = 0.f; return cudaSuccess; }
+template <class K> static inline cudaError_t cudaFuncSetAttribute(K, int, int) { return cudaSuccess; }
+template <class K> static inline cudaError_t cudaOccupancyMaxActiveBlocksPerMultiprocessor(int* n, K, int, size_t) { *n = 4; return cudaSuccess; }
+
+// stream capture: launches are recorded instead of run; a graph launch replays them in order
+static inline cudaError_t cudaStreamBeginCapture(cudaStream_t, int)
+{
+    simt::State& s = simt::S();
+    if (s.capturing) return cudaErrorInvalidValue;
+    s.capture = new std::vector<std::function<void()>>();
+    s.capturing = true;
+    return cudaSuccess;
+}
+static inline cudaError_t cudaStreamEndCapture(cudaStream_t, cudaGraph_t* g)
+{
+    simt::State& s = simt::S();
+    if (!s.capturing) return cudaErrorInvalidValue;
+    s.capturing = false;
+    *g = s.capture; s.capture = nullptr;
+    return cudaSuccess;
+}
+static inline cudaError_t cudaGraphInstantiate(cudaGraphExec_t* e, cudaGraph_t g, unsigned long long)
+{
+    *e = new std::vector<std::function<void()>>(*g);
+    return cudaSuccess;
+}
+static inline cudaError_t cudaGraphDestroy(cudaGraph_t g) { delete g; return cudaSuccess; }
+static inline cudaError_t cudaGraphExecDestroy(cudaGraphExec_t e) { delete e; return cudaSuccess; }
+static inline cudaError_t cudaGraphLaunch(cudaGraphExec_t e, cudaStream_t)
+{
+    for (auto& node : *e) node();
+    return cudaSuccess;
+}

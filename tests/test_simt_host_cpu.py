@@ -1,0 +1,313 @@
+"""The WHOLE library on the host, without a GPU: nb_api.cu, nb_force.cu and nb_step.cu are compiled with g++ against a stand-in
+for the CUDA runtime (tests/host/simt/cuda_runtime.h: one CUDA thread = one fibre, CTAs one after the other, shuffles / votes /
+barriers / mbarriers with their CUDA meaning, stream capture and graph replay) and driven through their real C ABI with numpy
+buffers.  What is compared with the oracle here is therefore the STRUCTURE of the CUDA path - launch plans, the work queue, the
+j-split, tile staging, lanes-over-i to lanes-over-j warp units, the shuffle butterfly, the partial-sum layouts and the
+fixed-order reduction, predict-in-force, the one-kernel scheduler, the device-planned block step and its CUDA graph - which
+tests/test_kernel_source_cpu.py (the formulas alone) cannot see and which otherwise only the `-m gpu` tests exercise.
+
+The sources are taken as they are, except for what cannot be C++: `K<<<grid, block, smem, stream>>>(args)` becomes
+simt::launch(K, grid, block, smem, stream, args); the helpers of nb_force.cu that are inline PTX (fma / mul with fixed operand
+order, the rsqrt seeds, mbarrier and bulk-copy wrappers, the register ballast) are removed and tests/host/simt/nb_force_shims.h
+supplies their C++ meaning; `extern __shared__` becomes a static array; %globaltimer becomes a counter.  The test asserts that
+every one of these edits found its target.
+
+NOT a product path: nothing under paper_1411_5234_b200/ refers to this; binding.System still refuses to run without a CUDA
+device.  Not covered: the machine code, timing, memory ordering, races between CTAs (they run one after the other here).
+"""
+import ctypes as C
+import os
+import re
+import subprocess
+
+import numpy as np
+import pytest
+
+from paper_1411_5234_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+CSRC = os.path.join(ROOT, "paper_1411_5234_b200", "csrc")
+SIMT = os.path.join(ROOT, "tests", "host", "simt")
+TOL = 1e-11
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the edits
+# ---------------------------------------------------------------------------------------------------------------
+def strip_function(text, signature, replacement=""):
+    """remove the definition that starts with `signature` (up to the brace that closes its body)"""
+    assert text.count(signature) == 1, signature
+    i = text.index(signature)
+    j = text.index("{", i + len(signature))
+    depth = 0
+    for k in range(j, len(text)):
+        depth += text[k] == "{"
+        depth -= text[k] == "}"
+        if depth == 0:
+            return text[:i] + replacement + text[k + 1:]
+    raise AssertionError(signature)
+
+
+LAUNCH = re.compile(r"([A-Za-z_]\w*(?:<[^<>()]*>)?)<<<([^;]*?)>>>\(")
+
+
+def to_host_source(name, text):
+    n_launch = len(re.findall(r"<<<", text))
+    text, n = LAUNCH.subn(r"simt::launch(\1, \2, ", text)
+    assert n == n_launch, (name, n, n_launch)
+    if name == "nb_force.cu":
+        for sig in ("__device__ __forceinline__ double F(double a, double b, double c)",
+                    "__device__ __forceinline__ double M(double a, double b)",
+                    "__device__ __forceinline__ double rsqrt_seed(double s)",
+                    "__device__ __forceinline__ float rsqrt_f32(float s)",
+                    "__device__ __forceinline__ uint32_t smem_u32(const void* p)",
+                    "__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)",
+                    "__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)",
+                    "__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)",
+                    "__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)"):
+            text = strip_function(text, sig)
+        text = strip_function(text, "template <int N>\n__device__ __forceinline__ void reg_ballast(const ForceArgs& A)",
+                              "template <int N>\ninline void reg_ballast(const ForceArgs&) {}")
+        lines, out, skip = text.split("\n"), [], False
+        n_macros = 0
+        for l in lines:
+            if skip:
+                skip = l.rstrip().endswith("\\")
+                continue
+            if re.match(r"#define V(SUB|ADD|MUL|FMA|FNMA|RSQ|TWICE)\(", l):
+                n_macros += 1
+                skip = l.rstrip().endswith("\\")
+                continue
+            out.append(l)
+        assert n_macros == 7
+        text = "\n".join(out)
+        fence = '        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");\n'
+        assert text.count(fence) == 1
+        text = text.replace(fence, "")
+        dyn = "extern __shared__ __align__(128) double2 dyn_smem[];"
+        assert text.count(dyn) == 1
+        text = text.replace(dyn, "alignas(128) static double2 dyn_smem[16384];      // 256 KiB: more than any kernel asks for")
+        inc = '#include "nb_internal.h"\n'
+        assert text.count(inc) == 1
+        text = text.replace(inc, inc + '#include "nb_force_shims.h"\n')
+    if name == "nb_api.cu":
+        # test-only switch of the HOST COPY: nb_init without its all-active startup evaluations, so that the plans of large N
+        # with few active particles (config 5) can be run on the host in seconds; a, jerk, snap are then 0 and dt is not set
+        loop = "for (int pass = 1; pass <= (ctx->order == 4 ? 1 : 2); ++pass) {"
+        assert text.count(loop) == 1
+        text = text.replace(loop, 'for (int pass = 1; pass <= (getenv("NB_SIMT_SKIP_STARTUP") ? 0 : ctx->order == 4 ? 1 : 2); ++pass) {')
+    if name == "nb_step.cu":
+        timer = 'asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));'
+        assert text.count(timer) == 1
+        text = text.replace(timer, "now = simt::clock_ns();")
+    text = text.replace("__shared__ alignas(8)", "alignas(8) __shared__")      # g++ wants the attribute before `static`
+    assert not re.search(r"\basm\b", re.sub(r"//.*", "", text)), name
+    return text
+
+
+@pytest.fixture(scope="module")
+def SIM(tmp_path_factory):
+    from paper_1411_5234_b200 import binding as B
+    out = str(tmp_path_factory.mktemp("simt_host"))
+    srcs = []
+    for name in ("nb_api.cu", "nb_force.cu", "nb_step.cu"):
+        text = to_host_source(name, open(os.path.join(CSRC, name)).read())
+        path = os.path.join(out, name.replace(".cu", "_host.cpp"))
+        open(path, "w").write(text)
+        srcs.append(path)
+    so = os.path.join(out, "libnb_simt_host.so")
+    cmd = ["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-w", "-U_FORTIFY_SOURCE", "-D_FORTIFY_SOURCE=0", "-shared", "-fPIC", "-I" + SIMT, "-I" + CSRC,
+           "-I" + os.path.join(ROOT, "include")] + srcs + ["-o", so]
+    r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+    assert r.returncode == 0, r.stdout[-6000:]
+    L = C.CDLL(so)
+    ref = B.lib()                                            # the real library: only its ctypes signatures are taken from it
+    for name in B.EXPORTS:
+        f, g = getattr(L, name), getattr(ref, name)
+        f.argtypes, f.restype = g.argtypes, g.restype
+
+    class HostSimSystem(B.System):
+        """binding.System's marshalling over the host build: numpy workspace (between two bands of 0xA5), host pointers"""
+
+        def __init__(self, m, x, v, eps, n_sms=148, eta=0.0, eta_s=0.0, k_min=0, k_max=0, order=0, check_indices=0, precision=0,
+                     guard_bytes=1 << 16, skip_startup=False):
+            os.environ["NB_SIMT_SMS"] = str(n_sms)
+            os.environ.pop("NB_SIMT_SKIP_STARTUP", None)
+            if skip_startup: os.environ["NB_SIMT_SKIP_STARTUP"] = "1"
+            self.L, self.host, self.device, self.N, self.ctx = L, True, 0, int(m.shape[0]), C.c_void_p()
+            nbytes = L.nb_workspace_bytes(self.N)
+            self._guard = (int(guard_bytes) + 255) // 256 * 256
+            self.workspace = np.empty(nbytes + 256 + 2 * self._guard, dtype=np.uint8)
+            self.workspace[:self._guard + 256] = 0xA5
+            self.workspace[-(self._guard + 256):] = 0xA5
+            base = (self.workspace.ctypes.data + self._guard + 255) // 256 * 256
+            self._ws_off, self._ws_bytes = base - self.workspace.ctypes.data, nbytes
+            self.cfg = B.nb_config(0, None, C.c_void_p(base), nbytes, 0, eta, eta_s, k_min, k_max, order, check_indices, precision)
+            m, x, v = self._in(m, (self.N,)), self._in(x, (self.N, 3)), self._in(v, (self.N, 3))
+            self._check(L.nb_init(C.byref(self.ctx), self.N, B._ptr(m), B._ptr(x), B._ptr(v), float(eps), C.byref(self.cfg)))
+
+        def guards_intact(self):
+            lo, hi = self.workspace[:self._ws_off], self.workspace[self._ws_off + self._ws_bytes:]
+            return bool((lo == 0xA5).all()) and bool((hi == 0xA5).all())
+
+    return HostSimSystem
+
+
+def relvec(g, o):
+    return np.linalg.norm(g - o, axis=-1) / np.linalg.norm(o, axis=-1)
+
+
+def assert_force_parity(g, o, tol=TOL):
+    for name, a, b in zip(("acc", "jerk", "snap"), g[:3], o[:3]):
+        assert relvec(a, b).max() <= tol, (name, relvec(a, b).max())
+    assert np.abs(g[3] / o[3] - 1).max() <= tol, ("pot", np.abs(g[3] / o[3] - 1).max())
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# config 1 through the host build: startup, one evaluation, eight shared steps
+# ---------------------------------------------------------------------------------------------------------------
+def test_config1_startup_force_and_steps(SIM, oracle):
+    c, m, x, v = W.config_inputs(1)
+    g = SIM(m, x, v, c.eps)
+    o = oracle.OracleSystem(m, x, v, c.eps)
+    for f, ref in (("A", o.a), ("J", o.j), ("S", o.s)):
+        assert relvec(g.nb_get_state(f), ref).max() <= TOL
+    assert np.array_equal(g.nb_get_state("DT"), o.dt)
+    g.nb_predict(0.0); o.predict(0.0)
+    assert_force_parity(g.nb_force(), o.force())
+    for _ in range(8):
+        t = o.t[0] + c.dt
+        g.nb_predict(t); g.nb_force(outputs=False); g.nb_corrector(None, c.dt)
+        o.shared_step(c.dt)
+    assert np.abs(g.nb_get_state("X") - o.x).max() <= 1e-13 and np.abs(g.nb_get_state("V") - o.v).max() <= 1e-12
+    Kg, Wg = g.nb_energy()
+    Ko, Wo = o.energy()
+    assert abs((Kg + Wg) - (Ko + Wo)) / abs(Ko + Wo) <= 1e-10
+    assert g.guards_intact()
+    g.nb_free()
+
+
+def oracle_on_records(oracle, g, eps, idx):
+    """O1 on the predicted records the kernels read (nb_force is a pure function of them)"""
+    m, xp, vp, ap = g.nb_get_state("M"), g.nb_get_state("XP"), g.nb_get_state("VP"), g.nb_get_state("AP")
+    return oracle.hermite6.force(m, xp, vp, ap, eps, idx)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# every kernel shape: warp units of every width (lanes over i ... lanes over j), padded and decomposed rests, ragged CTA
+# tiles, the j-split with its two partial-sum layouts and the reduction, on a "device" of 148 SMs and on one of 3
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,eps,masses,n_sms", [(1500, 1e-3, "equal", 148), (1027, 0.0, "kroupa", 3), (2, 0.0, "equal", 148), (257, 0.0, "kroupa", 148)])
+def test_force_shapes_and_active_sets(SIM, oracle, N, eps, masses, n_sms):
+    from paper_1411_5234_b200 import binding as B
+    m, x, v = W.plummer(N, 1000 + N, masses)
+    g = SIM(m, x, v, eps, n_sms=n_sms)
+    g.nb_predict(2.0 ** -9); g.nb_force(outputs=False); g.nb_corrector(None, 2.0 ** -9)     # all derivatives non-zero, D != 0 next
+    g.nb_predict(2.0 ** -9 + 2.0 ** -11)
+    rng = np.random.default_rng(N)
+    sizes = sorted({1, 2, 3, 5, 7, 9, 16, 17, 21, 24, 31, 33, 64, 97, 129, 255, 256, 300, 512, 1023, 1024, N} & set(range(1, N + 1)) | {N})
+    shapes = set()
+    for n_act in sizes:
+        idx = None if n_act == N else rng.choice(N, n_act, replace=False).astype(np.int32)
+        assert_force_parity(g.nb_force(idx), oracle_on_records(oracle, g, eps, idx))
+        p = B.nb_plan_force(N, n_act, n_sms)
+        workers = min(p.n_units * p.n_split, n_sms * 4) if p.kernel == 0 else 4 * min((p.n_units * p.n_split + 3) // 4, n_sms * 4)
+        shapes.add((p.kernel, p.n_split > 1, p.n_units * p.n_split > workers))
+    if N >= 1024:                                             # both kernels, split launches, and (3 SMs) the work queue in both
+        assert {k for k, _, _ in shapes} == {0, 1} and True in {sp for _, sp, _ in shapes}
+        if n_sms == 3: assert {k for k, _, q in shapes if q} == {0, 1}
+    perm = rng.permutation(N).astype(np.int32)                # permuted full list: row k <-> idx[k]
+    assert_force_parity(g.nb_force(perm), oracle_on_records(oracle, g, eps, perm))
+    # no j-split at all (the paper's "Bfactor off" arm): same results to rounding
+    g.nb_set_max_split(1)
+    idx = rng.choice(N, min(N, 37), replace=False).astype(np.int32)
+    assert_force_parity(g.nb_force(idx), oracle_on_records(oracle, g, eps, idx))
+    assert g.guards_intact()
+    g.nb_free()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# block steps: the one-kernel scheduler bit for bit, predictor / corrector / levels after every step
+# ---------------------------------------------------------------------------------------------------------------
+def test_block_steps_against_oracle(SIM, oracle):
+    N, eps = 384, 1e-3
+    m, x, v = W.plummer(N, 77, "kroupa")
+    g = SIM(m, x, v, eps)
+    o = oracle.OracleSystem(m, x, v, eps)
+    assert np.array_equal(g.nb_get_state("DT"), o.dt)
+    n_steps = 0
+    while True:
+        tg, ng, actg = g.nb_next_block()
+        to, acto = o.next_block()
+        assert tg == to and ng == acto.size and np.array_equal(actg, acto)
+        if to > 2.0 ** -5: break
+        g.nb_predict(tg); o.predict(to)
+        for f, ref in (("XP", o.xp), ("VP", o.vp), ("AP", o.ap)):
+            assert relvec(g.nb_get_state(f), ref).max() <= 1e-12, f
+        assert_force_parity(g.nb_force(actg), o.force(acto), 1e-10)
+        g.nb_corrector(actg, 0.0); o.corrector(acto, 0.0)
+        assert np.array_equal(g.nb_get_state("T"), o.t) and np.array_equal(g.nb_get_state("DT"), o.dt)
+        n_steps += 1
+    assert n_steps > 20
+    assert relvec(g.nb_get_state("X"), o.x).max() <= 1e-12 and relvec(g.nb_get_state("V"), o.v).max() <= 1e-11
+    g.nb_free()
+
+
+@pytest.mark.parametrize("N,eps,masses,n_sms", [(1200, 1e-4, "kroupa", 148), (300, 0.0, "equal", 5)])
+def test_run_blocks_is_bitwise_the_separate_calls(SIM, N, eps, masses, n_sms):
+    """nb_run_blocks (scheduler + plan on the device, predict-in-force, reduction + corrector in one kernel, the captured graph)
+    against the same steps call by call: identical schedules, bit-identical states; step budget and t_end respected"""
+    m, x, v = W.plummer(N, 77 + N, masses)
+    g1, g2 = SIM(m, x, v, eps, n_sms=n_sms), SIM(m, x, v, eps, n_sms=n_sms)
+    t_end = 2.0 ** -6
+    steps, acts = 0, 0
+    while True:
+        t, n, act = g1.nb_next_block()
+        if t > t_end: break
+        g1.nb_predict(t); g1.nb_force(act, outputs=False); g1.nb_corrector(act, 0.0)
+        steps += 1; acts += n
+    assert steps >= 10
+    s_a, t_a, n_a = g2.nb_run_blocks(t_end, max_steps=5)
+    assert s_a == 5 and t_a > 0
+    s_b, t_b, n_b = g2.nb_run_blocks(t_end / 2)
+    assert t_b <= t_end / 2
+    s_c, t_c, n_c = g2.nb_run_blocks(t_end)
+    assert s_a + s_b + s_c == steps and n_a + n_b + n_c == acts and t_c == t_end
+    assert g2.nb_run_blocks(t_end) == (0, -1.0, 0)
+    for f in ("X", "V", "A", "J", "S", "C", "T", "DT"):
+        assert np.array_equal(g1.nb_get_state(f), g2.nb_get_state(f)), f
+    na, _ = g2.nb_step_log()
+    assert na.size == steps and na.sum() == acts               # the device's own record of the steps
+    t1, n1, a1 = g1.nb_next_block(); t2, n2, a2 = g2.nb_next_block()
+    assert t1 == t2 and np.array_equal(a1, a2)
+    assert g1.guards_intact() and g2.guards_intact()
+    g1.nb_free(); g2.nb_free()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# config 5's plans on the host: N = 2^18 with a handful of active particles (one or two warp units x 1024-2048 slices; a whole
+# reduction block per particle and the [component][row][slice] layout of the partial sums, which small N never reaches)
+# ---------------------------------------------------------------------------------------------------------------
+def reduce_threads(n_act, S):
+    """nb_plan.h:nb_reduce_threads restated - ONLY to assert which reduction shape a case exercised"""
+    T = 1
+    while T < 256 and T * 4 <= S and n_act * T < (1 << 18): T *= 2
+    return T
+
+
+def test_large_n_small_active_sets(SIM, oracle):
+    from paper_1411_5234_b200 import binding as B
+    N, eps = 1 << 18, 1e-4
+    m, x, v = W.plummer(N, W.BASE_SEED + 4, "equal")
+    g = SIM(m, x, v, eps, skip_startup=True)                 # (the startup's 1.4e11 pairs are not for the host)
+    rng = np.random.default_rng(5)
+    a = rng.normal(size=(N, 3))
+    g.nb_set_state("A", a)
+    g.nb_predict(0.0)                                        # t_i = 0: the records are x, v and the a just set
+    for n_act in (1, 3, 8, 24):
+        idx = W.active_set(N, n_act, 50 + n_act)
+        assert_force_parity(g.nb_force(idx), oracle.hermite6.force(m, x, v, a, eps, idx))
+        p = B.nb_plan_force(N, n_act, 148)
+        assert p.kernel == 1 and p.n_split >= 1024 and reduce_threads(n_act, p.n_split) == 256     # a reduction block per particle
+    assert g.guards_intact()
+    g.nb_free()
