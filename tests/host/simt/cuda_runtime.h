@@ -62,8 +62,18 @@ struct Warp {
     unsigned long long slot[32];
 };
 
+// Switching fibres: glibc's swapcontext saves and restores the signal mask with a system call on every switch, which dominates
+// the run time of kernels that synchronise once per j-tile.  On x86-64 the switch is therefore done by hand (simt_switch.S:
+// callee-saved registers and the stack pointer, nothing else - no fibre changes the FP control words or the signal mask);
+// elsewhere ucontext is used.
+#if defined(__x86_64__) && !defined(NB_SIMT_UCONTEXT)
+#define NB_SIMT_FAST_SWITCH 1
+extern "C" void nb_simt_switch(void** save_sp, void* load_sp);
+#endif
+
 struct Fibre {
     ucontext_t ctx;
+    void* sp = nullptr;
     uint3 tid{0, 0, 0};
     int lane = 0, warp = 0;
     bool done = true;
@@ -80,6 +90,7 @@ struct State {
     Fibre fib[MAX_THREADS];
     char* stacks = nullptr;
     ucontext_t main_ctx;
+    void* main_sp = nullptr;
     Fibre* self = nullptr;
     Cta cta;
     std::function<void()> body;               // the kernel call of the launch that is running
@@ -91,7 +102,26 @@ struct State {
 
 inline State& S() { static State s; return s; }
 
-inline void yield() { State& s = S(); ++s.switches; swapcontext(&s.self->ctx, &s.main_ctx); }
+inline void to_main(Fibre* f)
+{
+    State& s = S();
+#ifdef NB_SIMT_FAST_SWITCH
+    nb_simt_switch(&f->sp, s.main_sp);
+#else
+    swapcontext(&f->ctx, &s.main_ctx);
+#endif
+}
+inline void to_fibre(Fibre* f)
+{
+    State& s = S();
+    s.self = f;
+#ifdef NB_SIMT_FAST_SWITCH
+    nb_simt_switch(&s.main_sp, f->sp);
+#else
+    swapcontext(&s.main_ctx, &f->ctx);
+#endif
+}
+inline void yield() { State& s = S(); ++s.switches; to_main(s.self); }
 
 inline void fibre_entry()
 {
@@ -102,7 +132,8 @@ inline void fibre_entry()
     s.progress += 1;
     s.cta.alive -= 1;
     s.cta.warps[f->warp].alive -= 1;
-    swapcontext(&f->ctx, &s.main_ctx);
+    to_main(f);                                  // never resumed
+    abort();
 }
 
 // barrier over the threads of the CTA that have not exited
@@ -145,19 +176,27 @@ inline void run_cta(unsigned block, unsigned bid, unsigned grid)
     for (unsigned t = 0; t < block; ++t) {
         Fibre& f = s.fib[t];
         f.tid = uint3{t, 0, 0}; f.lane = (int)(t & 31); f.warp = (int)(t >> 5); f.done = false;
+#ifdef NB_SIMT_FAST_SWITCH
+        // a fresh stack as nb_simt_switch expects to find it: six zeroed callee-saved registers, then the address it returns
+        // to; at fibre_entry's first instruction the stack pointer is 8 mod 16, as after a call
+        void** top = (void**)(s.stacks + STACK_BYTES * (t + 1));
+        top[-2] = (void*)fibre_entry; top[-1] = nullptr;
+        for (int r = 3; r <= 8; ++r) top[-r] = nullptr;
+        f.sp = (void*)(top - 8);
+#else
         getcontext(&f.ctx);
         f.ctx.uc_stack.ss_sp = s.stacks + STACK_BYTES * t;
         f.ctx.uc_stack.ss_size = STACK_BYTES;
         f.ctx.uc_link = nullptr;
         makecontext(&f.ctx, (void (*)())fibre_entry, 0);
+#endif
     }
     while (c.alive > 0) {
         const long long before = s.progress;
         for (unsigned t = 0; t < block; ++t) {
             Fibre& f = s.fib[t];
             if (f.done) continue;
-            s.self = &f;
-            swapcontext(&s.main_ctx, &f.ctx);
+            to_fibre(&f);
         }
         s.self = nullptr;
         // a fibre yields only while it waits for something another fibre of the CTA has to do: a whole round in which nobody

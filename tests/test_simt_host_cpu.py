@@ -117,7 +117,7 @@ def SIM(tmp_path_factory):
         srcs.append(path)
     so = os.path.join(out, "libnb_simt_host.so")
     cmd = ["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-w", "-U_FORTIFY_SOURCE", "-D_FORTIFY_SOURCE=0", "-shared", "-fPIC", "-I" + SIMT, "-I" + CSRC,
-           "-I" + os.path.join(ROOT, "include")] + srcs + ["-o", so]
+           "-I" + os.path.join(ROOT, "include")] + srcs + [os.path.join(SIMT, "simt_switch.S"), "-o", so]
     r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     assert r.returncode == 0, r.stdout[-6000:]
     L = C.CDLL(so)
