@@ -416,3 +416,98 @@ def test_mixed_precision_on_the_host(SIM, oracle):
     g.nb_free()
     with pytest.raises(B.NBError):
         SIM(m, x, v, eps, precision=B.NB_PREC_MIXED, order=8)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the boundary through the host build (host-pointer contexts): what include/nb.h promises about call order, argument and index
+# errors, state access, the scheduler on crafted times, an eps whose square underflows, bitwise repeatability
+# ---------------------------------------------------------------------------------------------------------------
+def test_scheduler_on_crafted_times_and_state_io(SIM, oracle):
+    N = 1500
+    m, x, v = W.plummer(N, 9)
+    g = SIM(m, x, v, 1e-3, skip_startup=True)
+    assert np.array_equal(g.nb_get_state("M"), m) and np.array_equal(g.nb_get_state("X"), x) and np.array_equal(g.nb_get_state("V"), v)
+    rng = np.random.default_rng(3)
+    dt = 2.0 ** rng.integers(-12, -3, N)
+    t = dt * rng.integers(0, 5, N)
+    g.nb_set_state("T", t); g.nb_set_state("DT", dt)
+    assert np.array_equal(g.nb_get_state("T"), t) and np.array_equal(g.nb_get_state("DT"), dt)
+    tn, n, act = g.nb_next_block()
+    act_o, tn_o = np.zeros(N, dtype=np.int32), C.c_double()
+    n_o = oracle.lib("ld").oracle_next_block(N, oracle.hermite6._p(t), oracle.hermite6._p(dt), C.byref(tn_o), oracle.hermite6._pi(act_o))
+    assert tn == tn_o.value and n == n_o and np.array_equal(act, act_o[:n_o])
+    g.nb_set_state("T", np.zeros(N)); g.nb_set_state("DT", np.full(N, 0.125))            # everyone active
+    tn, n, act = g.nb_next_block()
+    assert tn == 0.125 and n == N and np.array_equal(act, np.arange(N, dtype=np.int32))
+    idx = np.array([5, N - 1, 0, 17], dtype=np.int32)                                     # packed fields: neighbours untouched
+    for f in ("X", "V", "A", "J", "S", "C"):
+        val = rng.normal(size=(4, 3))
+        g.nb_set_state(f, val, idx)
+        assert np.array_equal(g.nb_get_state(f, idx), val) and np.array_equal(g.nb_get_state(f)[idx], val)
+    assert np.array_equal(g.nb_get_state("M"), m) and np.array_equal(g.nb_get_state("T"), np.zeros(N))
+    assert g.guards_intact()
+    g.nb_free()
+
+
+def test_call_order_argument_and_index_errors(SIM):
+    from paper_1411_5234_b200 import binding as B
+    N = 900
+    m, x, v = W.plummer(N, 31)
+    g = SIM(m, x, v, 1e-3)                                   # host pointers: index lists are verified by default
+    with pytest.raises(B.NBError) as e:
+        g.nb_force()
+    assert e.value.status == B.NB_ESTATE                     # no nb_predict yet
+    g.nb_predict(2.0 ** -10)
+    with pytest.raises(B.NBError) as e:
+        g.nb_corrector(None, 0.1)
+    assert e.value.status == B.NB_ESTATE                     # no nb_force yet
+    assert g.L.nb_force(g.ctx, None, N + 1, None, None, None, None) == B.NB_EINVAL
+    assert g.L.nb_force(g.ctx, None, 5, None, None, None, None) == B.NB_EINVAL            # NULL list needs n_act == N
+    assert g.L.nb_force(g.ctx, None, 0, None, None, None, None) == B.NB_OK                # empty active set: no-op
+    good = W.active_set(N, 100, 1)
+    for bad in (np.array([5, N, 7], dtype=np.int32), np.array([-1], dtype=np.int32), np.array([2 ** 31 - 1, 0], dtype=np.int32)):
+        for call in (lambda: g.nb_force(bad), lambda: g.nb_get_state("X", bad), lambda: g.nb_set_state("X", np.zeros((bad.size, 3)), bad)):
+            with pytest.raises(B.NBError) as e:
+                call()
+            assert e.value.status == B.NB_EINVAL
+        assert g.nb_check_indices(bad) == B.NB_EINVAL
+    dup = np.array([4, 9, 4], dtype=np.int32)
+    with pytest.raises(B.NBError) as e:
+        g.nb_force(dup)
+    assert e.value.status == B.NB_EINVAL
+    assert g.nb_check_indices(dup) == B.NB_EINVAL and g.nb_check_indices(dup, unique=False) == B.NB_OK
+    assert np.array_equal(g.nb_get_state("X", dup), x[dup])                               # reading a particle twice is fine
+    assert g.nb_check_indices(good) == B.NB_OK and g.nb_check_indices(np.arange(N, dtype=np.int32)) == B.NB_OK
+    g.nb_force(good, outputs=False)                          # nothing was corrupted: the context still works
+    with pytest.raises(B.NBError) as e:
+        g.nb_corrector(np.concatenate([good[:-1], good[:1]]), 2.0 ** -10)
+    assert e.value.status == B.NB_EINVAL
+    g.nb_corrector(good, 2.0 ** -10)
+    assert np.isfinite(g.nb_get_state("X")).all() and np.array_equal(g.nb_get_state("M"), m) and g.guards_intact()
+    g.nb_free()
+    gh = SIM(m, x, v, 1e-3, check_indices=-1, skip_startup=True)                          # checking switched off ...
+    assert gh.nb_check_indices(dup) == B.NB_EINVAL                                        # ... the explicit call still checks
+    gh.nb_free()
+    for kw in (dict(order=5), dict(k_min=-3, k_max=-20), dict(eta=-1.0), dict(precision=7)):
+        with pytest.raises(B.NBError) as e:
+            SIM(m, x, v, 1e-3, **kw)
+        assert e.value.status == B.NB_EINVAL
+
+
+def test_tiny_softening_and_repeatability(SIM, oracle):
+    """0 < eps < 1.5e-154: eps^2 underflows, the launch must take the index-masked (eps = 0) kernels and not produce NaN;
+    and the same call twice gives the same bits (fixed-order reduction, work queue left at zero)."""
+    N = 500
+    m, x, v = W.plummer(N, 33)
+    g0, g1 = SIM(m, x, v, 0.0), SIM(m, x, v, 1e-160)
+    for f in ("A", "J", "S"):
+        a0, a1 = g0.nb_get_state(f), g1.nb_get_state(f)
+        assert np.isfinite(a1).all() and np.array_equal(a0, a1), f
+    g1.nb_predict(2.0 ** -10)
+    for n_act in (3, 50, 300, N):
+        idx = None if n_act == N else W.active_set(N, n_act, 2)
+        got = g1.nb_force(idx)
+        assert_force_parity(got, oracle_on_records(oracle, g1, 0.0, idx))
+        again = g1.nb_force(idx)
+        assert all(np.array_equal(p, q) for p, q in zip(got, again)), n_act
+    g0.nb_free(); g1.nb_free()
