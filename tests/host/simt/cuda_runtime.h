@@ -96,7 +96,7 @@ struct State {
     std::function<void()> body;               // the kernel call of the launch that is running
     bool capturing = false;
     std::vector<std::function<void()>>* capture = nullptr;
-    long long launches = 0, switches = 0, progress = 0;   // progress: arrivals, releases, exits, completed copies
+    long long launches = 0, permuted = 0, switches = 0, progress = 0;   // permuted: launches run in another CTA order; progress: arrivals, releases, exits, completed copies
     unsigned long long clock = 0;
 };
 
@@ -214,7 +214,27 @@ inline void launch(void (*kernel)(P...), long long grid, long long block, size_t
         State& st = S();
         st.launches += 1;
         st.body = [kernel, &held]() { std::apply(kernel, held); };
-        for (long long b = 0; b < grid; ++b) run_cta((unsigned)block, (unsigned)b, (unsigned)grid);
+        // The order in which a GPU starts and finishes the CTAs of a grid is not defined.  NB_SIMT_CTA_ORDER = reverse | shuffle
+        // (a different permutation for every launch, reproducible) runs them in another order than 0, 1, 2, ...: work queues,
+        // last-block-done patterns and fixed-order reductions must give the same bits in any of them.
+        const char* order = getenv("NB_SIMT_CTA_ORDER");
+        if (order && (!strcmp(order, "reverse") || !strcmp(order, "shuffle"))) {
+            std::vector<unsigned> perm((size_t)grid);
+            for (long long b = 0; b < grid; ++b) perm[(size_t)b] = (unsigned)(order[0] == 'r' ? grid - 1 - b : b);
+            if (order[0] == 's') {
+                unsigned long long x = 0x9E3779B97F4A7C15ull * (unsigned long long)(st.launches + 1);
+                for (long long b = grid - 1; b > 0; --b) {                      // Fisher-Yates on a splitmix64 stream
+                    x += 0x9E3779B97F4A7C15ull;
+                    unsigned long long z = x;
+                    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull; z = (z ^ (z >> 27)) * 0x94D049BB133111EBull; z ^= z >> 31;
+                    std::swap(perm[(size_t)b], perm[(size_t)(z % (unsigned long long)(b + 1))]);
+                }
+            }
+            st.permuted += grid > 1;
+            for (unsigned b : perm) run_cta((unsigned)block, b, (unsigned)grid);
+        } else {
+            for (long long b = 0; b < grid; ++b) run_cta((unsigned)block, (unsigned)b, (unsigned)grid);
+        }
         st.body = nullptr;
     };
     if (s.capturing) s.capture->push_back(run);
@@ -224,6 +244,9 @@ inline void launch(void (*kernel)(P...), long long grid, long long block, size_t
 inline unsigned long long clock_ns() { return S().clock += 1000; }
 
 }  // namespace simt
+
+// for the test that permutes the CTAs: how many multi-CTA launches ran in another order than 0, 1, 2, ...
+extern "C" __attribute__((weak, used)) long long nb_simt_permuted_launches() { return simt::S().permuted; }
 
 #define threadIdx (simt::S().self->tid)
 #define blockIdx (simt::S().cta.bid)

@@ -511,3 +511,44 @@ def test_tiny_softening_and_repeatability(SIM, oracle):
         again = g1.nb_force(idx)
         assert all(np.array_equal(p, q) for p, q in zip(got, again)), n_act
     g0.nb_free(); g1.nb_free()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the order of the CTAs: a GPU starts and retires the CTAs of a grid in no defined order.  The host build runs them 0, 1, 2, ...
+# by default; here the same calls run with every grid reversed and with every grid shuffled (tests/host/simt/cuda_runtime.h:
+# NB_SIMT_CTA_ORDER).  The work queue (first item = CTA number, then the counter), its self-resetting counters, the scheduler's
+# last-block pass and the fixed-order reductions must give the same BITS whichever CTA comes first
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_sms", [148, 3])
+def test_results_do_not_depend_on_the_order_of_the_ctas(SIM, n_sms):
+    N, eps, t_end = 1100, 1e-4, 2.0 ** -7
+    m, x, v = W.plummer(N, 606, "kroupa")
+    rng = np.random.default_rng(6)
+    lists = [None] + [rng.choice(N, n, replace=False).astype(np.int32) for n in (1, 7, 40, 97, 300, 640)]
+    results, permuted = {}, {}
+    try:
+        for order in ("natural", "reverse", "shuffle"):
+            os.environ["NB_SIMT_CTA_ORDER"] = order
+            g = SIM(m, x, v, eps, n_sms=n_sms)
+            out = [g.nb_get_state(f) for f in ("A", "J", "S", "DT")]                     # startup: all-active launches
+            g.nb_predict(2.0 ** -10)
+            for idx in lists:
+                out += list(g.nb_force(idx))
+            steps, t_last, n_sum = g.nb_run_blocks(t_end)
+            assert steps >= 5 and t_last == t_end
+            out += [np.array([steps, n_sum])] + [g.nb_get_state(f) for f in ("X", "V", "A", "J", "S", "C", "T", "DT")]
+            t, n, act = g.nb_next_block()
+            out += [np.array([t, n]), act]
+            assert g.guards_intact()
+            g.L.nb_simt_permuted_launches.restype = C.c_longlong
+            permuted[order] = g.L.nb_simt_permuted_launches()
+            g.nb_free()
+            results[order] = out
+    finally:
+        os.environ.pop("NB_SIMT_CTA_ORDER", None)
+    # the switch took effect: dozens of multi-CTA launches ran permuted in each of the two modes (the counter is cumulative)
+    assert permuted["reverse"] - permuted["natural"] > 30 and permuted["shuffle"] - permuted["reverse"] > 30
+    for order in ("reverse", "shuffle"):
+        assert len(results[order]) == len(results["natural"])
+        for k, (p, q) in enumerate(zip(results["natural"], results[order])):
+            assert np.array_equal(p, q), (order, k)
