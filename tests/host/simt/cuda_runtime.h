@@ -96,7 +96,7 @@ struct State {
     std::function<void()> body;               // the kernel call of the launch that is running
     bool capturing = false;
     std::vector<std::function<void()>>* capture = nullptr;
-    long long launches = 0, permuted = 0, switches = 0, progress = 0;   // permuted: launches run in another CTA order; progress: arrivals, releases, exits, completed copies
+    long long launches = 0, permuted = 0, reordered = 0, switches = 0, progress = 0;   // permuted: launches run in another CTA order; reordered: CTAs run in another thread order; progress: arrivals, releases, exits, completed copies
     unsigned long long clock = 0;
 };
 
@@ -191,10 +191,27 @@ inline void run_cta(unsigned block, unsigned bid, unsigned grid)
         makecontext(&f.ctx, (void (*)())fibre_entry, 0);
 #endif
     }
+    // Which thread of a CTA runs first between two synchronisation points is not defined either.  NB_SIMT_THREAD_ORDER =
+    // reverse | shuffle (a new permutation every round, reproducible) resumes the fibres in another order than 0, 1, 2, ...: a
+    // read of shared or global memory that is not ordered after its write by a barrier then sees the old value in one of the
+    // orders, and the results differ (a poor man's racecheck: it finds missing barriers, not memory-model subtleties).
+    static unsigned ord[MAX_THREADS];
+    const char* torder = getenv("NB_SIMT_THREAD_ORDER");
+    const int tmode = !torder ? 0 : !strcmp(torder, "reverse") ? 1 : !strcmp(torder, "shuffle") ? 2 : 0;
+    for (unsigned t = 0; t < block; ++t) ord[t] = tmode == 1 ? block - 1 - t : t;
+    unsigned long long rnd = 0x9E3779B97F4A7C15ull * (unsigned long long)(s.launches * 4099 + bid + 1);
+    s.reordered += tmode != 0;
     while (c.alive > 0) {
         const long long before = s.progress;
-        for (unsigned t = 0; t < block; ++t) {
-            Fibre& f = s.fib[t];
+        if (tmode == 2)
+            for (unsigned t = block - 1; t > 0; --t) {
+                rnd += 0x9E3779B97F4A7C15ull;
+                unsigned long long z = rnd;
+                z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull; z = (z ^ (z >> 27)) * 0x94D049BB133111EBull; z ^= z >> 31;
+                std::swap(ord[t], ord[z % (t + 1)]);
+            }
+        for (unsigned k = 0; k < block; ++k) {
+            Fibre& f = s.fib[ord[k]];
             if (f.done) continue;
             to_fibre(&f);
         }
@@ -247,6 +264,7 @@ inline unsigned long long clock_ns() { return S().clock += 1000; }
 
 // for the test that permutes the CTAs: how many multi-CTA launches ran in another order than 0, 1, 2, ...
 extern "C" __attribute__((weak, used)) long long nb_simt_permuted_launches() { return simt::S().permuted; }
+extern "C" __attribute__((weak, used)) long long nb_simt_reordered_ctas() { return simt::S().reordered; }
 
 #define threadIdx (simt::S().self->tid)
 #define blockIdx (simt::S().cta.bid)

@@ -514,21 +514,29 @@ def test_tiny_softening_and_repeatability(SIM, oracle):
 
 
 # ---------------------------------------------------------------------------------------------------------------
-# the order of the CTAs: a GPU starts and retires the CTAs of a grid in no defined order.  The host build runs them 0, 1, 2, ...
-# by default; here the same calls run with every grid reversed and with every grid shuffled (tests/host/simt/cuda_runtime.h:
-# NB_SIMT_CTA_ORDER).  The work queue (first item = CTA number, then the counter), its self-resetting counters, the scheduler's
-# last-block pass and the fixed-order reductions must give the same BITS whichever CTA comes first
+# the order of the CTAs and of the threads: a GPU starts and retires the CTAs of a grid in no defined order, and which thread
+# of a CTA runs first between two synchronisation points is not defined either.  The host build runs both 0, 1, 2, ... by
+# default; here the same calls run with every grid reversed / shuffled and with the threads of every CTA resumed in reverse /
+# in a new random order every round (tests/host/simt/cuda_runtime.h: NB_SIMT_CTA_ORDER, NB_SIMT_THREAD_ORDER).  The work queue
+# (first item = CTA number, then the counter), its self-resetting counters, the scheduler's last-block pass and the fixed-order
+# reductions must give the same BITS whichever CTA comes first; and a shared-memory or global read that no barrier orders after
+# its write would see the old value in one of the thread orders (a poor man's racecheck: compute-sanitizer is closed on the
+# pool, profiles/r02_sanitizer.md).  Not covered: memory-model subtleties of real concurrent execution
 # ---------------------------------------------------------------------------------------------------------------
+ORDERS = [("natural", "natural"), ("reverse", "natural"), ("shuffle", "natural"), ("natural", "reverse"), ("natural", "shuffle"),
+          ("shuffle", "shuffle")]
+
+
 @pytest.mark.parametrize("n_sms", [148, 3])
-def test_results_do_not_depend_on_the_order_of_the_ctas(SIM, n_sms):
+def test_results_do_not_depend_on_the_order_of_ctas_and_threads(SIM, n_sms):
     N, eps, t_end = 1100, 1e-4, 2.0 ** -7
     m, x, v = W.plummer(N, 606, "kroupa")
     rng = np.random.default_rng(6)
     lists = [None] + [rng.choice(N, n, replace=False).astype(np.int32) for n in (1, 7, 40, 97, 300, 640)]
-    results, permuted = {}, {}
+    results, counters = [], []
     try:
-        for order in ("natural", "reverse", "shuffle"):
-            os.environ["NB_SIMT_CTA_ORDER"] = order
+        for cta_order, thread_order in ORDERS:
+            os.environ["NB_SIMT_CTA_ORDER"], os.environ["NB_SIMT_THREAD_ORDER"] = cta_order, thread_order
             g = SIM(m, x, v, eps, n_sms=n_sms)
             out = [g.nb_get_state(f) for f in ("A", "J", "S", "DT")]                     # startup: all-active launches
             g.nb_predict(2.0 ** -10)
@@ -540,15 +548,17 @@ def test_results_do_not_depend_on_the_order_of_the_ctas(SIM, n_sms):
             t, n, act = g.nb_next_block()
             out += [np.array([t, n]), act]
             assert g.guards_intact()
-            g.L.nb_simt_permuted_launches.restype = C.c_longlong
-            permuted[order] = g.L.nb_simt_permuted_launches()
+            g.L.nb_simt_permuted_launches.restype = g.L.nb_simt_reordered_ctas.restype = C.c_longlong
+            counters.append((g.L.nb_simt_permuted_launches(), g.L.nb_simt_reordered_ctas()))
             g.nb_free()
-            results[order] = out
+            results.append(out)
     finally:
-        os.environ.pop("NB_SIMT_CTA_ORDER", None)
-    # the switch took effect: dozens of multi-CTA launches ran permuted in each of the two modes (the counter is cumulative)
-    assert permuted["reverse"] - permuted["natural"] > 30 and permuted["shuffle"] - permuted["reverse"] > 30
-    for order in ("reverse", "shuffle"):
-        assert len(results[order]) == len(results["natural"])
-        for k, (p, q) in enumerate(zip(results["natural"], results[order])):
-            assert np.array_equal(p, q), (order, k)
+        os.environ.pop("NB_SIMT_CTA_ORDER", None); os.environ.pop("NB_SIMT_THREAD_ORDER", None)
+    # the switches took effect (the counters are cumulative): multi-CTA launches ran permuted, CTAs ran their threads reordered
+    for k, (cta_order, thread_order) in enumerate(ORDERS[1:], 1):
+        assert (counters[k][0] - counters[k - 1][0] > 30) == (cta_order != "natural"), ORDERS[k]
+        assert (counters[k][1] - counters[k - 1][1] > 100) == (thread_order != "natural"), ORDERS[k]
+    for k in range(1, len(ORDERS)):
+        assert len(results[k]) == len(results[0])
+        for i, (p, q) in enumerate(zip(results[0], results[k])):
+            assert np.array_equal(p, q), (ORDERS[k], i)
