@@ -521,10 +521,12 @@ def test_tiny_softening_and_repeatability(SIM, oracle):
 # (first item = CTA number, then the counter), its self-resetting counters, the scheduler's last-block pass and the fixed-order
 # reductions must give the same BITS whichever CTA comes first; and a shared-memory or global read that no barrier orders after
 # its write would see the old value in one of the thread orders (a poor man's racecheck: compute-sanitizer is closed on the
-# pool, profiles/r02_sanitizer.md).  Not covered: memory-model subtleties of real concurrent execution
+# pool, profiles/r02_sanitizer.md).  The bulk copies of the j-tiles land "early" (at issue: shows a stage overwritten while it is
+# still read) or "late" (NaN bytes at issue, data when the first thread waits on the mbarrier: shows a read that does not wait;
+# NB_SIMT_BULK_COPY).  Not covered: memory-model subtleties of real concurrent execution
 # ---------------------------------------------------------------------------------------------------------------
-ORDERS = [("natural", "natural"), ("reverse", "natural"), ("shuffle", "natural"), ("natural", "reverse"), ("natural", "shuffle"),
-          ("shuffle", "shuffle")]
+ORDERS = [("natural", "natural", "early"), ("reverse", "natural", "early"), ("shuffle", "natural", "early"), ("natural", "reverse", "early"),
+          ("natural", "shuffle", "early"), ("shuffle", "shuffle", "early"), ("natural", "natural", "late"), ("shuffle", "shuffle", "late")]
 
 
 @pytest.mark.parametrize("n_sms", [148, 3])
@@ -535,8 +537,8 @@ def test_results_do_not_depend_on_the_order_of_ctas_and_threads(SIM, n_sms):
     lists = [None] + [rng.choice(N, n, replace=False).astype(np.int32) for n in (1, 7, 40, 97, 300, 640)]
     results, counters = [], []
     try:
-        for cta_order, thread_order in ORDERS:
-            os.environ["NB_SIMT_CTA_ORDER"], os.environ["NB_SIMT_THREAD_ORDER"] = cta_order, thread_order
+        for cta_order, thread_order, bulk_copy in ORDERS:
+            os.environ["NB_SIMT_CTA_ORDER"], os.environ["NB_SIMT_THREAD_ORDER"], os.environ["NB_SIMT_BULK_COPY"] = cta_order, thread_order, bulk_copy
             g = SIM(m, x, v, eps, n_sms=n_sms)
             out = [g.nb_get_state(f) for f in ("A", "J", "S", "DT")]                     # startup: all-active launches
             g.nb_predict(2.0 ** -10)
@@ -548,16 +550,18 @@ def test_results_do_not_depend_on_the_order_of_ctas_and_threads(SIM, n_sms):
             t, n, act = g.nb_next_block()
             out += [np.array([t, n]), act]
             assert g.guards_intact()
-            g.L.nb_simt_permuted_launches.restype = g.L.nb_simt_reordered_ctas.restype = C.c_longlong
-            counters.append((g.L.nb_simt_permuted_launches(), g.L.nb_simt_reordered_ctas()))
+            g.L.nb_simt_permuted_launches.restype = g.L.nb_simt_reordered_ctas.restype = g.L.nb_simt_late_copies.restype = C.c_longlong
+            counters.append((g.L.nb_simt_permuted_launches(), g.L.nb_simt_reordered_ctas(), g.L.nb_simt_late_copies()))
             g.nb_free()
             results.append(out)
     finally:
-        os.environ.pop("NB_SIMT_CTA_ORDER", None); os.environ.pop("NB_SIMT_THREAD_ORDER", None)
-    # the switches took effect (the counters are cumulative): multi-CTA launches ran permuted, CTAs ran their threads reordered
-    for k, (cta_order, thread_order) in enumerate(ORDERS[1:], 1):
+        for name in ("NB_SIMT_CTA_ORDER", "NB_SIMT_THREAD_ORDER", "NB_SIMT_BULK_COPY"): os.environ.pop(name, None)
+    # the switches took effect (the counters are cumulative): multi-CTA launches ran permuted, CTAs ran their threads reordered,
+    # tiles arrived late
+    for k, (cta_order, thread_order, bulk_copy) in enumerate(ORDERS[1:], 1):
         assert (counters[k][0] - counters[k - 1][0] > 30) == (cta_order != "natural"), ORDERS[k]
         assert (counters[k][1] - counters[k - 1][1] > 100) == (thread_order != "natural"), ORDERS[k]
+        assert (counters[k][2] - counters[k - 1][2] > 1000) == (bulk_copy == "late"), ORDERS[k]
     for k in range(1, len(ORDERS)):
         assert len(results[k]) == len(results[0])
         for i, (p, q) in enumerate(zip(results[0], results[k])):
