@@ -137,8 +137,8 @@ def SIM(tmp_path_factory):
             self.L, self.host, self.device, self.N, self.ctx = L, True, 0, int(m.shape[0]), C.c_void_p()
             nbytes = L.nb_workspace_bytes(self.N)
             self._guard = (int(guard_bytes) + 255) // 256 * 256
-            self.workspace = np.empty(nbytes + 256 + 2 * self._guard, dtype=np.uint8)
-            self.workspace[:self._guard + 256] = 0xA5
+            self.workspace = np.full(nbytes + 256 + 2 * self._guard, 0xFF, dtype=np.uint8)      # the library gets NaNs and index -1:
+            self.workspace[:self._guard + 256] = 0xA5                                           # whatever it reads before writing shows
             self.workspace[-(self._guard + 256):] = 0xA5
             base = (self.workspace.ctypes.data + self._guard + 255) // 256 * 256
             self._ws_off, self._ws_bytes = base - self.workspace.ctypes.data, nbytes
