@@ -130,7 +130,7 @@ def SIM(tmp_path_factory):
         """binding.System's marshalling over the host build: numpy workspace (between two bands of 0xA5), host pointers"""
 
         def __init__(self, m, x, v, eps, n_sms=148, eta=0.0, eta_s=0.0, k_min=0, k_max=0, order=0, check_indices=0, precision=0,
-                     guard_bytes=1 << 16, skip_startup=False):
+                     guard_bytes=1 << 16, skip_startup=False, device_ptrs=False):
             os.environ["NB_SIMT_SMS"] = str(n_sms)
             os.environ.pop("NB_SIMT_SKIP_STARTUP", None)
             if skip_startup: os.environ["NB_SIMT_SKIP_STARTUP"] = "1"
@@ -142,7 +142,10 @@ def SIM(tmp_path_factory):
             self.workspace[-(self._guard + 256):] = 0xA5
             base = (self.workspace.ctypes.data + self._guard + 255) // 256 * 256
             self._ws_off, self._ws_bytes = base - self.workspace.ctypes.data, nbytes
-            self.cfg = B.nb_config(0, None, C.c_void_p(base), nbytes, 0, eta, eta_s, k_min, k_max, order, check_indices, precision)
+            # device_ptrs: the context is told that (h/d) pointers are DEVICE pointers (no staging copies, no synchronisation, index
+            # lists unverified unless asked for); on the host build device memory is host memory, so numpy arrays serve as both
+            self.cfg = B.nb_config(0, None, C.c_void_p(base), nbytes, 1 if device_ptrs else 0, eta, eta_s, k_min, k_max, order, check_indices,
+                                   precision)
             m, x, v = self._in(m, (self.N,)), self._in(x, (self.N, 3)), self._in(v, (self.N, 3))
             self._check(L.nb_init(C.byref(self.ctx), self.N, B._ptr(m), B._ptr(x), B._ptr(v), float(eps), C.byref(self.cfg)))
 
@@ -566,3 +569,39 @@ def test_results_do_not_depend_on_the_order_of_ctas_and_threads(SIM, n_sms):
         assert len(results[k]) == len(results[0])
         for i, (p, q) in enumerate(zip(results[0], results[k])):
             assert np.array_equal(p, q), (ORDERS[k], i)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# device-pointer contexts (nb_config.ptrs_on_device = 1) and the list nb_next_block leaves inside the context
+# (NB_ACTIVE_INTERNAL): same kernels, same plan as a host-pointer context with an explicit list - the same bits
+# ---------------------------------------------------------------------------------------------------------------
+def test_device_pointer_context_and_internal_active_list(SIM):
+    from paper_1411_5234_b200 import binding as B
+    N, eps = 900, 1e-3
+    m, x, v = W.plummer(N, 5, "kroupa")
+    gh, gd = SIM(m, x, v, eps), SIM(m, x, v, eps, device_ptrs=True)
+    for _ in range(6):
+        th, nh, acth = gh.nb_next_block()
+        td, nd, _ = gd.nb_next_block(want_list=False)
+        assert th == td and nh == nd
+        gh.nb_predict(th); gd.nb_predict(td)
+        fh, fd = gh.nb_force(acth), gd.nb_force(B.ACTIVE_INTERNAL, n_act=nd)
+        assert all(np.array_equal(a, b) for a, b in zip(fh, fd))
+        with pytest.raises(B.NBError) as e:
+            gd.nb_force(B.ACTIVE_INTERNAL, n_act=nd + 1)          # not the length of the internal list
+        assert e.value.status == B.NB_ESTATE
+        gh.nb_corrector(acth, 0.0); gd.nb_corrector(B.ACTIVE_INTERNAL, 0.0, n_act=nd)
+    td, nd, actd = gd.nb_next_block()                             # the list written through a "device" pointer
+    th, nh, acth = gh.nb_next_block()
+    assert td == th and np.array_equal(actd, acth)
+    for f in ("X", "V", "A", "J", "S", "C", "T", "DT"):
+        assert np.array_equal(gh.nb_get_state(f), gd.nb_get_state(f)), f
+    # index lists: the caller's contract by default in this mode, verified when asked for
+    gc = SIM(m, x, v, eps, device_ptrs=True, check_indices=1, skip_startup=True)
+    gc.nb_predict(0.0)
+    with pytest.raises(B.NBError) as e:
+        gc.nb_force(np.array([1, N + 5], dtype=np.int32))
+    assert e.value.status == B.NB_EINVAL
+    assert gc.nb_check_indices(acth) == B.NB_OK
+    assert gh.guards_intact() and gd.guards_intact() and gc.guards_intact()
+    gh.nb_free(); gd.nb_free(); gc.nb_free()
