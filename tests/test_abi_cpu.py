@@ -161,3 +161,32 @@ def test_product_path_has_no_oracle_or_cpu_fallback():
         from paper_1411_5234_b200 import binding
         with pytest.raises(RuntimeError):
             binding.System(np.ones(2), np.zeros((2, 3)), np.zeros((2, 3)), 1e-3)
+
+
+def test_plan_invariants_random_sizes(B):
+    """The same invariants on 3000 seeded random (N, n_act, n_sm), log-uniform up to the N <= 2^30 the library accepts: slices
+    cover the j-tiles with none empty, the launch fits the device, the partial sums fit the workspace, nothing that the kernels
+    index with int overflows (such plans must be refused with NB_EINVAL, and only far beyond the paper's sizes)."""
+    rng = np.random.default_rng(20260101)
+    p, L = B.nb_plan(), B.lib()
+    refused = 0
+    for _ in range(3000):
+        N = int(2 ** rng.uniform(0, 30))
+        n_act = max(1, min(N, int(2 ** rng.uniform(0, np.log2(N) + 0.01)))) if rng.random() < 0.8 else N
+        n_sm = int(rng.choice([1, 3, 8, 108, 132, 148, 160]))
+        rc = L.nb_plan_force(N, n_act, n_sm, C.byref(p))
+        if rc != B.NB_OK:
+            assert rc == B.NB_EINVAL and N > 1 << 24, (N, n_act, n_sm, rc)
+            refused += 1
+            continue
+        Npad = (N + 255) // 256 * 256
+        n_tiles = Npad // p.tile
+        S, st = p.n_split, p.slice_tiles
+        assert p.kernel in (0, 1) and p.n_units >= 1 and S >= 1 and st >= 1, (N, n_act, n_sm)
+        assert S * st >= n_tiles and (S - 1) * st < n_tiles, (N, n_act, n_sm)
+        assert 1 <= p.grid <= n_sm * p.ctas_per_sm, (N, n_act, n_sm)
+        rows = p.n_units * 128 if p.kernel == 0 else n_act
+        assert S * rows <= 8 * Npad + (1 << 19), (N, n_act, n_sm)
+        assert p.n_units * S < 2 ** 31 and rows < 2 ** 31, (N, n_act, n_sm)
+        assert n_act > 4096 or p.n_units == ((n_act + 127) // 128 if p.kernel == 0 else len(wu_units(n_act))), (N, n_act, n_sm)
+    assert refused < 300, refused
