@@ -4,6 +4,7 @@ validation) behaves.  No kernel is launched here."""
 import ctypes as C
 import os
 import re
+import subprocess
 
 import numpy as np
 import pytest
@@ -190,3 +191,31 @@ def test_plan_invariants_random_sizes(B):
         assert p.n_units * S < 2 ** 31 and rows < 2 ** 31, (N, n_act, n_sm)
         assert n_act > 4096 or p.n_units == ((n_act + 127) // 128 if p.kernel == 0 else len(wu_units(n_act))), (N, n_act, n_sm)
     assert refused < 300, refused
+
+
+def test_shipped_kernels_fit_the_occupancy_the_plan_assumes(B):
+    """The launch plan counts LI_CTAS_PER_SM = WU_CTAS_PER_SM = 4 resident CTAs of 128 threads per multiprocessor
+    (csrc/nb_internal.h); with 65536 registers that is at most 128 registers per thread.  Read from the machine code of the
+    shipped libnb.so (cuobjdump, no GPU): every force kernel fits, none has a local-memory frame beyond a few spill slots, and
+    the static shared memory of every kernel stays under the 48 KiB that needs no opt-in."""
+    import shutil
+    if shutil.which("cuobjdump") is None:
+        pytest.skip("cuobjdump (CUDA toolkit) is not on PATH")
+    B.lib()
+    out = subprocess.run(["cuobjdump", "--dump-resource-usage", B.LIB_PATH], stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+    assert out.returncode == 0, out.stdout[-2000:]
+    lines = out.stdout.split("\n")
+    usage = {}
+    for k, l in enumerate(lines):
+        m_ = re.match(r"\s*Function (\S+):", l)
+        if m_ and k + 1 < len(lines):
+            r = dict(kv.split(":") for kv in re.findall(r"\b(?:REG|STACK|SHARED|LOCAL):\d+", lines[k + 1]))
+            usage[m_.group(1)] = {key: int(val) for key, val in r.items()}
+    force = {n: u for n, u in usage.items() if re.search(r"force_(li|lim|wu|step)_kernel", n)}
+    assert len(force) >= 20, sorted(usage)                       # li / wu / step x eps x orders 4, 6, 8 + the mixed kernel x eps
+    for n, u in force.items():
+        assert u["REG"] <= 128, (n, u)                           # 4 CTAs x 128 threads x 128 registers = the register file
+        assert u["LOCAL"] == 0 and u["STACK"] <= 96, (n, u)
+    for n, u in usage.items():
+        assert u["SHARED"] <= 48 * 1024 and u["REG"] <= 255, (n, u)
+    assert any("reduce_correct_kernel" in n for n in usage) and any("sched_kernel" in n for n in usage) and any("predict_kernel" in n for n in usage)
