@@ -18,6 +18,7 @@ device.  Not covered: the machine code, timing, memory ordering, races between C
 import ctypes as C
 import os
 import re
+import shlex
 import subprocess
 
 import numpy as np
@@ -118,6 +119,9 @@ def SIM(tmp_path_factory):
     so = os.path.join(out, "libnb_simt_host.so")
     cmd = ["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-w", "-U_FORTIFY_SOURCE", "-D_FORTIFY_SOURCE=0", "-shared", "-fPIC", "-I" + SIMT, "-I" + CSRC,
            "-I" + os.path.join(ROOT, "include")] + srcs + [os.path.join(SIMT, "simt_switch.S"), "-o", so]
+    # NB_SIMT_CXXFLAGS: extra compiler flags for a one-off run, e.g. "-fsanitize=undefined -fno-sanitize-recover=undefined -g"
+    # (UBSan over the kernels' index arithmetic, shifts and alignment; profiles/r02_sanitizer.md)
+    cmd[1:1] = shlex.split(os.environ.get("NB_SIMT_CXXFLAGS", ""))
     r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     assert r.returncode == 0, r.stdout[-6000:]
     L = C.CDLL(so)
