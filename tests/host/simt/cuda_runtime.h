@@ -222,14 +222,41 @@ inline void run_cta(unsigned block, unsigned bid, unsigned grid)
     }
 }
 
+// Dynamic shared memory is one static array of the translation unit (the test's edit of `extern __shared__`), larger than any
+// launch asks for.  Under AddressSanitizer (NB_SIMT_CXXFLAGS=-fsanitize=address) every launch leaves only the bytes it asked
+// for addressable: an access to dynamic shared memory beyond the launch's size is then reported like one on the GPU would be by
+// compute-sanitizer's memcheck.  Without the sanitizer the two calls below do nothing.
+#if defined(__SANITIZE_ADDRESS__)
+extern "C" void __asan_poison_memory_region(void const volatile*, size_t);
+extern "C" void __asan_unpoison_memory_region(void const volatile*, size_t);
+#define NB_SIMT_POISON(p, n) __asan_poison_memory_region((p), (n))
+#define NB_SIMT_UNPOISON(p, n) __asan_unpoison_memory_region((p), (n))
+#else
+#define NB_SIMT_POISON(p, n) ((void)(p), (void)(n))
+#define NB_SIMT_UNPOISON(p, n) ((void)(p), (void)(n))
+#endif
+struct DynSmem { char* base = nullptr; size_t bytes = 0; };
+inline DynSmem& dyn_smem_array() { static DynSmem d; return d; }
+inline int register_dyn_smem(void* base, size_t bytes) { dyn_smem_array() = DynSmem{(char*)base, bytes}; return 0; }
+inline void bound_dyn_smem(size_t asked)
+{
+    DynSmem& d = dyn_smem_array();
+    if (!d.base) return;
+    if (asked > d.bytes) { fprintf(stderr, "simt: a launch asks for %zu bytes of dynamic shared memory\n", asked); abort(); }
+    const size_t lim = (asked + 7) / 8 * 8;                  // the sanitizer's granule
+    NB_SIMT_UNPOISON(d.base, d.bytes);
+    if (lim < d.bytes) NB_SIMT_POISON(d.base + lim, d.bytes - lim);
+}
+
 template <class... P, class... A>
-inline void launch(void (*kernel)(P...), long long grid, long long block, size_t /*smem*/, void* /*stream*/, A&&... args)
+inline void launch(void (*kernel)(P...), long long grid, long long block, size_t smem, void* /*stream*/, A&&... args)
 {
     State& s = S();
     std::tuple<std::decay_t<P>...> held(std::forward<A>(args)...);      // kernel arguments are passed by value
-    auto run = [kernel, grid, block, held]() {
+    auto run = [kernel, grid, block, smem, held]() {
         State& st = S();
         st.launches += 1;
+        bound_dyn_smem(smem);
         st.body = [kernel, &held]() { std::apply(kernel, held); };
         // The order in which a GPU starts and finishes the CTAs of a grid is not defined.  NB_SIMT_CTA_ORDER = reverse | shuffle
         // (a different permutation for every launch, reproducible) runs them in another order than 0, 1, 2, ...: work queues,

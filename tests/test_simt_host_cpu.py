@@ -87,7 +87,8 @@ def to_host_source(name, text):
         text = text.replace(fence, "")
         dyn = "extern __shared__ __align__(128) double2 dyn_smem[];"
         assert text.count(dyn) == 1
-        text = text.replace(dyn, "alignas(128) static double2 dyn_smem[16384];      // 256 KiB: more than any kernel asks for")
+        text = text.replace(dyn, "alignas(128) static double2 dyn_smem[16384];      // 256 KiB: more than any kernel asks for\n"
+                                 "static const int dyn_smem_registered = simt::register_dyn_smem(dyn_smem, sizeof dyn_smem);   // bounds per launch under ASan")
         inc = '#include "nb_internal.h"\n'
         assert text.count(inc) == 1
         text = text.replace(inc, inc + '#include "nb_force_shims.h"\n')
