@@ -160,12 +160,18 @@ inline void warp_barrier()
     }
 }
 
+struct DynSmem { char* base = nullptr; size_t bytes = 0, asked = 0; };
+inline DynSmem& dyn_smem_array() { static DynSmem d; return d; }
+inline int register_dyn_smem(void* base, size_t bytes) { dyn_smem_array() = DynSmem{(char*)base, bytes}; return 0; }
+
 // run one CTA to completion: round-robin over its fibres until all have exited
 inline void run_cta(unsigned block, unsigned bid, unsigned grid)
 {
     State& s = S();
     if (!s.stacks) s.stacks = (char*)aligned_alloc(4096, STACK_BYTES * MAX_THREADS);
     if (block > (unsigned)MAX_THREADS) { fprintf(stderr, "simt: block of %u threads\n", block); abort(); }
+    // a CTA finds garbage in its dynamic shared memory, not what the CTA before it left there: NaN bytes here
+    if (dyn_smem_array().base && dyn_smem_array().asked) memset(dyn_smem_array().base, 0xFF, dyn_smem_array().asked);
     Cta& c = s.cta;
     c.bid = uint3{bid, 0, 0}; c.bdim = uint3{block, 1, 1}; c.gdim = uint3{grid, 1, 1};
     c.alive = (int)block; c.arrived = 0; c.gen = 0;
@@ -235,15 +241,13 @@ extern "C" void __asan_unpoison_memory_region(void const volatile*, size_t);
 #define NB_SIMT_POISON(p, n) ((void)(p), (void)(n))
 #define NB_SIMT_UNPOISON(p, n) ((void)(p), (void)(n))
 #endif
-struct DynSmem { char* base = nullptr; size_t bytes = 0; };
-inline DynSmem& dyn_smem_array() { static DynSmem d; return d; }
-inline int register_dyn_smem(void* base, size_t bytes) { dyn_smem_array() = DynSmem{(char*)base, bytes}; return 0; }
 inline void bound_dyn_smem(size_t asked)
 {
     DynSmem& d = dyn_smem_array();
     if (!d.base) return;
     if (asked > d.bytes) { fprintf(stderr, "simt: a launch asks for %zu bytes of dynamic shared memory\n", asked); abort(); }
     const size_t lim = (asked + 7) / 8 * 8;                  // the sanitizer's granule
+    d.asked = asked;
     NB_SIMT_UNPOISON(d.base, d.bytes);
     if (lim < d.bytes) NB_SIMT_POISON(d.base + lim, d.bytes - lim);
 }
