@@ -537,8 +537,8 @@ ORDERS = [("natural", "natural", "early"), ("reverse", "natural", "early"), ("sh
           ("natural", "shuffle", "early"), ("shuffle", "shuffle", "early"), ("natural", "natural", "late"), ("shuffle", "shuffle", "late")]
 
 
-@pytest.mark.parametrize("n_sms", [148, 3])
-def test_results_do_not_depend_on_the_order_of_ctas_and_threads(SIM, n_sms):
+@pytest.mark.parametrize("n_sms,order", [(148, 6), (3, 6), (5, 8), (148, 4)])
+def test_results_do_not_depend_on_the_order_of_ctas_and_threads(SIM, n_sms, order):
     N, eps, t_end = 1100, 1e-4, 2.0 ** -7
     m, x, v = W.plummer(N, 606, "kroupa")
     rng = np.random.default_rng(6)
@@ -547,13 +547,14 @@ def test_results_do_not_depend_on_the_order_of_ctas_and_threads(SIM, n_sms):
     try:
         for cta_order, thread_order, bulk_copy in ORDERS:
             os.environ["NB_SIMT_CTA_ORDER"], os.environ["NB_SIMT_THREAD_ORDER"], os.environ["NB_SIMT_BULK_COPY"] = cta_order, thread_order, bulk_copy
-            g = SIM(m, x, v, eps, n_sms=n_sms)
+            g = SIM(m, x, v, eps, n_sms=n_sms, order=order)
             out = [g.nb_get_state(f) for f in ("A", "J", "S", "DT")]                     # startup: all-active launches
             g.nb_predict(2.0 ** -10)
             for idx in lists:
                 out += list(g.nb_force(idx))
+                if order == 8: out.append(g.nb_force_crackle(N if idx is None else idx.size))
             steps, t_last, n_sum = g.nb_run_blocks(t_end)
-            assert steps >= 5 and t_last == t_end
+            assert steps >= 3 and t_last == t_end
             out += [np.array([steps, n_sum])] + [g.nb_get_state(f) for f in ("X", "V", "A", "J", "S", "C", "T", "DT")]
             t, n, act = g.nb_next_block()
             out += [np.array([t, n]), act]
