@@ -9,6 +9,11 @@
 // barriers count the threads that have not exited; shuffles and votes exchange through a per-warp slot array between two warp
 // barriers.  Shared memory is `static` storage (CTAs do not overlap).  Global-memory atomics are plain operations.  Streams are
 // in order and synchronous; a stream capture records the launches as closures and a graph launch replays them.
+// Switches (environment, read at every launch): NB_SIMT_SMS = multiprocessors the device reports; NB_SIMT_CTA_ORDER = reverse |
+// shuffle and NB_SIMT_THREAD_ORDER = reverse | shuffle = the order in which CTAs of a grid run and threads of a CTA are resumed
+// (undefined on a GPU: results must not depend on it); NB_SIMT_BULK_COPY = late (nb_force_shims.h) = bulk copies land at the
+// first mbarrier wait instead of at issue.  Every CTA starts with 0xFF bytes in its dynamic shared memory; built with
+// -fsanitize=address (NB_SIMT_CXXFLAGS of the test) only the dynamic shared memory a launch asked for is addressable.
 // What it is not: a product path (nothing under paper_1411_5234_b200/ refers to it; the library refuses to run without a CUDA
 // device), a model of timing, of memory ordering or of races between CTAs, or a check of the machine code.  The GPU parity
 // tests (-m gpu) remain the proof for the B200.
