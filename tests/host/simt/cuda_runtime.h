@@ -12,7 +12,7 @@
 // Switches (environment, read at every launch): NB_SIMT_SMS = multiprocessors the device reports; NB_SIMT_CTA_ORDER = reverse |
 // shuffle and NB_SIMT_THREAD_ORDER = reverse | shuffle = the order in which CTAs of a grid run and threads of a CTA are resumed
 // (undefined on a GPU: results must not depend on it); NB_SIMT_BULK_COPY = late (nb_force_shims.h) = bulk copies land at the
-// first mbarrier wait instead of at issue.  Every CTA starts with 0xFF bytes in its dynamic shared memory; built with
+// first mbarrier wait instead of at issue.  Every CTA starts with 0xFF bytes in its dynamic and static shared memory; built with
 // -fsanitize=address (NB_SIMT_CXXFLAGS of the test) only the dynamic shared memory a launch asked for is addressable.
 // What it is not: a product path (nothing under paper_1411_5234_b200/ refers to it; the library refuses to run without a CUDA
 // device), a model of timing, of memory ordering or of races between CTAs, or a check of the machine code.  The GPU parity
@@ -43,7 +43,17 @@
 #define __forceinline__ inline
 #define __launch_bounds__(...)
 #define __align__(n) alignas(n)
+// static shared memory: static storage, collected in one section so that every CTA can be started with garbage in it (on the GPU a
+// CTA does not find zeros, nor what the CTA before it left).  Under AddressSanitizer plain statics instead: variables in a named
+// section get no red zones, and there the bounds are worth more than the garbage.
+#if defined(__SANITIZE_ADDRESS__)
 #define __shared__ static
+#else
+#define NB_SIMT_SMEM_SECTION 1
+#define __shared__ __attribute__((section("nb_smem"))) static
+extern "C" char __start_nb_smem[] __attribute__((weak, visibility("hidden")));
+extern "C" char __stop_nb_smem[] __attribute__((weak, visibility("hidden")));
+#endif
 
 struct alignas(16) double2 { double x, y; };
 struct alignas(32) double4 { double x, y, z, w; };
@@ -165,6 +175,10 @@ inline void warp_barrier()
     }
 }
 
+// static shared arrays inside TEMPLATE kernels do not follow the section attribute; the test appends a registration to their
+// declarations instead (first execution of the kernel), and run_cta fills what is registered
+inline std::vector<std::pair<char*, size_t>>& smem_regions() { static std::vector<std::pair<char*, size_t>> v; return v; }
+inline int register_smem(void* p, size_t n) { smem_regions().emplace_back((char*)p, n); return 0; }
 struct DynSmem { char* base = nullptr; size_t bytes = 0, asked = 0; };
 inline DynSmem& dyn_smem_array() { static DynSmem d; return d; }
 inline int register_dyn_smem(void* base, size_t bytes) { dyn_smem_array() = DynSmem{(char*)base, bytes}; return 0; }
@@ -176,6 +190,10 @@ inline void run_cta(unsigned block, unsigned bid, unsigned grid)
     if (!s.stacks) s.stacks = (char*)aligned_alloc(4096, STACK_BYTES * MAX_THREADS);
     if (block > (unsigned)MAX_THREADS) { fprintf(stderr, "simt: block of %u threads\n", block); abort(); }
     // a CTA finds garbage in its dynamic shared memory, not what the CTA before it left there: NaN bytes here
+    for (auto& r : smem_regions()) memset(r.first, 0xFF, r.second);
+#ifdef NB_SIMT_SMEM_SECTION
+    if (__start_nb_smem && __stop_nb_smem > __start_nb_smem) memset(__start_nb_smem, 0xFF, (size_t)(__stop_nb_smem - __start_nb_smem));
+#endif
     if (dyn_smem_array().base && dyn_smem_array().asked) memset(dyn_smem_array().base, 0xFF, dyn_smem_array().asked);
     Cta& c = s.cta;
     c.bid = uint3{bid, 0, 0}; c.bdim = uint3{block, 1, 1}; c.gdim = uint3{grid, 1, 1};

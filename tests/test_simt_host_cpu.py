@@ -102,6 +102,11 @@ def to_host_source(name, text):
         timer = 'asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));'
         assert text.count(timer) == 1
         text = text.replace(timer, "now = simt::clock_ns();")
+    # every static shared array with a single declarator registers itself with the stand-in, which fills it with 0xFF bytes before
+    # every CTA (a CTA finds garbage in shared memory on the GPU, not zeros and not its predecessor's values)
+    text, n_reg = re.subn(r"^(\s*)__shared__ ((?:alignas\(8\) )?[\w ]+?) (\w+)((?:\[\w+\])*);[ \t]*$",
+                          r"\1__shared__ \2 \3\4; static const int \3_registered_ = simt::register_smem(&\3, sizeof \3);", text, flags=re.M)
+    assert n_reg == {"nb_force.cu": 7, "nb_step.cu": 6}.get(name, 0), (name, n_reg)
     text = text.replace("__shared__ alignas(8)", "alignas(8) __shared__")      # g++ wants the attribute before `static`
     assert not re.search(r"\basm\b", re.sub(r"//.*", "", text)), name
     return text
