@@ -13,7 +13,10 @@ supplies their C++ meaning; `extern __shared__` becomes a static array; %globalt
 every one of these edits found its target.
 
 NOT a product path: nothing under paper_1411_5234_b200/ refers to this; binding.System still refuses to run without a CUDA
-device.  Not covered: the machine code, timing, memory ordering, races between CTAs (they run one after the other here).
+device.  Not covered: the machine code, timing, the memory model of truly concurrent CTAs.  CTAs run one after the other here,
+but in any order the test asks for, threads are resumed in any order, bulk copies land early or late, shared memory and the workspace
+start out as garbage (the switches are listed at the top of tests/host/simt/cuda_runtime.h); NB_SIMT_CXXFLAGS builds the library with
+a sanitizer (profiles/r02_sanitizer.md).
 """
 import ctypes as C
 import os
